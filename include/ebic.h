@@ -1,0 +1,148 @@
+/*
+ * ebic.h -- C ABI of libebic.so: EBIC population fitness evaluation and matched-row extraction
+ * on one NVIDIA B200 (sm_100a).
+ *
+ * The operation (PAPER.md = arXiv 1807.09932 text; line numbers refer to /root/reference/PAPER.md):
+ *   "EBIC search is driven by counting of rows, a greater or equal relation between the values in
+ *   columns" and missing values are "no longer counted towards the score of the bicluster"
+ *   (section 2 Methods, "Handling missing values"); up to 2^31-1 rows per GPU
+ *   and a population of up to 65,535 individuals, 1,600 typical ("Support for
+ *   Big Data").  The paper writes no formula; the exact definition used here is the one in
+ *   DESIGN.md section 3 (readings R1-R16), identical to the CPU oracle's header:
+ *
+ *     individual k = ordered column list c_0..c_{L-1} = col_ids[offsets[k] .. offsets[k+1])
+ *     ok(k,r)  = AND_{i<L-1} ( M[r][c_{i+1}] >= M[r][c_i] )        IEEE-754 ordered >= on float32
+ *                AND ( missing_mode == ON  =>  no M[r][c_i] is NaN )
+ *     count[k] = #{ r : ok(k,r) }             mask[k] bit r = ok(k,r)
+ *
+ * Conventions
+ *   - Every function returns a status code (EBIC_OK == 0).  Nothing throws, aborts or prints.
+ *   - "device" pointers are CUDA device (or managed) memory of the CURRENT device; "host or device"
+ *     pointers are classified with cudaPointerGetAttributes.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - The caller owns every buffer it passes.  The context owns its transposed copy of the matrix,
+ *     the NaN bitmask, the rank tiles and its scratch; the input matrix is not retained.
+ *   - One call in flight per context at a time (shared scratch).  Different contexts are independent.
+ *   - Bit layout of a mask: row r <-> 64-bit word r/64, bit r%64 (LSB first, little endian; the same
+ *     bytes viewed as uint8 have row r at byte r/8, bit r%8).  Bits >= rows are zero.
+ */
+#ifndef EBIC_H_
+#define EBIC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ebic_ctx ebic_ctx; /* opaque; owns device memory */
+
+enum {
+    EBIC_OK = 0,
+    EBIC_ERR_ARG = 1,         /* NULL / non-positive size / unknown mode / bad chosen index       */
+    EBIC_ERR_OOM = 2,         /* cudaMalloc failed                                                */
+    EBIC_ERR_CUDA = 3,        /* any other CUDA runtime error (no device, launch failure, ...)    */
+    EBIC_ERR_BAD_COLUMN = 4,  /* a column id outside [0, cols) was found on the device            */
+    EBIC_ERR_BAD_OFFSETS = 5  /* offsets[k] < 0, offsets[k+1] < offsets[k] or offsets[k+1] > n_ids */
+};
+enum { EBIC_MISSING_OFF = 0, EBIC_MISSING_ON = 1 };
+
+/* Kernel selection for ebic_eval_fitness (all give bit-identical counts). */
+enum {
+    EBIC_KERNEL_AUTO = 0,    /* fastest applicable: RANK8 if cols <= 127, else TILED_F32, else DIRECT */
+    EBIC_KERNEL_DIRECT = 1,  /* one thread per row, column-major global loads (any shape)          */
+    EBIC_KERNEL_TILED_F32 = 2, /* float32 row tiles staged in shared memory by TMA bulk copies    */
+    EBIC_KERNEL_RANK8 = 3    /* per-row order-preserving 8-bit rank tiles (cols <= 127)           */
+};
+
+/*
+ * Loader (a genes x samples matrix with optional missing values).
+ *   matrix        dense ROW-MAJOR float32 [rows][cols]; host or device pointer; any NaN = missing.
+ *   rows          1 .. 2^31-1.        cols  1 .. 2^31-1 (memory permitting).
+ *   missing_mode  EBIC_MISSING_OFF / EBIC_MISSING_ON.
+ *   out           receives the context.
+ * Transposes to column-major, builds the packed NaN bitmask and per-column non-missing counts and,
+ * when cols <= 127, the 8-bit rank tiles.  Synchronous: `matrix` may be freed on return.
+ * Errors: EBIC_ERR_ARG, EBIC_ERR_OOM, EBIC_ERR_CUDA (then *out == NULL).
+ */
+int ebic_create(const float *matrix, int64_t rows, int32_t cols, int32_t missing_mode,
+                ebic_ctx **out);
+
+/* Frees everything the context owns.  NULL is allowed. */
+int ebic_destroy(ebic_ctx *ctx);
+
+/*
+ * count[k] for the whole population (population CSR as in BASELINE.json north_star).
+ *   offsets  int32 [n_ind+1], col_ids int32 [n_ids]: host or device (both the same kind).
+ *   n_ind    0 .. 2^31-2 (0 is a no-op).   n_ids  number of entries of col_ids (>= offsets[n_ind]).
+ *   counts   uint64 [n_ind], host or device, overwritten.
+ * Asynchronous and stream-ordered when every pointer is a device pointer.  With host pointers the
+ * population is copied in and the counts copied out on `cuda_stream`, and the call returns after the
+ * stream has been synchronised.
+ * Population contents are validated on the device: an individual with a column id outside
+ * [0, cols) or with bad offsets gets count 0, the others are unaffected, and a sticky error
+ * (EBIC_ERR_BAD_COLUMN / EBIC_ERR_BAD_OFFSETS, the larger code wins) is kept for ebic_status().
+ * Returns host-detectable errors only (EBIC_ERR_ARG / _OOM / _CUDA).
+ */
+int ebic_eval_fitness(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_ids, int32_t n_ind,
+                      int64_t n_ids, uint64_t *counts, void *cuda_stream);
+
+/*
+ * Matched-row bitmasks (and optionally counts) of chosen individuals -- the rows of a bicluster
+ * (results are biclusters = rows + columns).
+ *   chosen   int32 [n_chosen] indices into the CSR population, host or device (same kind as offsets);
+ *            an index outside [0, n_ind) yields an all-zero mask and the sticky EBIC_ERR_BAD_OFFSETS.
+ *   masks    uint64 [n_chosen][ebic_mask_words(ctx)], host or device, overwritten.
+ *   counts   uint64 [n_chosen] or NULL.
+ * Same asynchrony, validation and error rules as ebic_eval_fitness.
+ */
+int ebic_extract_rows(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_ids, int32_t n_ind,
+                      int64_t n_ids, const int32_t *chosen, int32_t n_chosen, uint64_t *masks,
+                      uint64_t *counts, void *cuda_stream);
+
+/* ceil(rows / 64): uint64 words per mask.  -1 if ctx is NULL. */
+int64_t ebic_mask_words(const ebic_ctx *ctx);
+
+/*
+ * Synchronises `cuda_stream`, returns the sticky device error raised since the last ebic_status()
+ * (EBIC_OK if none) and clears it.  EBIC_ERR_CUDA if the stream itself reports an error.
+ */
+int ebic_status(ebic_ctx *ctx, void *cuda_stream);
+
+/* Selects the fitness kernel (EBIC_KERNEL_*).  EBIC_ERR_ARG if it cannot run this shape. */
+int ebic_set_kernel(ebic_ctx *ctx, int32_t kernel);
+
+/*
+ * Instrumentation for roofline accounting: when on, the tiled fitness kernels add the number of
+ * (row, column-visit) operand fetches they actually executed to a device counter (one extra global
+ * atomic per warp).  ebic_get_info(ctx, 10) synchronises the device, returns the counter and
+ * resets it.  Off by default; never on inside a timed region.
+ */
+int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
+
+/*
+ * Introspection for tests and the benchmark.  `what`:
+ *   0 rows, 1 cols, 2 padded leading dimension ld, 3 missing_mode, 4 kernel ebic_eval_fitness will
+ *   use, 5 rows per shared-memory tile of that kernel, 6 CTAs of its last launch, 7 SM count,
+ *   8 kernels launched by this context so far, 9 bytes of device memory the context owns,
+ *   10 executed column visits since the last read (see ebic_set_instrumentation).
+ * Returns -1 for NULL / unknown `what`.
+ */
+int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);
+
+/*
+ * Read-back of loader products for parity tests (synchronous D2H copies on the legacy stream).
+ *   ebic_debug_read(ctx, what, dst, dst_bytes): what = 0 column-major matrix float32 [cols][ld];
+ *   1 NaN bitmask uint32 [cols][ld/32]; 2 per-column non-missing counts uint64 [cols];
+ *   3 rank tiles uint8 [cols][ld] (EBIC_ERR_ARG if not built).
+ *   dst_bytes must equal the product's size.
+ */
+int ebic_debug_read(const ebic_ctx *ctx, int32_t what, void *dst, int64_t dst_bytes);
+
+/* Static string for a status code. */
+const char *ebic_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EBIC_H_ */

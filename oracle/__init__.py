@@ -52,11 +52,12 @@ def _load():
         u64p = ctypes.POINTER(ctypes.c_uint64)
         lib.oracle_eval_fitness.restype = ctypes.c_int
         lib.oracle_eval_fitness.argtypes = [f32p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
-                                            i32p, i32p, ctypes.c_int32, u64p, ctypes.c_int32]
+                                            i32p, i32p, ctypes.c_int32, ctypes.c_int64, u64p,
+                                            ctypes.c_int32]
         lib.oracle_extract_rows.restype = ctypes.c_int
         lib.oracle_extract_rows.argtypes = [f32p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int32,
-                                            i32p, i32p, ctypes.c_int32, i32p, ctypes.c_int32,
-                                            u64p, u64p]
+                                            i32p, i32p, ctypes.c_int32, ctypes.c_int64, i32p,
+                                            ctypes.c_int32, u64p, u64p]
         lib.oracle_max_threads.restype = ctypes.c_int
         lib.oracle_max_threads.argtypes = []
         _lib = lib
@@ -95,7 +96,7 @@ def eval_fitness(matrix, missing_mode, offsets, col_ids, n_threads: int = 0):
     ids_buf = ids if ids.size else np.zeros(1, dtype=np.int32)
     st = lib.oracle_eval_fitness(_ptr(m, ctypes.c_float), m.shape[0], m.shape[1], int(missing_mode),
                                  _ptr(off, ctypes.c_int32), _ptr(ids_buf, ctypes.c_int32), n_ind,
-                                 _ptr(counts, ctypes.c_uint64), int(n_threads))
+                                 ids.size, _ptr(counts, ctypes.c_uint64), int(n_threads))
     return int(st), counts
 
 
@@ -114,6 +115,6 @@ def extract_rows(matrix, missing_mode, offsets, col_ids, chosen):
     ch_buf = ch if ch.size else np.zeros(1, dtype=np.int32)
     st = lib.oracle_extract_rows(_ptr(m, ctypes.c_float), m.shape[0], m.shape[1], int(missing_mode),
                                  _ptr(off, ctypes.c_int32), _ptr(ids_buf, ctypes.c_int32), n_ind,
-                                 _ptr(ch_buf, ctypes.c_int32), ch.size,
+                                 ids.size, _ptr(ch_buf, ctypes.c_int32), ch.size,
                                  _ptr(masks, ctypes.c_uint64), _ptr(counts, ctypes.c_uint64))
     return int(st), masks, counts

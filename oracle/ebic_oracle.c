@@ -33,9 +33,10 @@
  *   R6  L = 0: vacuous truth, count = rows, mask all ones (tail bits zero), both modes.
  *   R7  duplicate columns are legal and get no special case.
  *   R8  column id outside [0, cols) -> that individual is invalid: count 0 / mask all zero, and the
- *       call returns ORACLE_ERR_BAD_COLUMN.  offsets[k] < 0 or offsets[k+1] < offsets[k] -> that
- *       individual is invalid the same way and the call returns ORACLE_ERR_BAD_OFFSETS.  If both
- *       kinds occur the larger code (BAD_OFFSETS) is returned.  Valid individuals are unaffected.
+ *       call returns ORACLE_ERR_BAD_COLUMN.  offsets[k] < 0, offsets[k+1] < offsets[k] or
+ *       offsets[k+1] > n_ids (the length of col_ids) -> that individual is invalid the same way
+ *       and the call returns ORACLE_ERR_BAD_OFFSETS.  If both kinds occur the larger code
+ *       (BAD_OFFSETS) is returned.  Valid individuals are unaffected.
  *   R9  -0.0 >= +0.0 and +0.0 >= -0.0 are true; infinities are ordinary values; denormals compare
  *       by value (no flush-to-zero: compile WITHOUT -ffast-math / -Ofast).
  *   R10 counts are uint64; all row arithmetic is int64.
@@ -95,11 +96,11 @@ static int oracle_row_ok(const float *row, const int32_t *ids, int32_t L, int32_
 }
 
 /* R8.  Returns 0 if individual k is well formed, else the error code it raises. */
-static int oracle_check_individual(const int32_t *offsets, const int32_t *col_ids, int32_t cols,
-                                   int32_t k)
+static int oracle_check_individual(const int32_t *offsets, const int32_t *col_ids, int64_t n_ids,
+                                   int32_t cols, int32_t k)
 {
     int32_t b = offsets[k], e = offsets[k + 1], i;
-    if (b < 0 || e < b)
+    if (b < 0 || e < b || (int64_t)e > n_ids)
         return ORACLE_ERR_BAD_OFFSETS;
     for (i = b; i < e; ++i)
         if (col_ids[i] < 0 || col_ids[i] >= cols)
@@ -118,16 +119,16 @@ int oracle_max_threads(void)
 
 /*
  * count[k] for every individual of the population.
- * M: host, row-major [rows][cols].  offsets: [n_ind+1].  col_ids: [offsets[n_ind]].
+ * M: host, row-major [rows][cols].  offsets: [n_ind+1].  col_ids: [n_ids].
  * counts: [n_ind], overwritten.  n_threads <= 0 -> all cores OpenMP reports.
  */
 int oracle_eval_fitness(const float *M, int64_t rows, int32_t cols, int32_t missing_mode,
                         const int32_t *offsets, const int32_t *col_ids, int32_t n_ind,
-                        uint64_t *counts, int32_t n_threads)
+                        int64_t n_ids, uint64_t *counts, int32_t n_threads)
 {
     int status = ORACLE_OK;
     int32_t k;
-    if (!M || rows <= 0 || cols <= 0 || n_ind < 0 ||
+    if (!M || rows <= 0 || cols <= 0 || n_ind < 0 || n_ids < 0 ||
         (missing_mode != ORACLE_MISSING_OFF && missing_mode != ORACLE_MISSING_ON))
         return ORACLE_ERR_ARG;
     if (n_ind == 0)
@@ -143,7 +144,7 @@ int oracle_eval_fitness(const float *M, int64_t rows, int32_t cols, int32_t miss
 
 #pragma omp parallel for schedule(dynamic, 1) num_threads(n_threads)
     for (k = 0; k < n_ind; ++k) {                         /* individuals (outer) */
-        int err = oracle_check_individual(offsets, col_ids, cols, k);
+        int err = oracle_check_individual(offsets, col_ids, n_ids, cols, k);
         uint64_t c = 0;
         if (err == ORACLE_OK) {
             const int32_t *ids = col_ids + offsets[k];
@@ -164,32 +165,32 @@ int oracle_eval_fitness(const float *M, int64_t rows, int32_t cols, int32_t miss
 /*
  * mask[j] (and optionally count[j]) for the chosen individuals chosen[0..n_chosen).
  * masks: [n_chosen][ceil(rows/64)] uint64, overwritten (R16).  counts may be NULL.
- * A chosen index outside [0, n_ind) is an argument error (nothing is written).
+ * A chosen index outside [0, n_ind) names no individual: its mask is all zero, its count 0 and the
+ * call returns ORACLE_ERR_BAD_OFFSETS (same treatment as an individual with bad offsets, R8).
  */
 int oracle_extract_rows(const float *M, int64_t rows, int32_t cols, int32_t missing_mode,
                         const int32_t *offsets, const int32_t *col_ids, int32_t n_ind,
-                        const int32_t *chosen, int32_t n_chosen, uint64_t *masks, uint64_t *counts)
+                        int64_t n_ids, const int32_t *chosen, int32_t n_chosen, uint64_t *masks,
+                        uint64_t *counts)
 {
     int status = ORACLE_OK;
     int64_t words;
     int32_t j;
-    if (!M || rows <= 0 || cols <= 0 || n_ind < 0 || n_chosen < 0 ||
+    if (!M || rows <= 0 || cols <= 0 || n_ind < 0 || n_ids < 0 || n_chosen < 0 ||
         (missing_mode != ORACLE_MISSING_OFF && missing_mode != ORACLE_MISSING_ON))
         return ORACLE_ERR_ARG;
     if (n_chosen == 0)
         return ORACLE_OK;
     if (!offsets || !chosen || !masks)
         return ORACLE_ERR_ARG;
-    for (j = 0; j < n_chosen; ++j)
-        if (chosen[j] < 0 || chosen[j] >= n_ind)
-            return ORACLE_ERR_ARG;
     words = (rows + 63) / 64;
 
     for (j = 0; j < n_chosen; ++j) {
         int32_t k = chosen[j];
         uint64_t *mask = masks + (int64_t)j * words;
         uint64_t c = 0;
-        int err = oracle_check_individual(offsets, col_ids, cols, k);
+        int err = (k < 0 || k >= n_ind) ? ORACLE_ERR_BAD_OFFSETS
+                                        : oracle_check_individual(offsets, col_ids, n_ids, cols, k);
         int64_t w, r;
         for (w = 0; w < words; ++w)
             mask[w] = 0;

@@ -1,0 +1,284 @@
+"""Thin Python binding over libebic.so (the C ABI of include/ebic.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library.  PyTorch is used for device
+memory and streams only.  If the library is missing or no CUDA device is present the calls raise
+-- there is no CPU fallback.
+
+Module-level functions carry the C names (`ebic_create`, `ebic_eval_fitness`, ...) and take raw
+pointers / sizes.  `Ebic` is the convenience wrapper the tests and bench.py use: it accepts torch
+CUDA tensors (device pointers) or numpy arrays / CPU tensors (host pointers) and passes their
+addresses straight through.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+from typing import Optional
+
+import numpy as np
+
+EBIC_OK = 0
+EBIC_ERR_ARG = 1
+EBIC_ERR_OOM = 2
+EBIC_ERR_CUDA = 3
+EBIC_ERR_BAD_COLUMN = 4
+EBIC_ERR_BAD_OFFSETS = 5
+EBIC_MISSING_OFF = 0
+EBIC_MISSING_ON = 1
+EBIC_KERNEL_AUTO = 0
+EBIC_KERNEL_DIRECT = 1
+EBIC_KERNEL_TILED_F32 = 2
+EBIC_KERNEL_RANK8 = 3
+KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8"}
+
+LIB_PATH = Path(__file__).resolve().parent / "libebic.so"
+
+# every symbol include/ebic.h declares: (restype, argtypes)
+_vp, _i32, _i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+SYMBOLS = {
+    "ebic_create": (ctypes.c_int, [_vp, _i64, _i32, _i32, ctypes.POINTER(_vp)]),
+    "ebic_destroy": (ctypes.c_int, [_vp]),
+    "ebic_eval_fitness": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _vp]),
+    "ebic_extract_rows": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _i32, _vp, _vp, _vp]),
+    "ebic_mask_words": (_i64, [_vp]),
+    "ebic_status": (ctypes.c_int, [_vp, _vp]),
+    "ebic_set_kernel": (ctypes.c_int, [_vp, _i32]),
+    "ebic_set_instrumentation": (ctypes.c_int, [_vp, _i32]),
+    "ebic_get_info": (_i64, [_vp, _i32]),
+    "ebic_debug_read": (ctypes.c_int, [_vp, _i32, _vp, _i64]),
+    "ebic_strerror": (ctypes.c_char_p, [ctypes.c_int]),
+}
+
+_lib = None
+
+
+class EbicError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: status {status} ({strerror(status)})")
+
+
+def load_library() -> ctypes.CDLL:
+    """Load libebic.so; raises (loudly) when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not LIB_PATH.exists():
+            raise FileNotFoundError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1807_09932_b200.csrc.build` "
+                "(there is no CPU fallback)")
+        lib = ctypes.CDLL(str(LIB_PATH))
+        for name, (res, args) in SYMBOLS.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def strerror(status: int) -> str:
+    try:
+        return load_library().ebic_strerror(int(status)).decode()
+    except Exception:
+        return "?"
+
+
+# ---------------------------------------------------------------- C names, raw pointers
+def ebic_create(matrix_ptr: int, rows: int, cols: int, missing_mode: int) -> int:
+    out = _vp()
+    st = load_library().ebic_create(matrix_ptr, rows, cols, missing_mode, ctypes.byref(out))
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_create")
+    return out.value
+
+
+def ebic_destroy(ctx: int) -> None:
+    load_library().ebic_destroy(ctx)
+
+
+def ebic_eval_fitness(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, counts_ptr, stream=0) -> None:
+    st = load_library().ebic_eval_fitness(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, counts_ptr, stream)
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_eval_fitness")
+
+
+def ebic_extract_rows(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, chosen_ptr, n_chosen, masks_ptr,
+                      counts_ptr, stream=0) -> None:
+    st = load_library().ebic_extract_rows(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, chosen_ptr, n_chosen,
+                                          masks_ptr, counts_ptr, stream)
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_extract_rows")
+
+
+def ebic_mask_words(ctx) -> int:
+    return int(load_library().ebic_mask_words(ctx))
+
+
+def ebic_status(ctx, stream=0) -> int:
+    return int(load_library().ebic_status(ctx, stream))
+
+
+def ebic_set_kernel(ctx, kernel: int) -> None:
+    st = load_library().ebic_set_kernel(ctx, kernel)
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_set_kernel")
+
+
+def ebic_set_instrumentation(ctx, on: bool) -> None:
+    load_library().ebic_set_instrumentation(ctx, 1 if on else 0)
+
+
+def ebic_get_info(ctx, what: int) -> int:
+    return int(load_library().ebic_get_info(ctx, what))
+
+
+def ebic_debug_read(ctx, what: int, dst: np.ndarray) -> None:
+    st = load_library().ebic_debug_read(ctx, what, dst.ctypes.data, dst.nbytes)
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_debug_read")
+
+
+# ---------------------------------------------------------------- convenience wrapper
+def _require_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("ebic-b200 needs a CUDA device (B200, sm_100a); there is no CPU fallback")
+    return torch
+
+
+def _ptr(a) -> int:
+    """Address of a torch tensor (CPU or CUDA) or numpy array; the array must be contiguous."""
+    if a is None:
+        return 0
+    if isinstance(a, np.ndarray):
+        if not a.flags.c_contiguous:
+            raise ValueError("array must be C-contiguous")
+        return a.ctypes.data
+    if not a.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    return a.data_ptr()
+
+
+def _is_cuda(a) -> bool:
+    return (not isinstance(a, np.ndarray)) and a.is_cuda
+
+
+def _stream_handle(stream) -> int:
+    torch = _require_cuda()
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+class Ebic:
+    """One loaded matrix (ebic_ctx).  matrix: float32 [rows][cols], torch CUDA/CPU tensor or numpy."""
+
+    def __init__(self, matrix, missing_mode: int):
+        torch = _require_cuda()
+        load_library()
+        if isinstance(matrix, np.ndarray):
+            if matrix.dtype != np.float32 or matrix.ndim != 2:
+                raise ValueError("matrix must be float32 [rows][cols]")
+            matrix = np.ascontiguousarray(matrix)
+        else:
+            if matrix.dtype != torch.float32 or matrix.dim() != 2:
+                raise ValueError("matrix must be float32 [rows][cols]")
+            matrix = matrix.contiguous()
+            if matrix.is_cuda:
+                torch.cuda.current_stream().synchronize()      # ebic_create runs on the legacy stream
+        self.rows, self.cols = int(matrix.shape[0]), int(matrix.shape[1])
+        self.missing_mode = int(missing_mode)
+        self._ctx = ebic_create(_ptr(matrix), self.rows, self.cols, self.missing_mode)
+        self.mask_words = ebic_mask_words(self._ctx)
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_ctx", None):
+            ebic_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- the two hot calls
+    def eval_fitness(self, offsets, col_ids, counts=None, stream=None):
+        """counts (uint64 bit pattern in an int64 tensor / uint64 numpy array) for the whole population.
+
+        Device tensors in -> device tensor out, asynchronous on `stream` (default: torch's current
+        stream).  numpy / CPU tensors in -> numpy uint64 out, synchronous (host buffers, the copies
+        happen inside the call).
+        """
+        torch = _require_cuda()
+        n_ind = int(offsets.shape[0]) - 1
+        n_ids = int(col_ids.shape[0])
+        if _is_cuda(offsets):
+            if counts is None:
+                counts = torch.empty(n_ind, dtype=torch.int64, device=offsets.device)
+        elif counts is None:
+            counts = np.empty(n_ind, dtype=np.uint64)
+        ebic_eval_fitness(self._ctx, _ptr(offsets), _ptr(col_ids), n_ind, n_ids, _ptr(counts),
+                          _stream_handle(stream))
+        return counts
+
+    def extract_rows(self, offsets, col_ids, chosen, masks=None, counts=None, want_counts=True, stream=None):
+        """(masks [n_chosen][mask_words], counts [n_chosen] or None) for the chosen individuals."""
+        torch = _require_cuda()
+        n_ind = int(offsets.shape[0]) - 1
+        n_ids = int(col_ids.shape[0])
+        n_chosen = int(chosen.shape[0])
+        if _is_cuda(offsets):
+            if masks is None:
+                masks = torch.empty((n_chosen, self.mask_words), dtype=torch.int64, device=offsets.device)
+            if counts is None and want_counts:
+                counts = torch.empty(n_chosen, dtype=torch.int64, device=offsets.device)
+        else:
+            if masks is None:
+                masks = np.empty((n_chosen, self.mask_words), dtype=np.uint64)
+            if counts is None and want_counts:
+                counts = np.empty(n_chosen, dtype=np.uint64)
+        ebic_extract_rows(self._ctx, _ptr(offsets), _ptr(col_ids), n_ind, n_ids, _ptr(chosen), n_chosen,
+                          _ptr(masks), _ptr(counts), _stream_handle(stream))
+        return masks, counts
+
+    # -- status / knobs / introspection
+    def status(self, stream=None) -> int:
+        return ebic_status(self._ctx, _stream_handle(stream))
+
+    def set_kernel(self, kernel: int) -> None:
+        ebic_set_kernel(self._ctx, kernel)
+
+    def set_instrumentation(self, on: bool) -> None:
+        ebic_set_instrumentation(self._ctx, on)
+
+    def info(self, what: int) -> int:
+        return ebic_get_info(self._ctx, what)
+
+    @property
+    def ld(self) -> int:
+        return self.info(2)
+
+    @property
+    def kernel(self) -> int:
+        return self.info(4)
+
+    def debug_read(self, what: int) -> np.ndarray:
+        ld, cols = self.ld, self.cols
+        if what == 0:
+            dst = np.empty((cols, ld), dtype=np.float32)
+        elif what == 1:
+            dst = np.empty((cols, ld // 32), dtype=np.uint32)
+        elif what == 2:
+            dst = np.empty(cols, dtype=np.uint64)
+        elif what == 3:
+            dst = np.empty((cols, ld), dtype=np.uint8)
+        else:
+            raise ValueError(what)
+        ebic_debug_read(self._ctx, what, dst)
+        return dst

@@ -1,0 +1,111 @@
+// extract_kernels.cuh -- SURVEY.md 8(a) row a7: matched-row bitmask (and count) of chosen individuals.
+// results are biclusters = rows + columns; the rows of an individual are the rows
+// for which ok(k,r) of include/ebic.h holds.  HBM-bound: reads 4*L bytes per row, writes 1/8 byte.
+//
+// Bit layout: row r <-> uint32 word r/32, bit r%32 (== little-endian uint64 word r/64, bit r%64).
+// A warp covers 128 consecutive rows per step: lane l evaluates rows base + 32*w + l for w = 0..3, so
+// the ballot of predicate w IS mask word w and every column load is one coalesced 128-byte request.
+#pragma once
+#include "ebic_device.cuh"
+
+namespace ebic {
+
+constexpr int kExtractMaxSmemIds = 1024;
+
+// grid.x over row chunks (rows_per_block = 8 warps * 128 rows * kExtractSteps), grid.y over chosen.
+constexpr int kExtractSteps = 4;
+constexpr int kExtractRowsPerBlock = 8 * 128 * kExtractSteps;
+
+__global__ void __launch_bounds__(256)
+extract_rows_kernel(const float* __restrict__ Mc, int64_t ld, int64_t rows, int32_t cols, int32_t missing_on,
+                    const uint32_t* __restrict__ nanmask, const int32_t* __restrict__ offsets,
+                    const int32_t* __restrict__ col_ids, int32_t n_ind, int64_t n_ids,
+                    const int32_t* __restrict__ chosen, int32_t n_chosen, uint32_t* __restrict__ masks32,
+                    int64_t words32, unsigned long long* __restrict__ counts, int32_t* __restrict__ err)
+{
+    __shared__ int32_t s_ids[kExtractMaxSmemIds];
+    __shared__ int32_t s_bad;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t ldw = ld / 32;
+    const int64_t w_block = static_cast<int64_t>(blockIdx.x) * (kExtractRowsPerBlock / 32);
+
+    for (int32_t j = blockIdx.y; j < n_chosen; j += gridDim.y) {
+        // ---- validate the chosen individual (every block does it; L is small) ----
+        if (tid == 0) s_bad = 0;
+        __syncthreads();
+        const int32_t k = chosen[j];
+        int32_t b = 0, L = -1;
+        int bad = 0;
+        if (k < 0 || k >= n_ind) {
+            bad = 5;
+        } else {
+            b = offsets[k];
+            const int32_t e = offsets[k + 1];
+            if (b < 0 || e < b || static_cast<int64_t>(e) > n_ids) bad = 5;
+            else L = e - b;
+        }
+        if (!bad) {
+            for (int32_t i = tid; i < L; i += 256) {
+                const int32_t id = col_ids[b + i];
+                if (id < 0 || id >= cols) s_bad = 4;             // benign race: same value
+                else if (i < kExtractMaxSmemIds) s_ids[i] = id;
+            }
+        }
+        __syncthreads();
+        if (!bad) bad = s_bad;
+        if (bad && tid == 0 && blockIdx.x == 0) atomicMax(err, bad);
+        const int32_t* gids = col_ids + b;
+
+        uint32_t* out = masks32 + static_cast<int64_t>(j) * words32;
+        unsigned int local = 0;
+        for (int step = 0; step < kExtractSteps; ++step) {
+            const int64_t w0 = w_block + (step * 8 + warp) * 4;   // first of this warp's 4 words
+            if (w0 >= words32) break;
+            unsigned int word = 0;                                 // lane w (< 4) ends up with word w
+            if (bad) {
+                word = 0;
+            } else if (L >= 2) {
+                const float* base = Mc + w0 * 32 + lane;
+                const int32_t id0 = (0 < kExtractMaxSmemIds) ? s_ids[0] : gids[0];
+                const float* c0 = base + static_cast<int64_t>(id0) * ld;
+                float v0 = c0[0], v1 = c0[32], v2 = c0[64], v3 = c0[96];
+                bool p0 = true, p1 = true, p2 = true, p3 = true;
+                for (int32_t i = 1; i < L; ++i) {
+                    const int32_t id = (i < kExtractMaxSmemIds) ? s_ids[i] : __ldg(&gids[i]);
+                    const float* c = base + static_cast<int64_t>(id) * ld;
+                    const float u0 = c[0], u1 = c[32], u2 = c[64], u3 = c[96];
+                    p0 = p0 & (u0 >= v0);
+                    p1 = p1 & (u1 >= v1);
+                    p2 = p2 & (u2 >= v2);
+                    p3 = p3 & (u3 >= v3);
+                    v0 = u0; v1 = u1; v2 = u2; v3 = u3;
+                }
+                const unsigned int b0 = __ballot_sync(0xffffffffu, p0);
+                const unsigned int b1 = __ballot_sync(0xffffffffu, p1);
+                const unsigned int b2 = __ballot_sync(0xffffffffu, p2);
+                const unsigned int b3 = __ballot_sync(0xffffffffu, p3);
+                word = lane == 0 ? b0 : lane == 1 ? b1 : lane == 2 ? b2 : b3;
+            } else if (lane < 4) {
+                // L <= 1: closed form.  Valid rows of word w: [32w, min(rows, 32w+32)).
+                const int64_t w = w0 + lane;
+                const int64_t left = rows - w * 32;
+                const unsigned int valid = left >= 32 ? 0xffffffffu : left <= 0 ? 0u : ((1u << left) - 1u);
+                if (L == 1 && missing_on && w < ldw)
+                    word = ~nanmask[static_cast<int64_t>(s_ids[0]) * ldw + w] & valid;
+                else
+                    word = valid;
+            }
+            if (lane < 4 && w0 + lane < words32) {
+                out[w0 + lane] = word;
+                local += __popc(word);
+            }
+        }
+        if (counts != nullptr) {
+            local = __reduce_add_sync(0xffffffffu, local);
+            if (lane == 0 && local) atomicAdd(&counts[j], static_cast<unsigned long long>(local));
+        }
+        __syncthreads();                                           // s_ids / s_bad are reused for the next j
+    }
+}
+
+}  // namespace ebic

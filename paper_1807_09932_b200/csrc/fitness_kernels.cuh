@@ -1,0 +1,341 @@
+// fitness_kernels.cuh -- SURVEY.md 8(a) rows a3 (population ingest), a4 (tile staging),
+// a5 (trend predicate) and a6 (count accumulation).
+//
+// Definition (include/ebic.h): count[k] = #{ r : AND_i M[r][c_{i+1}] >= M[r][c_i]
+// and, in missing mode, no M[r][c_i] is NaN }.  For L >= 2 an ordered >= is already false on NaN, so
+// the chain kernels need no NaN test and no mode; L <= 1 has a closed form from the loader's
+// per-column non-missing counts and is resolved by the ingest kernel.  Padding rows are NaN / 0x7F.
+#pragma once
+#include "ebic_device.cuh"
+
+namespace ebic {
+
+// ------------------------------------------------------------------------------------------------
+// a3  Population ingest + validation.  One thread per individual.
+//   meta[k] = { slot4, L }   slot4 = index (in int4 units) of the individual's padded id group in `pids`
+//                            L = chromosome length, or -1 if the individual is invalid.
+//   pids    = ids copied to a 16-byte aligned slot, padded to a multiple of 4 with the last id, so the
+//             chain kernels fetch four ids with one uniform 128-bit load.  Slot of individual k starts
+//             at (offsets[k] + 3k) & ~3: disjoint from its neighbours without a prefix sum.
+//   counts[k] is initialised: rows (L = 0, or L = 1 in mode OFF), non-missing rows of the column
+//             (L = 1, mode ON), else 0 -- the chain kernels then add to it.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __restrict__ col_ids,
+                         int32_t n_ind, int64_t n_ids, int32_t cols, int64_t rows, int32_t missing_on,
+                         const unsigned long long* __restrict__ nonmissing, int2* __restrict__ meta,
+                         int32_t* __restrict__ pids, unsigned long long* __restrict__ counts,
+                         int32_t* __restrict__ err)
+{
+    const int32_t k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_ind) return;
+    const int32_t b = offsets[k], e = offsets[k + 1];
+    if (b < 0 || e < b || static_cast<int64_t>(e) > n_ids) {
+        meta[k] = make_int2(0, -1);
+        counts[k] = 0;
+        atomicMax(err, 5 /* EBIC_ERR_BAD_OFFSETS */);
+        return;
+    }
+    const int32_t L = e - b;
+    const int64_t slot = (static_cast<int64_t>(b) + 3ll * k) & ~3ll;
+    bool bad = false;
+    int32_t last = 0;
+    for (int32_t i = 0; i < L; ++i) {
+        int32_t id = col_ids[b + i];
+        if (id < 0 || id >= cols) {
+            bad = true;
+            id = 0;
+        }
+        pids[slot + i] = id;
+        last = id;
+    }
+    for (int32_t i = L; i < ((L + 3) & ~3); ++i) pids[slot + i] = last;
+    if (bad) {
+        meta[k] = make_int2(static_cast<int32_t>(slot >> 2), -1);
+        counts[k] = 0;
+        atomicMax(err, 4 /* EBIC_ERR_BAD_COLUMN */);
+        return;
+    }
+    meta[k] = make_int2(static_cast<int32_t>(slot >> 2), L);
+    unsigned long long c = 0;
+    if (L == 0) c = static_cast<unsigned long long>(rows);
+    else if (L == 1) c = missing_on ? nonmissing[last] : static_cast<unsigned long long>(rows);
+    counts[k] = c;
+}
+
+// ------------------------------------------------------------------------------------------------
+// DIRECT kernel: one thread per row, column-major global loads, ballot + popc, one global atomic
+// per warp and individual.  Any shape; the simple GPU witness the tiled kernels are diffed against.
+// grid.x = ld / 256 row blocks, grid.y = population slices.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+fitness_direct_kernel(const float* __restrict__ Mc, int64_t ld, const int2* __restrict__ meta,
+                      const int32_t* __restrict__ pids, int32_t n_ind,
+                      unsigned long long* __restrict__ counts)
+{
+    const int64_t r = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;   // < ld; padding is NaN
+    const int lane = threadIdx.x & 31;
+    const int32_t per = (n_ind + gridDim.y - 1) / gridDim.y;
+    const int32_t k_begin = blockIdx.y * per;
+    const int32_t k_end = min(n_ind, k_begin + per);
+    for (int32_t k = k_begin; k < k_end; ++k) {
+        const int2 m = __ldg(&meta[k]);
+        if (m.y < 2) continue;
+        const int32_t* ids = pids + 4ll * m.x;
+        float prev = Mc[static_cast<int64_t>(__ldg(&ids[0])) * ld + r];
+        bool ok = true;
+        for (int32_t i = 1; i < m.y; ++i) {
+            const float cur = Mc[static_cast<int64_t>(__ldg(&ids[i])) * ld + r];
+            ok = ok & (cur >= prev);
+            prev = cur;
+        }
+        const unsigned int c = __popc(__ballot_sync(0xffffffffu, ok));
+        if (lane == 0 && c) atomicAdd(&counts[k], static_cast<unsigned long long>(c));
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Tiled kernels (TILED_F32 and RANK8): persistent CTAs, one per SM.
+//
+// Work space = (row tile t, individual k) pairs in tile-major order; CTA b owns the contiguous
+// range [P*b/G, P*(b+1)/G), P = n_tiles * n_ind: equal shares whatever the shape, and every tile is
+// loaded by at most (its share of CTAs) + 1 CTAs.  Warp `n_cons` is the producer: for every tile of
+// the CTA's range it waits for the buffer to be released, arms the "full" mbarrier with the tile's
+// byte count and issues one TMA bulk copy per column (T contiguous rows of a column-major column).
+// Consumer warps wait on "full", each takes every n_cons-th individual of the tile's range,
+// evaluates it on all slabs of the tile, warp-reduces the count and adds it to the CTA's
+// shared-memory counter of that individual; then releases the buffer ("empty" mbarrier, one arrival
+// per consumer warp).  Counters are flushed with one 64-bit global atomic per (CTA, individual).
+// Per-CTA counters are uint32: a CTA sees < 2^31 rows, so they cannot overflow.
+// ------------------------------------------------------------------------------------------------
+struct TiledParams {
+    const void* M;                   // column-major [cols][ld] (float or uint8 ranks)
+    int64_t ld;
+    int32_t cols;
+    int32_t T;                       // rows per tile (multiple of the slab size)
+    int64_t n_tiles;                 // ceil(ld / T)
+    const int2* meta;                // [n_ind] of this launch's population chunk
+    const int4* pids4;
+    int32_t n_ind;                   // individuals in this launch (<= kMaxIndPerLaunch)
+    unsigned long long* counts;      // [n_ind]
+    unsigned long long* visits;      // executed column visits (instrumented build) or nullptr
+};
+
+constexpr int kMaxIndPerLaunch = 8192;
+constexpr int kSmemHeader = 128;     // 4 mbarriers, padded
+
+__host__ __device__ inline size_t tiled_smem_bytes(int32_t cols, int32_t T, int32_t elem, int32_t n_ind) {
+    size_t cnt = (static_cast<size_t>(n_ind) * 4 + 127) & ~static_cast<size_t>(127);
+    return kSmemHeader + cnt + 2 * static_cast<size_t>(cols) * T * elem;
+}
+
+// ---- a5 on float32: 4 rows per lane, one LDS.128 + 4 FSETP.GE.AND per column -------------------
+__device__ __forceinline__ int chain_f32(const float* base, int32_t T, int4 g, const int4* gp, int32_t L)
+{
+    float4 prev = *reinterpret_cast<const float4*>(base + g.x * T);
+    bool p0 = true, p1 = true, p2 = true, p3 = true;
+#define EBIC_STEP_F32(ID)                                                         \
+    {                                                                             \
+        const float4 cur = *reinterpret_cast<const float4*>(base + (ID) * T);     \
+        p0 = p0 & (cur.x >= prev.x);                                              \
+        p1 = p1 & (cur.y >= prev.y);                                              \
+        p2 = p2 & (cur.z >= prev.z);                                              \
+        p3 = p3 & (cur.w >= prev.w);                                              \
+        prev = cur;                                                               \
+    }
+    EBIC_STEP_F32(g.y);
+    if (L > 2) {
+        EBIC_STEP_F32(g.z);
+        if (L > 3) EBIC_STEP_F32(g.w);
+    }
+    for (int32_t i = 4; i < L; i += 4) {
+        g = __ldg(++gp);
+        EBIC_STEP_F32(g.x);
+        if (i + 1 < L) {
+            EBIC_STEP_F32(g.y);
+            if (i + 2 < L) {
+                EBIC_STEP_F32(g.z);
+                if (i + 3 < L) EBIC_STEP_F32(g.w);
+            }
+        }
+    }
+#undef EBIC_STEP_F32
+    return static_cast<int>(p0) + static_cast<int>(p1) + static_cast<int>(p2) + static_cast<int>(p3);
+}
+
+// ---- a5 on rank codes: 16 rows per lane and slab, NS slabs per id fetch ------------------------
+// code = 0x80|rank (rank <= 126) or 0x7F (missing).  Per byte: cur - prev + 0x80 stays in [1, 255]
+// for every code pair, so the 32-bit IADD3 never carries between bytes, and its bit 7 is set iff
+// rank(cur) >= rank(prev) when both are values.  AND-ing with `cur` clears bit 7 when cur is missing;
+// a missing prev was already cleared one step earlier (acc starts as the first column's code).
+template <int NS>
+__device__ __forceinline__ int chain_r8(const uint8_t* base, int32_t T, int4 g, const int4* gp, int32_t L)
+{
+    constexpr unsigned int H = 0x80808080u;
+    uint4 prev[NS], acc[NS];
+    {
+        const uint8_t* col = base + g.x * T;
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            prev[s] = *reinterpret_cast<const uint4*>(col + s * kRowsPerSlabR8);
+            acc[s] = prev[s];
+        }
+    }
+#define EBIC_STEP_R8(ID)                                                                   \
+    {                                                                                      \
+        const uint8_t* col = base + (ID) * T;                                              \
+        _Pragma("unroll") for (int s = 0; s < NS; ++s) {                                   \
+            const uint4 cur = *reinterpret_cast<const uint4*>(col + s * kRowsPerSlabR8);   \
+            acc[s].x &= (cur.x - prev[s].x + H) & cur.x;                                   \
+            acc[s].y &= (cur.y - prev[s].y + H) & cur.y;                                   \
+            acc[s].z &= (cur.z - prev[s].z + H) & cur.z;                                   \
+            acc[s].w &= (cur.w - prev[s].w + H) & cur.w;                                   \
+            prev[s] = cur;                                                                 \
+        }                                                                                  \
+    }
+    EBIC_STEP_R8(g.y);
+    if (L > 2) {
+        EBIC_STEP_R8(g.z);
+        if (L > 3) EBIC_STEP_R8(g.w);
+    }
+    for (int32_t i = 4; i < L; i += 4) {
+        g = __ldg(++gp);
+        EBIC_STEP_R8(g.x);
+        if (i + 1 < L) {
+            EBIC_STEP_R8(g.y);
+            if (i + 2 < L) {
+                EBIC_STEP_R8(g.z);
+                if (i + 3 < L) EBIC_STEP_R8(g.w);
+            }
+        }
+    }
+#undef EBIC_STEP_R8
+    int total = 0;
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const unsigned int m = (acc[s].x & H) | ((acc[s].y & H) >> 1) | ((acc[s].z & H) >> 2) | ((acc[s].w & H) >> 3);
+        total += __popc(m);
+    }
+    return total;
+}
+
+struct ElemF32 {
+    using type = float;
+    static constexpr int kSlabRows = kRowsPerSlabF32;
+    static constexpr int kLaneElems = 4;
+};
+struct ElemR8 {
+    using type = uint8_t;
+    static constexpr int kSlabRows = kRowsPerSlabR8;
+    static constexpr int kLaneElems = 16;
+};
+
+template <class E>
+__device__ __forceinline__ int eval_individual_on_tile(const typename E::type* tile, int32_t T, int32_t nslabs,
+                                                        int lane, int4 g0, const int4* gp, int32_t L);
+
+template <>
+__device__ __forceinline__ int eval_individual_on_tile<ElemF32>(const float* tile, int32_t T, int32_t nslabs,
+                                                                int lane, int4 g0, const int4* gp, int32_t L)
+{
+    int cnt = 0;
+    const float* base = tile + lane * 4;
+    for (int32_t s = 0; s < nslabs; ++s) cnt += chain_f32(base + s * kRowsPerSlabF32, T, g0, gp, L);
+    return cnt;
+}
+
+template <>
+__device__ __forceinline__ int eval_individual_on_tile<ElemR8>(const uint8_t* tile, int32_t T, int32_t nslabs,
+                                                               int lane, int4 g0, const int4* gp, int32_t L)
+{
+    int cnt = 0;
+    const uint8_t* base = tile + lane * 16;
+    int32_t s = 0;
+    for (; s + 4 <= nslabs; s += 4) cnt += chain_r8<4>(base + s * kRowsPerSlabR8, T, g0, gp, L);
+    for (; s + 2 <= nslabs; s += 2) cnt += chain_r8<2>(base + s * kRowsPerSlabR8, T, g0, gp, L);
+    for (; s < nslabs; ++s) cnt += chain_r8<1>(base + s * kRowsPerSlabR8, T, g0, gp, L);
+    return cnt;
+}
+
+template <class E, int NCONS>
+__global__ void __launch_bounds__((NCONS + 1) * 32, 1)
+fitness_tiled_kernel(const TiledParams p)
+{
+    using elem_t = typename E::type;
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem);          // [2]
+    uint64_t* empty = full + 2;                                  // [2]
+    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(smem + kSmemHeader);
+    const size_t cnt_bytes = (static_cast<size_t>(p.n_ind) * 4 + 127) & ~static_cast<size_t>(127);
+    elem_t* tiles = reinterpret_cast<elem_t*>(smem + kSmemHeader + cnt_bytes);
+    const size_t tile_elems = static_cast<size_t>(p.cols) * p.T;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t P = p.n_tiles * p.n_ind;
+    const int64_t pb = P * blockIdx.x / gridDim.x;
+    const int64_t pe = P * (blockIdx.x + 1) / gridDim.x;
+    if (pb >= pe) return;                                        // CTA-uniform
+    const int64_t t0 = pb / p.n_ind, t1 = (pe - 1) / p.n_ind;
+    const int32_t ntl = static_cast<int32_t>(t1 - t0 + 1);
+
+    for (int32_t k = tid; k < p.n_ind; k += blockDim.x) s_cnt[k] = 0;
+    if (tid == 0) {
+        mbar_init(&full[0], 1);
+        mbar_init(&full[1], 1);
+        mbar_init(&empty[0], NCONS);
+        mbar_init(&empty[1], NCONS);
+        fence_mbar_init();
+    }
+    __syncthreads();
+
+    if (warp == NCONS) {
+        // ---------------- producer warp (a4) ----------------
+        const elem_t* M = reinterpret_cast<const elem_t*>(p.M);
+        for (int32_t j = 0; j < ntl; ++j) {
+            const int buf = j & 1;
+            mbar_wait(&empty[buf], ((j >> 1) & 1) ^ 1);          // passes immediately for j < 2
+            const int64_t r0 = (t0 + j) * p.T;
+            const int32_t nrows = static_cast<int32_t>(min(static_cast<int64_t>(p.T), p.ld - r0));
+            const uint32_t col_bytes = static_cast<uint32_t>(nrows) * sizeof(elem_t);
+            if (lane == 0) mbar_arrive_expect_tx(&full[buf], col_bytes * static_cast<uint32_t>(p.cols));
+            __syncwarp();
+            elem_t* dst = tiles + buf * tile_elems;
+            for (int32_t c = lane; c < p.cols; c += 32)
+                bulk_copy_g2s(dst + static_cast<size_t>(c) * p.T, M + static_cast<int64_t>(c) * p.ld + r0, col_bytes,
+                              &full[buf]);
+        }
+    } else {
+        // ---------------- consumer warps (a5, a6) ----------------
+        unsigned long long visited = 0;
+        for (int32_t j = 0; j < ntl; ++j) {
+            const int buf = j & 1;
+            const int64_t r0 = (t0 + j) * p.T;
+            const int32_t nrows = static_cast<int32_t>(min(static_cast<int64_t>(p.T), p.ld - r0));
+            const int32_t nslabs = nrows / E::kSlabRows;
+            const int32_t ka = (j == 0) ? static_cast<int32_t>(pb - t0 * p.n_ind) : 0;
+            const int32_t kb = (j == ntl - 1) ? static_cast<int32_t>(pe - t1 * p.n_ind) : p.n_ind;
+            const elem_t* tile = tiles + buf * tile_elems;
+            mbar_wait(&full[buf], (j >> 1) & 1);
+            for (int32_t k = ka + warp; k < kb; k += NCONS) {
+                const int2 m = __ldg(&p.meta[k]);
+                if (m.y < 2) continue;
+                const int4* gp = p.pids4 + m.x;
+                const int4 g0 = __ldg(gp);
+                int cnt = eval_individual_on_tile<E>(tile, p.T, nslabs, lane, g0, gp, m.y);
+                cnt = __reduce_add_sync(0xffffffffu, cnt);
+                if (lane == 0 && cnt) atomicAdd(&s_cnt[k], static_cast<unsigned int>(cnt));
+                visited += static_cast<unsigned long long>(m.y) * nrows;
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[buf]);
+        }
+        if (p.visits != nullptr && lane == 0 && visited) atomicAdd(p.visits, visited);
+    }
+    __syncthreads();
+    for (int32_t k = tid; k < p.n_ind; k += blockDim.x) {
+        const unsigned int c = s_cnt[k];
+        if (c) atomicAdd(&p.counts[k], static_cast<unsigned long long>(c));
+    }
+}
+
+}  // namespace ebic

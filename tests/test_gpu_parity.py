@@ -1,0 +1,312 @@
+"""Parity of the CUDA path (through the C ABI, via the thin binding) against the CPU oracle.
+
+Bar: bit-exact (integer counts and bitmasks from exact float32 comparisons; tolerance 0).
+Every fitness kernel (DIRECT, TILED_F32, RANK8) is compared with the oracle on the same seeded
+inputs.  All tests here need the B200.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from conftest import csr, golden_names, load_golden, mask_to_bits
+from paper_1807_09932_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+ON, OFF = 1, 0
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1807_09932_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def kernels_for(eb, B):
+    ks = [B.EBIC_KERNEL_DIRECT]
+    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8):
+        try:
+            eb.set_kernel(k)
+            ks.append(k)
+        except B.EbicError:
+            pass
+    eb.set_kernel(B.EBIC_KERNEL_AUTO)
+    return ks
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def gpu_counts(eb, B, off, ids, kernel, device=True):
+    import torch
+    eb.set_kernel(kernel)
+    if device:
+        c = eb.eval_fitness(dev(off), dev(ids))
+        torch.cuda.synchronize()
+        out = c.cpu().numpy().view(np.uint64)
+    else:
+        out = eb.eval_fitness(off, ids)
+    eb.set_kernel(B.EBIC_KERNEL_AUTO)
+    return out
+
+
+def gpu_masks(eb, off, ids, chosen, device=True):
+    import torch
+    ch = np.asarray(chosen, dtype=np.int32)
+    if device:
+        m, c = eb.extract_rows(dev(off), dev(ids), dev(ch))
+        torch.cuda.synchronize()
+        return m.cpu().numpy().view(np.uint64), c.cpu().numpy().view(np.uint64)
+    return eb.extract_rows(off, ids, ch)
+
+
+def check_all(B, oracle_mod, matrix, mode, off, ids, chosen=None, expect_status=0):
+    """Every kernel's counts and the extraction masks equal the oracle's, element by element."""
+    st, want = oracle_mod.eval_fitness(matrix, mode, off, ids)
+    assert st == expect_status
+    with B.Ebic(matrix, mode) as eb:
+        for kern in kernels_for(eb, B):
+            got = gpu_counts(eb, B, off, ids, kern)
+            assert (got == want).all(), (B.KERNEL_NAMES[kern], np.flatnonzero(got != want)[:10])
+            assert eb.status() == expect_status
+        n_ind = off.size - 1
+        if chosen is None:
+            chosen = np.arange(n_ind, dtype=np.int32)
+        if len(chosen):
+            st, wm, wc = oracle_mod.extract_rows(matrix, mode, off, ids, chosen)
+            gm, gc = gpu_masks(eb, off, ids, chosen)
+            assert (gm == wm).all()
+            assert (gc == wc).all()
+            assert eb.status() == st
+    return want
+
+
+# ------------------------------------------------------------------------- loader (a1, a2, a2')
+@pytest.mark.parametrize("rows,cols,nan_rate", [(1, 1, 0.0), (200, 20, 0.1), (513, 33, 0.05), (4097, 100, 0.02)])
+def test_loader_products(B, rows, cols, nan_rate):
+    rng = np.random.default_rng(rows)
+    m = rng.standard_normal((rows, cols), dtype=np.float32)
+    m[rng.random((rows, cols)) < nan_rate] = np.nan
+    m[0, 0] = np.float32(-0.0) if nan_rate == 0 else m[0, 0]
+    for src in (m, dev(m)):                                    # host pointer and device pointer
+        with B.Ebic(src, ON) as eb:
+            ld = eb.ld
+            assert ld % 512 == 0 and ld >= rows and ld - rows < 512
+            mc = eb.debug_read(0)
+            assert (mc[:, :rows].view(np.uint32) == m.T.view(np.uint32)).all()   # bit-exact transpose
+            assert np.isnan(mc[:, rows:]).all()                                   # padding = missing
+            mask = eb.debug_read(1)
+            bits = np.unpackbits(mask.view(np.uint8), bitorder="little").reshape(cols, ld).astype(bool)
+            assert (bits[:, :rows] == np.isnan(m.T)).all() and bits[:, rows:].all()
+            assert (eb.debug_read(2) == (~np.isnan(m)).sum(axis=0).astype(np.uint64)).all()
+            rk = eb.debug_read(3)
+            below = (m[:, None, :] < m[:, :, None]).sum(axis=2)                   # [rows][cols]
+            code = np.where(np.isnan(m), 0x7F, 0x80 | below).astype(np.uint8)
+            assert (rk[:, :rows] == code.T).all() and (rk[:, rows:] == 0x7F).all()
+
+
+# ------------------------------------------------------------------------- hand fixtures on the GPU
+@pytest.mark.parametrize("name", golden_names())
+def test_golden_fixtures_on_gpu(B, oracle_mod, name):
+    m, cases = load_golden(name)
+    for mode in (ON, OFF):
+        sel = [c for c in cases if (c["mode"] == "BOTH" or c["mode"] == ("ON" if mode else "OFF"))]
+        off, ids = csr([c["ids"] for c in sel])
+        want = check_all(B, oracle_mod, m, mode, off, ids)
+        assert want.tolist() == [c["count"] for c in sel]       # and both equal the hand-typed answer
+        with B.Ebic(m, mode) as eb:
+            gm, gc = gpu_masks(eb, off, ids, np.arange(len(sel)))
+            for j, c in enumerate(sel):
+                assert (mask_to_bits(gm[j], m.shape[0]) == np.array([ch == "1" for ch in c["mask"]])).all()
+
+
+# ------------------------------------------------------------------------- the five workloads
+@pytest.mark.parametrize("index", [0, 1, 2, 3])
+def test_workload_full_size(B, oracle_mod, index):
+    w = W.make_workload(index)
+    chosen = [k for k, _ in w.planted_individuals][:8] + [w.n_ind - 1]
+    check_all(B, oracle_mod, w.matrix, w.missing_mode, w.offsets, w.col_ids, np.array(chosen, np.int32))
+
+
+def test_workload_c5_scaled(B, oracle_mod):
+    """C5's recipe at a size the oracle finishes in seconds: several tiles, a ragged tail (300,001
+    rows is not a multiple of 32, 128, 512 or any tile size)."""
+    w = W.make_workload(4, rows=300_001, n_ind=512)
+    chosen = [k for k, _ in w.planted_individuals][:6]
+    check_all(B, oracle_mod, w.matrix, w.missing_mode, w.offsets, w.col_ids, np.array(chosen, np.int32))
+
+
+def test_planted_recovery_on_gpu(B):
+    w = W.make_workload(0)
+    with B.Ebic(w.matrix, w.missing_mode) as eb:
+        chosen = [k for k, _ in w.planted_individuals]
+        gm, gc = gpu_masks(eb, w.offsets, w.col_ids, chosen)
+        for slot, (k, b) in enumerate(w.planted_individuals):
+            assert np.flatnonzero(mask_to_bits(gm[slot], w.rows)).tolist() == w.planted[b].rows.tolist()
+
+
+# ------------------------------------------------------------------------- edge cases
+@pytest.mark.parametrize("rows", [1, 31, 32, 33, 127, 128, 129, 511, 512, 513, 1025, 65_535, 65_536, 65_537])
+def test_row_count_edges(B, oracle_mod, rows):
+    """Ragged tails around every tile / slab / word size and the paper's old 65,535-row limit."""
+    m, off, ids = W.random_case(rows, rows, 7, 40, (0, 7), 0.05, True, False)
+    for mode in (ON, OFF):
+        check_all(B, oracle_mod, m, mode, off, ids, np.arange(0, 40, 3, dtype=np.int32))
+
+
+@pytest.mark.parametrize("n_ind", [1, 2, 31, 8191, 8192, 8193, 20_000])
+def test_population_size_edges(B, oracle_mod, n_ind):
+    """Around the per-launch population chunk (8192) and beyond."""
+    m, off, ids = W.random_case(n_ind, 3000, 12, n_ind, (0, 5), 0.03, False, True)
+    check_all(B, oracle_mod, m, ON, off, ids, np.array([0, n_ind - 1], np.int32))
+
+
+def test_population_65536(B, oracle_mod):
+    """One more than the paper's population limit of 65,535."""
+    m, off, ids = W.random_case(65536, 1000, 10, 65_536, (2, 4), 0.0, False, True)
+    check_all(B, oracle_mod, m, OFF, off, ids, np.array([65_535], np.int32))
+
+
+def test_long_and_degenerate_chromosomes(B, oracle_mod):
+    rows, cols = 2000, 16
+    m, _, _ = W.random_case(77, rows, cols, 1, (1, 1), 0.02, True, True)
+    rng = np.random.default_rng(5)
+    inc = np.argsort(m[0])                                         # a long chain some rows can satisfy
+    chroms = [[], [3], [3, 3], [3, 3, 3, 3, 3], list(range(cols)), list(range(cols))[::-1],
+              inc.tolist(), (inc.tolist() * 3)[:40], rng.integers(0, cols, 1500).tolist(),
+              [5] * 1100, rng.integers(0, cols, 33).tolist(), [7, 7, 2, 2]]
+    off, ids = csr(chroms)
+    for mode in (ON, OFF):
+        check_all(B, oracle_mod, m, mode, off, ids)
+
+
+def test_wide_matrix_falls_back(B, oracle_mod):
+    """cols > 127: no rank tiles; cols so large that no float tile double-buffers: DIRECT only."""
+    for cols in (128, 200, 500):
+        m, off, ids = W.random_case(cols, 700, cols, 50, (0, 9), 0.02, False, True)
+        with B.Ebic(m, ON) as eb:
+            with pytest.raises(B.EbicError):
+                eb.set_kernel(B.EBIC_KERNEL_RANK8)
+            expected = B.EBIC_KERNEL_TILED_F32 if cols <= 200 else B.EBIC_KERNEL_DIRECT
+            assert eb.kernel == expected
+        check_all(B, oracle_mod, m, ON, off, ids, np.arange(0, 50, 7, dtype=np.int32))
+
+
+def test_empty_calls(B):
+    import torch
+    m = np.zeros((10, 3), dtype=np.float32)
+    with B.Ebic(m, ON) as eb:
+        c = eb.eval_fitness(dev(np.zeros(1, np.int32)), dev(np.zeros(0, np.int32)))
+        assert c.numel() == 0
+        off, ids = csr([[0, 1]])
+        masks, counts = eb.extract_rows(dev(off), dev(ids), torch.zeros(0, dtype=torch.int32, device="cuda"))
+        assert masks.shape == (0, 1) and eb.status() == 0
+
+
+def test_invalid_population_sticky_error(B, oracle_mod):
+    m, _, _ = W.random_case(3, 600, 5, 1)
+    good = [[0, 1], [2], [], [4, 3, 2]]
+    # bad column id
+    off, ids = csr(good + [[1, 5], [0, -2, 1]])
+    check_all(B, oracle_mod, m, ON, off, ids, expect_status=B.EBIC_ERR_BAD_COLUMN)
+    # non-monotone offsets (individual 1), offsets beyond n_ids (last)
+    off = np.array([0, 2, 1, 3, 9], dtype=np.int32)
+    ids = np.array([0, 1, 2, 3], dtype=np.int32)
+    check_all(B, oracle_mod, m, ON, off, ids, expect_status=B.EBIC_ERR_BAD_OFFSETS)
+    # chosen index out of range
+    off, ids = csr(good)
+    with B.Ebic(m, ON) as eb:
+        st, wm, wc = oracle_mod.extract_rows(m, ON, off, ids, [1, 9, -1, 0])
+        gm, gc = gpu_masks(eb, off, ids, [1, 9, -1, 0])
+        assert (gm == wm).all() and (gc == wc).all()
+        assert eb.status() == st == B.EBIC_ERR_BAD_OFFSETS
+        assert eb.status() == 0                                    # cleared after being read
+        # the error does not poison later calls
+        assert (gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_AUTO) == oracle_mod.eval_fitness(m, ON, off, ids)[1]).all()
+
+
+def test_host_pointers_and_streams(B, oracle_mod):
+    import torch
+    w = W.make_workload(1, rows=5000, n_ind=300)
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    chosen = np.array([0, 4, 299], dtype=np.int32)
+    _, wm, wc = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
+    with B.Ebic(w.matrix, w.missing_mode) as eb:
+        # numpy in -> numpy out (host buffers, copies inside the call)
+        assert (eb.eval_fitness(w.offsets, w.col_ids) == want).all()
+        gm, gc = eb.extract_rows(w.offsets, w.col_ids, chosen)
+        assert (gm == wm).all() and (gc == wc).all()
+        # pinned host tensors
+        po, pi = torch.from_numpy(w.offsets).pin_memory(), torch.from_numpy(w.col_ids).pin_memory()
+        out = torch.empty(w.n_ind, dtype=torch.int64).pin_memory()
+        eb.eval_fitness(po, pi, counts=out)
+        assert (out.numpy().view(np.uint64) == want).all()
+        # a non-default stream, stream-ordered with a later copy
+        s = torch.cuda.Stream()
+        d_off, d_ids = dev(w.offsets), dev(w.col_ids)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            c = eb.eval_fitness(d_off, d_ids)
+            host = c.to("cpu", non_blocking=False)
+        assert (host.numpy().view(np.uint64) == want).all()
+
+
+def test_instrumentation_counts_nominal_visits(B):
+    w = W.make_workload(2, rows=20_000, n_ind=200)
+    with B.Ebic(w.matrix, w.missing_mode) as eb:
+        for kern in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8):
+            eb.set_kernel(kern)
+            eb.set_instrumentation(True)
+            eb.eval_fitness(dev(w.offsets), dev(w.col_ids))
+            visits = eb.info(10)
+            eb.set_instrumentation(False)
+            assert visits == eb.ld * int(w.lengths.sum())          # no work skipped: executed == nominal
+
+
+# ------------------------------------------------------------------------- full-size C5 (bench config)
+def test_c5_full_size_sampled(B, oracle_mod):
+    """BASELINE.json configs[4] at full size, in the launch configuration bench.py times: a sample of
+    individuals against the oracle one by one, plus properties that hold at any size."""
+    w = W.make_workload(4)
+    d_off, d_ids = dev(w.offsets), dev(w.col_ids)
+    rng = np.random.default_rng(99)
+    sample = np.unique(np.concatenate([[k for k, _ in w.planted_individuals][:16],
+                                       rng.choice(w.n_ind, 32, replace=False)])).astype(np.int32)
+    sub_off, sub_ids = csr([w.col_ids[w.offsets[k]:w.offsets[k + 1]].tolist() for k in sample])
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, sub_off, sub_ids)
+    with B.Ebic(w.matrix, w.missing_mode) as eb:
+        import torch
+        results = {}
+        for kern in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32):
+            eb.set_kernel(kern)
+            c = eb.eval_fitness(d_off, d_ids)
+            torch.cuda.synchronize()
+            results[kern] = c.cpu().numpy().view(np.uint64)
+            assert (results[kern][sample] == want).all(), B.KERNEL_NAMES[kern]
+        assert (results[B.EBIC_KERNEL_RANK8] == results[B.EBIC_KERNEL_TILED_F32]).all()
+        counts = results[B.EBIC_KERNEL_RANK8]
+        # properties: planted rows are a subset; popcount(mask) == count; tail bits zero
+        chosen = np.array([k for k, _ in w.planted_individuals][:4], dtype=np.int32)
+        gm, gc = gpu_masks(eb, w.offsets, w.col_ids, chosen)
+        for slot, (k, b) in enumerate(w.planted_individuals[:4]):
+            bits = mask_to_bits(gm[slot], w.rows)
+            assert bits[w.planted[b].clean_rows].all()
+            assert int(bits.sum()) == int(gc[slot]) == int(counts[k])
+        # closed form on uniformly random individuals: count ~ Binomial(rows, (1-p)^L / L!)
+        import math
+        p = w.cfg.nan_rate
+        first_random = 4 * len(w.planted)
+        for k in range(first_random, first_random + 200):
+            L = int(w.lengths[k])
+            if L > 5:
+                continue
+            q = (1 - p) ** L / math.factorial(L)
+            sigma = math.sqrt(w.rows * q * (1 - q))
+            # planted rows (<= 2.6e6 of 1.7e7) bias the count upwards a little; allow for it
+            assert -6 * sigma <= int(counts[k]) - w.rows * q <= 6 * sigma + 0.2 * w.rows * q

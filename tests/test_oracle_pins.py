@@ -286,7 +286,12 @@ def test_errors(oracle_mod):
     with pytest.raises(Exception):
         oracle_mod.eval_fitness(m.reshape(-1), ON, off, ids)
     assert oracle_mod.eval_fitness(m, 7, *csr(good))[0] == oracle_mod.ERR_ARG
-    assert oracle_mod.extract_rows(m, ON, *csr(good), [3])[0] == oracle_mod.ERR_ARG
+    st, masks, c = oracle_mod.extract_rows(m, ON, *csr(good), [3, 1, -1])   # 3, -1: no such individual
+    assert st == oracle_mod.ERR_BAD_OFFSETS and not masks[0].any() and not masks[2].any()
+    assert c.tolist() == [0, int(ref[1]), 0]
+    off_long = np.array([0, 2, 5], dtype=np.int32)         # offsets[2] > n_ids == 3
+    st, counts = oracle_mod.eval_fitness(m, ON, off_long, np.array([0, 1, 2], dtype=np.int32))
+    assert st == oracle_mod.ERR_BAD_OFFSETS and counts[1] == 0 and counts[0] == ref[0]
     st, counts = oracle_mod.eval_fitness(m, ON, np.zeros(1, np.int32), np.zeros(0, np.int32))
     assert st == 0 and counts.size == 0
 
