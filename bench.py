@@ -1,0 +1,494 @@
+#!/usr/bin/env python
+"""bench.py -- row-pair comparisons/s of EBIC population fitness evaluation on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c1..c5] [--kernel auto|rank8|tiled_f32|direct]
+    python bench.py --impl reference ...      # the CPU oracle as it stands, on the host cores
+    python bench.py --table                   # every workload x every kernel -> gpurun_out/table.json
+
+A step = one pass of the hot path over one population: population ingest
++ validation, tile staging, trend predicate, count accumulation (`ebic_eval_fitness`) and the
+matched-row bitmasks of 8 chosen individuals (`ebic_extract_rows`).  The loader (a1/a2: transpose,
+NaN mask, rank tiles) runs once per dataset in `ebic_create`; its time is reported as `create_ms`.
+
+`value`  = nominal row-pair comparisons of the fitness evaluation (rows * sum(max(L-1,0))) per second of
+           step time, population and matrix resident in HBM, CUDA events on the launch stream, L2
+           flushed between steps, max over ranks.
+`e2e`    = same, through the C-ABI with HOST buffers: pinned population in, counts and masks out,
+           copies inside the timed region.
+`roofline` is for the dominant kernel (the fitness kernel), timed live with CUDA events recorded by
+the library around that kernel on its stream (DESIGN.md section 6 derives the peak).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+from paper_1807_09932_b200 import workloads as W  # noqa: E402
+
+METRIC = "row_pair_comparisons_per_s"
+UNIT = "comparisons/s"
+N_CHOSEN = 8
+WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4}
+KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3}
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return json.loads(p.read_text()), "measured"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows, self.proc, self.gpu = [], None, gpu_index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def __exit__(self, *exc):
+        if self.proc:
+            time.sleep(0.15)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[1]))
+                mx.append(float(r[2]))
+                for name, flag in zip(names, r[5:9]):
+                    if flag.lower().startswith("active"):
+                        reasons.add(name)
+            except Exception:
+                continue
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def pick_chosen(w):
+    ch = [k for k, _ in w.planted_individuals][:N_CHOSEN]
+    k = 0
+    while len(ch) < min(N_CHOSEN, w.n_ind):
+        if k not in ch:
+            ch.append(k)
+        k += 1
+    return np.array(ch, dtype=np.int32)
+
+
+# ----------------------------------------------------------------------------------------------------
+# roofline of the fitness kernel
+# ----------------------------------------------------------------------------------------------------
+def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None):
+    f_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    smem_peak_gbs = sm_count * 128 * f_hz / 1e9            # 128 B / clk / SM shared-memory data pipe
+    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "direct": 4}[kernel_name]
+    achieved = visits_executed * bytes_per_visit / kernel_s / 1e9
+    return {"bound": "alu", "resource": "shared-memory data pipe (128 B/clk/SM) == ALU pipe at 0.5 op/visit"
+            if kernel_name == "rank8" else "shared-memory data pipe (128 B/clk/SM)",
+            "kernel": "fitness_" + kernel_name, "achieved": achieved, "peak": smem_peak_gbs, "unit": "GB/s",
+            "frac": achieved / smem_peak_gbs, "traffic": traffic,
+            "bytes_per_visit": bytes_per_visit, "visits_per_launch": visits_executed,
+            "kernel_ms": kernel_s * 1e3, "peak_basis": f"{sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz ({peaks_kind} sm_max_mhz)"}
+
+
+# ----------------------------------------------------------------------------------------------------
+# GPU arm
+# ----------------------------------------------------------------------------------------------------
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1807_09932_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("launch with torch.distributed.run --nproc-per-node N for --gpus N")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    peaks, peaks_kind = measured_peaks()
+
+    idx = WORKLOADS[args.workload]
+    t0 = time.time()
+    # weak scaling: every rank holds its own `rows`-row slice of an (N x rows)-row dataset
+    w = W.make_workload(idx, rows=args.rows, n_ind=args.n_ind)
+    if world > 1 and rank > 0:
+        rng = np.random.default_rng([2, idx, rank])
+        w.matrix = w.matrix[rng.permutation(w.rows)]           # a different slice per rank, same recipe
+    gen_s = time.time() - t0
+    chosen = pick_chosen(w)
+
+    torch.cuda.synchronize()
+    t0 = time.time()
+    eb = B.Ebic(w.matrix, w.missing_mode)                      # host matrix -> H2D + loader kernels
+    torch.cuda.synchronize()
+    create_ms = (time.time() - t0) * 1e3
+    eb.set_kernel(KERNELS[args.kernel])
+    kernel_name = B.KERNEL_NAMES[eb.kernel]
+
+    d_off = torch.from_numpy(w.offsets).cuda()
+    d_ids = torch.from_numpy(w.col_ids).cuda()
+    d_chosen = torch.from_numpy(chosen).cuda()
+    d_counts = torch.empty(w.n_ind, dtype=torch.int64, device="cuda")
+    d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
+    d_mcnt = torch.empty(len(chosen), dtype=torch.int64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def step():
+        eb.eval_fitness(d_off, d_ids, counts=d_counts)
+        if world > 1:
+            dist.all_reduce(d_counts)                          # the path's one exchange step (8(e))
+        eb.extract_rows(d_off, d_ids, d_chosen, masks=d_masks, counts=d_mcnt)
+
+    launches0 = eb.info(8)
+    for _ in range(max(args.warmup, 0)):
+        flush.zero_()
+        step()
+    torch.cuda.synchronize()
+    launches_per_step = (eb.info(8) - launches0) // max(args.warmup, 1) if args.warmup else None
+
+    # executed visits of one evaluation (instrumented, outside the timed region)
+    eb.set_instrumentation(1)
+    eb.eval_fitness(d_off, d_ids, counts=d_counts)
+    visits_exec = eb.info(10)
+    eb.set_instrumentation(2)                                   # event pairs around the fitness kernel
+
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    starts = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    ends = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
+    with ClockSampler(local_rank) as clk:
+        wall0 = time.time()
+        for i in range(args.steps):
+            flush.zero_()                                       # L2 flush, outside the step's event pair
+            starts[i].record()
+            step()
+            ends[i].record()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        wall_s = time.time() - wall0
+    step_ms = [s.elapsed_time(e) for s, e in zip(starts, ends)]
+    total_ms = float(sum(step_ms))
+    kernel_ns = eb.info(11)
+    eb.set_instrumentation(0)
+    if launches_per_step is None:
+        launches_per_step = 3
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    comparisons = w.comparisons * world
+    value = comparisons / (ms_per_step * 1e-3)
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region
+    p_off = torch.from_numpy(w.offsets).pin_memory()
+    p_ids = torch.from_numpy(w.col_ids).pin_memory()
+    p_chosen = torch.from_numpy(chosen).pin_memory()
+    h_counts = torch.empty(w.n_ind, dtype=torch.int64).pin_memory()
+    h_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64).pin_memory()
+    h_mcnt = torch.empty(len(chosen), dtype=torch.int64).pin_memory()
+
+    def e2e_step():
+        eb.eval_fitness(p_off, p_ids, counts=h_counts)          # H2D population, kernels, D2H counts, sync
+        eb.extract_rows(p_off, p_ids, p_chosen, masks=h_masks, counts=h_mcnt)
+
+    for _ in range(3):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_t = []
+    for _ in range(args.steps):
+        flush.zero_()
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        e2e_step()
+        e2e_t.append(time.perf_counter() - t1)
+    e2e_s = float(np.mean(e2e_t))
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = int(p_off.numel() * 4 * 2 + p_ids.numel() * 4 * 2 + p_chosen.numel() * 4)
+    d2h = int(h_counts.numel() * 8 + h_masks.numel() * 8 + h_mcnt.numel() * 8)
+    assert (h_counts.numpy() == d_counts.cpu().numpy()).all() or world > 1
+
+    out = None
+    if rank == 0:
+        sm_count = eb.info(7)
+        roof = roofline(kernel_name, visits_exec, kernel_ns * 1e-9, peaks, peaks_kind, sm_count,
+                        traffic=args.traffic)
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "u8" if kernel_name == "rank8" else "f32", "data": "synthetic",
+            "config": {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind,
+                       "sum_L": int(w.lengths.sum()), "missing_mode": w.missing_mode, "kernel": kernel_name,
+                       "tile_rows": eb.info(5), "ctas": eb.info(6), "n_chosen": int(len(chosen)),
+                       "l2": "flushed between steps (256 MiB write)",
+                       "parallelism": f"row-sharded x{world}, 1 all-reduce(int64[n_ind]) per step" if world > 1 else "1 GPU"},
+            "individuals_rows_per_s": w.n_ind * w.rows * world / (ms_per_step * 1e-3),
+            "clocks": clk.summary(),
+            "e2e": {"value": comparisons / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3},
+            "gpu_launches": int(launches_per_step * args.steps),
+            "roofline": roof,
+            "create_ms": create_ms, "generate_s": gen_s, "wall_s_timed_region": wall_s,
+            "step_ms_min_max": [min(step_ms), max(step_ms)],
+        }
+        if not args.no_cpu_baseline and world == 1:
+            out["cpu_baseline"] = cpu_baseline(w, budget_s=args.cpu_budget)
+    eb.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return out
+
+
+# ----------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# ----------------------------------------------------------------------------------------------------
+def oracle_sample(w, n_sample, seed=0):
+    """A bounded sample of the workload: `n_sample` individuals (all rows), drawn without replacement."""
+    rng = np.random.default_rng([3, seed])
+    n_sample = min(n_sample, w.n_ind)
+    pick = np.sort(rng.choice(w.n_ind, n_sample, replace=False)) if n_sample < w.n_ind else np.arange(w.n_ind)
+    chrom = [w.col_ids[w.offsets[k]:w.offsets[k + 1]] for k in pick]
+    off = np.zeros(len(chrom) + 1, dtype=np.int32)
+    off[1:] = np.cumsum([c.size for c in chrom])
+    ids = np.concatenate(chrom).astype(np.int32)
+    comparisons = int(w.rows) * int(np.maximum(np.diff(off) - 1, 0).sum())
+    return off, ids, comparisons
+
+
+def cpu_baseline(w, budget_s=15.0):
+    import oracle
+    cores = oracle.max_threads()
+    # calibrate on 8 individuals, then size the sample to ~budget_s of CPU work
+    off, ids, comps = oracle_sample(w, max(8, cores), seed=1)
+    t0 = time.perf_counter()
+    oracle.eval_fitness(w.matrix, w.missing_mode, off, ids)
+    rate = comps / max(time.perf_counter() - t0, 1e-6)
+    n = int(min(w.n_ind, max(cores, budget_s * rate / max(w.comparisons / w.n_ind, 1))))
+    off, ids, comps = oracle_sample(w, n, seed=2)
+    t0 = time.perf_counter()
+    oracle.eval_fitness(w.matrix, w.missing_mode, off, ids)
+    dt = time.perf_counter() - t0
+    return {"value": comps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n} of {w.n_ind} individuals x all {w.rows} rows, {comps:.3e} comparisons in {dt:.2f} s"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, on the host cores, same workload / metric / unit."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return None
+    import oracle
+    oracle.build()
+    w = W.make_workload(WORKLOADS[args.workload], rows=args.rows, n_ind=args.n_ind)
+    cores = oracle.max_threads()
+    off, ids, comps = oracle_sample(w, max(8, cores), seed=1)
+    t0 = time.perf_counter()
+    oracle.eval_fitness(w.matrix, w.missing_mode, off, ids)
+    rate = comps / max(time.perf_counter() - t0, 1e-6)
+    per_step_budget = min(10.0, 120.0 / max(args.steps + args.warmup, 1))
+    n = int(min(w.n_ind, max(cores, per_step_budget * rate / max(w.comparisons / w.n_ind, 1))))
+    times, comps = [], 0
+    for i in range(args.warmup + args.steps):
+        off, ids, comps = oracle_sample(w, n, seed=10 + i)
+        t0 = time.perf_counter()
+        oracle.eval_fitness(w.matrix, w.missing_mode, off, ids)
+        if i >= args.warmup:
+            times.append((time.perf_counter() - t0, comps))
+    total_t = sum(t for t, _ in times)
+    total_c = sum(c for _, c in times)
+    value = total_c / total_t
+    sample = f"each step: {n} of {w.n_ind} individuals x all {w.rows} rows (fresh sample per step)"
+    return {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_t / len(times) * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind,
+                       "missing_mode": w.missing_mode, "kernel": "cpu oracle (oracle/ebic_oracle.c)"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+# ----------------------------------------------------------------------------------------------------
+# --table: every workload x kernel, kernel-only and graph-replay timings
+# ----------------------------------------------------------------------------------------------------
+def run_table(args):
+    import torch
+    from paper_1807_09932_b200 import binding as B
+    peaks, peaks_kind = measured_peaks()
+    torch.cuda.set_device(0)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    rows_out = []
+    names = args.table_workloads.split(",")
+    for name in names:
+        w = W.make_workload(WORKLOADS[name])
+        eb = B.Ebic(w.matrix, w.missing_mode)
+        d_off, d_ids = torch.from_numpy(w.offsets).cuda(), torch.from_numpy(w.col_ids).cuda()
+        d_counts = torch.empty(w.n_ind, dtype=torch.int64, device="cuda")
+        chosen = pick_chosen(w)
+        d_chosen = torch.from_numpy(chosen).cuda()
+        d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
+        for kname in ("rank8", "tiled_f32", "direct"):
+            if kname == "direct" and w.comparisons > 2e10:
+                continue
+            try:
+                eb.set_kernel(KERNELS[kname])
+            except B.EbicError:
+                continue
+            reps = 5 if w.comparisons > 1e11 else 20
+            for _ in range(3):
+                eb.eval_fitness(d_off, d_ids, counts=d_counts)
+            eb.set_instrumentation(1)
+            eb.eval_fitness(d_off, d_ids, counts=d_counts)
+            visits = eb.info(10) if kname != "direct" else eb.ld * int(w.lengths.sum())
+            eb.set_instrumentation(2)
+            call_ms = []
+            for _ in range(reps):
+                flush.zero_()
+                s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                s.record()
+                eb.eval_fitness(d_off, d_ids, counts=d_counts)
+                e.record()
+                torch.cuda.synchronize()
+                call_ms.append(s.elapsed_time(e))
+            kernel_ms = eb.info(11) / 1e6
+            eb.set_instrumentation(0)
+            # CUDA-graph replay of the whole call (ingest + fitness): separates launch latency
+            graph_ms = None
+            try:
+                g = torch.cuda.CUDAGraph()
+                side = torch.cuda.Stream()
+                with torch.cuda.stream(side):
+                    eb.eval_fitness(d_off, d_ids, counts=d_counts, stream=side)
+                    torch.cuda.synchronize()
+                    with torch.cuda.graph(g, stream=side):
+                        eb.eval_fitness(d_off, d_ids, counts=d_counts, stream=side)
+                torch.cuda.synchronize()
+                s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                s.record()
+                for _ in range(reps):
+                    g.replay()
+                e.record()
+                torch.cuda.synchronize()
+                graph_ms = s.elapsed_time(e) / reps
+            except Exception as ex:                              # noqa: BLE001
+                log("graph replay unavailable:", ex)
+                torch.cuda.synchronize()
+            roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7))
+            rows_out.append({"workload": w.cfg.name, "kernel": kname, "call_ms_median": statistics.median(call_ms),
+                             "kernel_ms": kernel_ms, "graph_replay_ms": graph_ms,
+                             "comparisons_per_s": w.comparisons / (statistics.median(call_ms) * 1e-3),
+                             "comparisons_per_s_kernel": w.comparisons / (kernel_ms * 1e-3),
+                             "individuals_rows_per_s": w.n_ind * w.rows / (statistics.median(call_ms) * 1e-3),
+                             "roofline_frac": roof["frac"], "achieved_gbs": roof["achieved"], "tile_rows": eb.info(5),
+                             "ctas": eb.info(6)})
+            log(json.dumps(rows_out[-1]))
+        # extraction (a7): HBM-bound
+        eb.set_kernel(0)
+        ex_ms = []
+        for _ in range(10):
+            flush.zero_()
+            s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s.record()
+            eb.extract_rows(d_off, d_ids, d_chosen, masks=d_masks, want_counts=False)
+            e.record()
+            torch.cuda.synchronize()
+            ex_ms.append(s.elapsed_time(e))
+        Lsum = int(sum(w.lengths[k] for k in chosen))
+        ex_bytes = eb.ld * 4 * Lsum + len(chosen) * eb.mask_words * 8
+        rows_out.append({"workload": w.cfg.name, "kernel": "extract_rows", "call_ms_median": statistics.median(ex_ms),
+                         "hbm_gbs": ex_bytes / (statistics.median(ex_ms) * 1e-3) / 1e9,
+                         "hbm_frac": ex_bytes / (statistics.median(ex_ms) * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                         "n_chosen": int(len(chosen)), "bytes": ex_bytes})
+        log(json.dumps(rows_out[-1]))
+        if not args.no_cpu_baseline:
+            rows_out.append({"workload": w.cfg.name, "kernel": "cpu_oracle", **cpu_baseline(w, budget_s=args.cpu_budget)})
+            log(json.dumps(rows_out[-1]))
+        eb.close()
+        del w
+    out_dir = ROOT / "gpurun_out"
+    out_dir.mkdir(exist_ok=True)
+    (out_dir / "table.json").write_text(json.dumps(rows_out, indent=1))
+    return {"table": rows_out}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ebic", choices=["ebic", "reference"])
+    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--kernel", default="auto", choices=sorted(KERNELS))
+    ap.add_argument("--rows", type=int, default=None, help="override the workload's row count")
+    ap.add_argument("--n-ind", type=int, default=None, dest="n_ind")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of CPU work for cpu_baseline")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the fitness kernel from an ncu --set full capture")
+    ap.add_argument("--table", action="store_true")
+    ap.add_argument("--table-workloads", default="c1,c2,c3,c4,c5")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ebic" and not args.table:
+        log("note: fewer than 3 warm-up steps requested; using 3 (timing rules)")
+        args.warmup = 3
+    if args.table:
+        out = run_table(args)
+    elif args.impl == "reference":
+        out = run_reference(args)
+    else:
+        out = run_gpu(args)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()

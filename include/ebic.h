@@ -113,10 +113,16 @@ int ebic_status(ebic_ctx *ctx, void *cuda_stream);
 int ebic_set_kernel(ebic_ctx *ctx, int32_t kernel);
 
 /*
- * Instrumentation for roofline accounting: when on, the tiled fitness kernels add the number of
- * (row, column-visit) operand fetches they actually executed to a device counter (one extra global
- * atomic per warp).  ebic_get_info(ctx, 10) synchronises the device, returns the counter and
- * resets it.  Off by default; never on inside a timed region.
+ * Instrumentation for roofline accounting.  `on` is a bit set:
+ *   bit 0  the tiled fitness kernels add the number of (row, column-visit) operand fetches they
+ *          actually executed to a device counter (one extra global atomic per warp);
+ *          ebic_get_info(ctx, 10) synchronises the device, returns the counter and resets it.
+ *          Never on inside a timed region.
+ *   bit 1  every ebic_eval_fitness brackets its fitness kernel launch(es) -- not the ingest kernel --
+ *          with a pair of CUDA events on the call's stream (ring of 256 pairs);
+ *          ebic_get_info(ctx, 11) synchronises the device and returns their mean duration in ns,
+ *          ebic_get_info(ctx, 12) the number of evals timed.  Setting the mode restarts the ring.
+ * Off (0) by default.
  */
 int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
 
@@ -125,7 +131,8 @@ int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
  *   0 rows, 1 cols, 2 padded leading dimension ld, 3 missing_mode, 4 kernel ebic_eval_fitness will
  *   use, 5 rows per shared-memory tile of that kernel, 6 CTAs of its last launch, 7 SM count,
  *   8 kernels launched by this context so far, 9 bytes of device memory the context owns,
- *   10 executed column visits since the last read (see ebic_set_instrumentation).
+ *   10 executed column visits since the last read, 11 mean fitness-kernel time in ns, 12 evals
+ *   timed (see ebic_set_instrumentation).
  * Returns -1 for NULL / unknown `what`.
  */
 int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);

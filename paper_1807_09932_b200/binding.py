@@ -122,8 +122,8 @@ def ebic_set_kernel(ctx, kernel: int) -> None:
         raise EbicError(st, "ebic_set_kernel")
 
 
-def ebic_set_instrumentation(ctx, on: bool) -> None:
-    load_library().ebic_set_instrumentation(ctx, 1 if on else 0)
+def ebic_set_instrumentation(ctx, on: int) -> None:
+    load_library().ebic_set_instrumentation(ctx, int(on))
 
 
 def ebic_get_info(ctx, what: int) -> int:
@@ -254,7 +254,7 @@ class Ebic:
     def set_kernel(self, kernel: int) -> None:
         ebic_set_kernel(self._ctx, kernel)
 
-    def set_instrumentation(self, on: bool) -> None:
+    def set_instrumentation(self, on: int) -> None:
         ebic_set_instrumentation(self._ctx, on)
 
     def info(self, what: int) -> int:

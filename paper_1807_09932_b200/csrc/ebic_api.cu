@@ -42,6 +42,13 @@ struct ebic_ctx {
     void* stage[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     int64_t stage_cap[5] = {0, 0, 0, 0, 0};
 
+    // bit 1 of `instrument`: time the fitness kernel(s) of each eval with CUDA events on its stream
+    static constexpr int kTimingRing = 256;
+    cudaEvent_t ev_begin[kTimingRing] = {};
+    cudaEvent_t ev_end[kTimingRing] = {};
+    int32_t time_kernels = 0;
+    int64_t timed_evals = 0;
+
     int64_t bytes_owned = 0;
     int64_t launches = 0;
     int32_t last_grid = 0;
@@ -174,6 +181,14 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());
 
+    const int slot = static_cast<int>(ctx->timed_evals % ebic_ctx::kTimingRing);
+    if (ctx->time_kernels) {
+        if (!ctx->ev_begin[slot]) {
+            EBIC_TRY(cudaEventCreate(&ctx->ev_begin[slot]));
+            EBIC_TRY(cudaEventCreate(&ctx->ev_end[slot]));
+        }
+        EBIC_TRY(cudaEventRecord(ctx->ev_begin[slot], stream));
+    }
     for (int32_t k0 = 0; k0 < n_ind; k0 += kMaxIndPerLaunch) {
         const int32_t n = std::min<int32_t>(kMaxIndPerLaunch, n_ind - k0);
         const int32_t kernel = resolve_kernel(ctx, n);
@@ -198,6 +213,10 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
             st = cuda_status(cudaGetLastError());
         }
         if (st) return st;
+    }
+    if (ctx->time_kernels) {
+        EBIC_TRY(cudaEventRecord(ctx->ev_end[slot], stream));
+        ctx->timed_evals++;
     }
     return EBIC_OK;
 }
@@ -320,6 +339,10 @@ int ebic_destroy(ebic_ctx* ctx) {
     cudaFree(ctx->meta);
     cudaFree(ctx->pids);
     for (void* s : ctx->stage) cudaFree(s);
+    for (int i = 0; i < ebic_ctx::kTimingRing; ++i) {
+        if (ctx->ev_begin[i]) cudaEventDestroy(ctx->ev_begin[i]);
+        if (ctx->ev_end[i]) cudaEventDestroy(ctx->ev_end[i]);
+    }
     cudaGetLastError();
     delete ctx;
     return EBIC_OK;
@@ -435,7 +458,9 @@ int ebic_set_kernel(ebic_ctx* ctx, int32_t kernel) {
 
 int ebic_set_instrumentation(ebic_ctx* ctx, int32_t on) {
     if (!ctx) return EBIC_ERR_ARG;
-    ctx->count_visits = on ? 1 : 0;
+    ctx->count_visits = (on & 1) ? 1 : 0;
+    ctx->time_kernels = (on & 2) ? 1 : 0;
+    ctx->timed_evals = 0;
     return EBIC_OK;
 }
 
@@ -462,6 +487,24 @@ int64_t ebic_get_info(ebic_ctx* ctx, int32_t what) {
             }
             return static_cast<int64_t>(v);
         }
+        case 11: {   // mean fitness-kernel time of the evals timed since instrumentation was set, in ns
+            if (ctx->timed_evals == 0 || cudaDeviceSynchronize() != cudaSuccess) {
+                cudaGetLastError();
+                return -1;
+            }
+            const int64_t n = std::min<int64_t>(ctx->timed_evals, ebic_ctx::kTimingRing);
+            double total_ms = 0;
+            for (int64_t i = 0; i < n; ++i) {
+                float ms = 0;
+                if (cudaEventElapsedTime(&ms, ctx->ev_begin[i], ctx->ev_end[i]) != cudaSuccess) {
+                    cudaGetLastError();
+                    return -1;
+                }
+                total_ms += ms;
+            }
+            return static_cast<int64_t>(total_ms / n * 1e6);
+        }
+        case 12: return ctx->timed_evals;
         default: return -1;
     }
 }

@@ -298,7 +298,9 @@ def test_c5_full_size_sampled(B, oracle_mod):
             bits = mask_to_bits(gm[slot], w.rows)
             assert bits[w.planted[b].clean_rows].all()
             assert int(bits.sum()) == int(gc[slot]) == int(counts[k])
-        # closed form on uniformly random individuals: count ~ Binomial(rows, (1-p)^L / L!)
+        # closed form on uniformly random individuals: count ~ Binomial(rows, (1-p)^L / L!) on the rows
+        # that are iid; planted rows (sorted in some column order) can shift it either way, by at most
+        # the number of planted rows in biclusters sharing a column with the individual.
         import math
         p = w.cfg.nan_rate
         first_random = 4 * len(w.planted)
@@ -306,7 +308,13 @@ def test_c5_full_size_sampled(B, oracle_mod):
             L = int(w.lengths[k])
             if L > 5:
                 continue
+            chrom = set(w.col_ids[w.offsets[k]:w.offsets[k + 1]].tolist())
+            affected = sum(b.rows.size for b in w.planted if chrom & set(b.order.tolist()))
             q = (1 - p) ** L / math.factorial(L)
             sigma = math.sqrt(w.rows * q * (1 - q))
-            # planted rows (<= 2.6e6 of 1.7e7) bias the count upwards a little; allow for it
-            assert -6 * sigma <= int(counts[k]) - w.rows * q <= 6 * sigma + 0.2 * w.rows * q
+            assert abs(int(counts[k]) - w.rows * q) <= 6 * sigma + affected, (k, L, int(counts[k]), w.rows * q)
+        # third witness on the whole population: the simple DIRECT kernel
+        eb.set_kernel(B.EBIC_KERNEL_DIRECT)
+        c = eb.eval_fitness(d_off, d_ids)
+        torch.cuda.synchronize()
+        assert (c.cpu().numpy().view(np.uint64) == counts).all()
