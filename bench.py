@@ -168,6 +168,7 @@ def run_gpu(args):
     torch.cuda.synchronize()
     create_ms = (time.time() - t0) * 1e3
     eb.set_kernel(KERNELS[args.kernel])
+    eb.set_early_exit(args.early_exit)
     kernel_name = B.KERNEL_NAMES[eb.kernel]
 
     d_off = torch.from_numpy(w.offsets).cuda()
@@ -270,6 +271,7 @@ def run_gpu(args):
             "config": {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind,
                        "sum_L": int(w.lengths.sum()), "missing_mode": w.missing_mode, "kernel": kernel_name,
                        "tile_rows": eb.info(5), "ctas": eb.info(6), "n_chosen": int(len(chosen)),
+                       "early_exit": bool(args.early_exit),
                        "l2": "flushed between steps (256 MiB write)",
                        "parallelism": f"row-sharded x{world}, 1 all-reduce(int64[n_ind]) per step" if world > 1 else "1 GPU"},
             "individuals_rows_per_s": w.n_ind * w.rows * world / (ms_per_step * 1e-3),
@@ -376,11 +378,12 @@ def run_table(args):
         chosen = pick_chosen(w)
         d_chosen = torch.from_numpy(chosen).cuda()
         d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
-        for kname in ("rank8", "tiled_f32", "direct"):
+        for kname, ee in (("rank8", 0), ("rank8", 1), ("tiled_f32", 0), ("tiled_f32", 1), ("direct", 0)):
             if kname == "direct" and w.comparisons > 2e10:
                 continue
             try:
                 eb.set_kernel(KERNELS[kname])
+                eb.set_early_exit(ee)
             except B.EbicError:
                 continue
             reps = 5 if w.comparisons > 1e11 else 20
@@ -423,7 +426,9 @@ def run_table(args):
                 log("graph replay unavailable:", ex)
                 torch.cuda.synchronize()
             roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7))
-            rows_out.append({"workload": w.cfg.name, "kernel": kname, "call_ms_median": statistics.median(call_ms),
+            rows_out.append({"workload": w.cfg.name, "kernel": kname, "early_exit": ee,
+                             "executed_over_nominal_visits": visits / (eb.ld * int(w.lengths.sum())),
+                             "call_ms_median": statistics.median(call_ms),
                              "kernel_ms": kernel_ms, "graph_replay_ms": graph_ms,
                              "comparisons_per_s": w.comparisons / (statistics.median(call_ms) * 1e-3),
                              "comparisons_per_s_kernel": w.comparisons / (kernel_ms * 1e-3),
@@ -474,6 +479,9 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of CPU work for cpu_baseline")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the fitness kernel from an ncu --set full capture")
+    ap.add_argument("--early-exit", type=int, default=0, dest="early_exit",
+                    help="1: let warps stop a chromosome once no row can match (fewer executed visits); "
+                         "0 (default for the headline): plain work, every column of every chromosome visited")
     ap.add_argument("--table", action="store_true")
     ap.add_argument("--table-workloads", default="c1,c2,c3,c4,c5")
     args = ap.parse_args()

@@ -113,6 +113,14 @@ int ebic_status(ebic_ctx *ctx, void *cuda_stream);
 int ebic_set_kernel(ebic_ctx *ctx, int32_t kernel);
 
 /*
+ * Early exit (default on): a warp stops walking a chromosome once none of the rows it holds can still
+ * match.  Results are identical; only the number of executed column visits changes (on random
+ * populations most rows fail within the first few columns).  Off = every column of every chromosome
+ * is visited for every row ("plain work": executed visits == rows * sum(L)).
+ */
+int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
+
+/*
  * Instrumentation for roofline accounting.  `on` is a bit set:
  *   bit 0  the tiled fitness kernels add the number of (row, column-visit) operand fetches they
  *          actually executed to a device counter (one extra global atomic per warp);
@@ -132,7 +140,7 @@ int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
  *   use, 5 rows per shared-memory tile of that kernel, 6 CTAs of its last launch, 7 SM count,
  *   8 kernels launched by this context so far, 9 bytes of device memory the context owns,
  *   10 executed column visits since the last read, 11 mean fitness-kernel time in ns, 12 evals
- *   timed (see ebic_set_instrumentation).
+ *   timed (see ebic_set_instrumentation), 13 early exit on/off.
  * Returns -1 for NULL / unknown `what`.
  */
 int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);

@@ -43,6 +43,7 @@ SYMBOLS = {
     "ebic_mask_words": (_i64, [_vp]),
     "ebic_status": (ctypes.c_int, [_vp, _vp]),
     "ebic_set_kernel": (ctypes.c_int, [_vp, _i32]),
+    "ebic_set_early_exit": (ctypes.c_int, [_vp, _i32]),
     "ebic_set_instrumentation": (ctypes.c_int, [_vp, _i32]),
     "ebic_get_info": (_i64, [_vp, _i32]),
     "ebic_debug_read": (ctypes.c_int, [_vp, _i32, _vp, _i64]),
@@ -120,6 +121,10 @@ def ebic_set_kernel(ctx, kernel: int) -> None:
     st = load_library().ebic_set_kernel(ctx, kernel)
     if st != EBIC_OK:
         raise EbicError(st, "ebic_set_kernel")
+
+
+def ebic_set_early_exit(ctx, on: bool) -> None:
+    load_library().ebic_set_early_exit(ctx, 1 if on else 0)
 
 
 def ebic_set_instrumentation(ctx, on: int) -> None:
@@ -253,6 +258,9 @@ class Ebic:
 
     def set_kernel(self, kernel: int) -> None:
         ebic_set_kernel(self._ctx, kernel)
+
+    def set_early_exit(self, on: bool) -> None:
+        ebic_set_early_exit(self._ctx, on)
 
     def set_instrumentation(self, on: int) -> None:
         ebic_set_instrumentation(self._ctx, on)

@@ -38,6 +38,9 @@ struct ebic_ctx {
     int64_t meta_cap = 0;
     int32_t* pids = nullptr;
     int64_t pids_cap = 0;
+    uint8_t* pids8 = nullptr;               // packed byte ids for the tiled kernels (cols <= 256)
+    int64_t pids8_cap = 0;
+    int32_t early_exit = 1;
     // staging for host-pointer calls
     void* stage[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     int64_t stage_cap[5] = {0, 0, 0, 0, 0};
@@ -120,6 +123,7 @@ int32_t pick_tile_rows(const ebic_ctx* ctx, int32_t elem, int32_t quantum, int32
 }
 
 int32_t tile_rows_f32(const ebic_ctx* ctx, int32_t n_ind_launch) {
+    if (ctx->cols > 256) return 0;          // the tiled kernels read byte ids
     return pick_tile_rows(ctx, 4, kRowsPerSlabF32, 1024, n_ind_launch);
 }
 int32_t tile_rows_r8(const ebic_ctx* ctx, int32_t n_ind_launch) {
@@ -150,8 +154,9 @@ int launch_tiled(ebic_ctx* ctx, const void* M, int32_t T, const int2* meta, int3
     p.T = T;
     p.n_tiles = (ctx->ld + T - 1) / T;
     p.meta = meta;
-    p.pids4 = reinterpret_cast<const int4*>(ctx->pids);
+    p.idw = reinterpret_cast<const uint32_t*>(ctx->pids8);
     p.n_ind = n_ind;
+    p.early_exit = ctx->early_exit;
     p.counts = counts;
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
     const size_t smem = tiled_smem_bytes(ctx->cols, T, sizeof(typename E::type), n_ind);
@@ -174,10 +179,14 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     if (st) return st;
     st = grow(ctx, reinterpret_cast<void**>(&ctx->pids), &ctx->pids_cap, (n_ids + 3ll * n_ind + 8) * 4);
     if (st) return st;
+    if (ctx->cols <= 256) {
+        st = grow(ctx, reinterpret_cast<void**>(&ctx->pids8), &ctx->pids8_cap, n_ids + 3ll * n_ind + 8);
+        if (st) return st;
+    }
 
     ingest_population_kernel<<<(n_ind + 255) / 256, 256, 0, stream>>>(
         offsets, col_ids, n_ind, n_ids, ctx->cols, ctx->rows, ctx->missing_mode == EBIC_MISSING_ON,
-        ctx->nonmissing, ctx->meta, ctx->pids, counts, ctx->d_err);
+        ctx->nonmissing, ctx->meta, ctx->pids, ctx->cols <= 256 ? ctx->pids8 : nullptr, counts, ctx->d_err);
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());
 
@@ -338,6 +347,7 @@ int ebic_destroy(ebic_ctx* ctx) {
     cudaFree(ctx->d_err);
     cudaFree(ctx->meta);
     cudaFree(ctx->pids);
+    cudaFree(ctx->pids8);
     for (void* s : ctx->stage) cudaFree(s);
     for (int i = 0; i < ebic_ctx::kTimingRing; ++i) {
         if (ctx->ev_begin[i]) cudaEventDestroy(ctx->ev_begin[i]);
@@ -456,6 +466,12 @@ int ebic_set_kernel(ebic_ctx* ctx, int32_t kernel) {
     return EBIC_OK;
 }
 
+int ebic_set_early_exit(ebic_ctx* ctx, int32_t on) {
+    if (!ctx) return EBIC_ERR_ARG;
+    ctx->early_exit = on ? 1 : 0;
+    return EBIC_OK;
+}
+
 int ebic_set_instrumentation(ebic_ctx* ctx, int32_t on) {
     if (!ctx) return EBIC_ERR_ARG;
     ctx->count_visits = (on & 1) ? 1 : 0;
@@ -505,6 +521,7 @@ int64_t ebic_get_info(ebic_ctx* ctx, int32_t what) {
             return static_cast<int64_t>(total_ms / n * 1e6);
         }
         case 12: return ctx->timed_evals;
+        case 13: return ctx->early_exit;
         default: return -1;
     }
 }

@@ -57,6 +57,14 @@ __device__ __forceinline__ void bulk_copy_g2s(void* smem_dst, const void* gmem_s
         : "memory");
 }
 
+// 128-bit shared-memory load from a 32-bit shared-window address (SASS: LDS.128 [R+imm]): the address
+// comes straight out of one IMAD (id * column stride + lane base), no generic-pointer arithmetic.
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+
 __device__ __forceinline__ bool is_nan_bits(float v) {
     return (__float_as_uint(v) & 0x7fffffffu) > 0x7f800000u;
 }

@@ -12,11 +12,14 @@ namespace ebic {
 
 // ------------------------------------------------------------------------------------------------
 // a3  Population ingest + validation.  One thread per individual.
-//   meta[k] = { slot4, L }   slot4 = index (in int4 units) of the individual's padded id group in `pids`
-//                            L = chromosome length, or -1 if the individual is invalid.
-//   pids    = ids copied to a 16-byte aligned slot, padded to a multiple of 4 with the last id, so the
-//             chain kernels fetch four ids with one uniform 128-bit load.  Slot of individual k starts
-//             at (offsets[k] + 3k) & ~3: disjoint from its neighbours without a prefix sum.
+//   meta[k] = { slot4, L }   slot4 = index, in 4-entry groups, of the individual's id slot; L = chromosome
+//                            length, or -1 if the individual is invalid.
+//   pids    = int32 ids copied to the slot (entries 4*slot4 ..), padded to a multiple of 4 with the last id
+//             (read by the DIRECT kernel);
+//   pids8   = the same ids as bytes (bytes 4*slot4 ..), written when cols <= 256: the tiled kernels fetch
+//             four ids with one warp-uniform 32-bit load.
+//   The slot of individual k starts at entry (offsets[k] + 3k) & ~3: 4-aligned and disjoint from its
+//   neighbours without a prefix sum.
 //   counts[k] is initialised: rows (L = 0, or L = 1 in mode OFF), non-missing rows of the column
 //             (L = 1, mode ON), else 0 -- the chain kernels then add to it.
 // ------------------------------------------------------------------------------------------------
@@ -24,8 +27,8 @@ __global__ void __launch_bounds__(256)
 ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __restrict__ col_ids,
                          int32_t n_ind, int64_t n_ids, int32_t cols, int64_t rows, int32_t missing_on,
                          const unsigned long long* __restrict__ nonmissing, int2* __restrict__ meta,
-                         int32_t* __restrict__ pids, unsigned long long* __restrict__ counts,
-                         int32_t* __restrict__ err)
+                         int32_t* __restrict__ pids, uint8_t* __restrict__ pids8,
+                         unsigned long long* __restrict__ counts, int32_t* __restrict__ err)
 {
     const int32_t k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n_ind) return;
@@ -38,6 +41,7 @@ ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __r
     }
     const int32_t L = e - b;
     const int64_t slot = (static_cast<int64_t>(b) + 3ll * k) & ~3ll;
+    const bool bytes = pids8 != nullptr;
     bool bad = false;
     int32_t last = 0;
     for (int32_t i = 0; i < L; ++i) {
@@ -47,9 +51,13 @@ ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __r
             id = 0;
         }
         pids[slot + i] = id;
+        if (bytes) pids8[slot + i] = static_cast<uint8_t>(id);
         last = id;
     }
-    for (int32_t i = L; i < ((L + 3) & ~3); ++i) pids[slot + i] = last;
+    for (int32_t i = L; i < ((L + 3) & ~3); ++i) {
+        pids[slot + i] = last;
+        if (bytes) pids8[slot + i] = static_cast<uint8_t>(last);
+    }
     if (bad) {
         meta[k] = make_int2(static_cast<int32_t>(slot >> 2), -1);
         counts[k] = 0;
@@ -109,14 +117,15 @@ fitness_direct_kernel(const float* __restrict__ Mc, int64_t ld, const int2* __re
 // Per-CTA counters are uint32: a CTA sees < 2^31 rows, so they cannot overflow.
 // ------------------------------------------------------------------------------------------------
 struct TiledParams {
-    const void* M;                   // column-major [cols][ld] (float or uint8 ranks)
+    const void* M;                   // column-major [cols][ld] (float or uint8 rank codes)
     int64_t ld;
     int32_t cols;
     int32_t T;                       // rows per tile (multiple of the slab size)
     int64_t n_tiles;                 // ceil(ld / T)
     const int2* meta;                // [n_ind] of this launch's population chunk
-    const int4* pids4;
+    const uint32_t* idw;             // packed ids, four uint8 per word (pids8 viewed as words)
     int32_t n_ind;                   // individuals in this launch (<= kMaxIndPerLaunch)
+    int32_t early_exit;              // stop a chain once no row of the warp's slab group is alive
     unsigned long long* counts;      // [n_ind]
     unsigned long long* visits;      // executed column visits (instrumented build) or nullptr
 };
@@ -129,131 +138,190 @@ __host__ __device__ inline size_t tiled_smem_bytes(int32_t cols, int32_t T, int3
     return kSmemHeader + cnt + 2 * static_cast<size_t>(cols) * T * elem;
 }
 
-// ---- a5 on float32: 4 rows per lane, one LDS.128 + 4 FSETP.GE.AND per column -------------------
-__device__ __forceinline__ int chain_f32(const float* base, int32_t T, int4 g, const int4* gp, int32_t L)
-{
-    float4 prev = *reinterpret_cast<const float4*>(base + g.x * T);
-    bool p0 = true, p1 = true, p2 = true, p3 = true;
-#define EBIC_STEP_F32(ID)                                                         \
-    {                                                                             \
-        const float4 cur = *reinterpret_cast<const float4*>(base + (ID) * T);     \
-        p0 = p0 & (cur.x >= prev.x);                                              \
-        p1 = p1 & (cur.y >= prev.y);                                              \
-        p2 = p2 & (cur.z >= prev.z);                                              \
-        p3 = p3 & (cur.w >= prev.w);                                              \
-        prev = cur;                                                               \
-    }
-    EBIC_STEP_F32(g.y);
-    if (L > 2) {
-        EBIC_STEP_F32(g.z);
-        if (L > 3) EBIC_STEP_F32(g.w);
-    }
-    for (int32_t i = 4; i < L; i += 4) {
-        g = __ldg(++gp);
-        EBIC_STEP_F32(g.x);
-        if (i + 1 < L) {
-            EBIC_STEP_F32(g.y);
-            if (i + 2 < L) {
-                EBIC_STEP_F32(g.z);
-                if (i + 3 < L) EBIC_STEP_F32(g.w);
-            }
-        }
-    }
-#undef EBIC_STEP_F32
-    return static_cast<int>(p0) + static_cast<int>(p1) + static_cast<int>(p2) + static_cast<int>(p3);
+__device__ __forceinline__ uint32_t id_byte(uint32_t w, int b) {   // b is a compile-time constant: one PRMT
+    return __byte_perm(w, 0, 0x4440 + b);
 }
 
-// ---- a5 on rank codes: 16 rows per lane and slab, NS slabs per id fetch ------------------------
-// code = 0x80|rank (rank <= 126) or 0x7F (missing).  Per byte: cur - prev + 0x80 stays in [1, 255]
-// for every code pair, so the 32-bit IADD3 never carries between bytes, and its bit 7 is set iff
-// rank(cur) >= rank(prev) when both are values.  AND-ing with `cur` clears bit 7 when cur is missing;
-// a missing prev was already cleared one step earlier (acc starts as the first column's code).
+// ---- a5 on float32: 4 rows per lane and slab: one LDS.128 + 4 FSETP.GE.AND per column -----------
+struct ChainF32 {
+    uint32_t base;                   // shared address of tile + (slab * 128 + lane * 4) * 4
+    uint32_t stride;                 // bytes between columns of the tile = T * 4
+    float4 prev;
+    bool p0, p1, p2, p3;
+    __device__ __forceinline__ float4 load(uint32_t id) const {
+        const uint4 v = lds128(id * stride + base);
+        return make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
+    }
+    __device__ __forceinline__ void init(uint32_t id) {
+        prev = load(id);
+        p0 = p1 = p2 = p3 = true;
+    }
+    __device__ __forceinline__ void step(uint32_t id) {
+        const float4 cur = load(id);
+        p0 = p0 & (cur.x >= prev.x);
+        p1 = p1 & (cur.y >= prev.y);
+        p2 = p2 & (cur.z >= prev.z);
+        p3 = p3 & (cur.w >= prev.w);
+        prev = cur;
+    }
+    __device__ __forceinline__ bool alive() const { return p0 | p1 | p2 | p3; }
+    __device__ __forceinline__ int count() const {
+        return static_cast<int>(p0) + static_cast<int>(p1) + static_cast<int>(p2) + static_cast<int>(p3);
+    }
+};
+
+// ---- a5 on rank codes: 16 rows per lane and slab, NS slabs per id fetch -------------------------
+// code = 0x80|rank (rank <= 126) or 0x7F (missing).  Per byte: cur - prev + 0x80 stays in [1, 255] for
+// every code pair, so the 32-bit IADD3 never carries between bytes, and its bit 7 is set iff
+// rank(cur) >= rank(prev) when both are values.  AND-ing with `cur` clears bit 7 when cur is missing; a
+// missing prev was already cleared one step earlier (acc starts as the first column's code).
 template <int NS>
-__device__ __forceinline__ int chain_r8(const uint8_t* base, int32_t T, int4 g, const int4* gp, int32_t L)
-{
-    constexpr unsigned int H = 0x80808080u;
+struct ChainR8 {
+    static constexpr unsigned int H = 0x80808080u;
+    uint32_t base;                   // shared address of tile + slab * 512 + lane * 16
+    uint32_t stride;                 // bytes between columns of the tile = T
     uint4 prev[NS], acc[NS];
-    {
-        const uint8_t* col = base + g.x * T;
+    __device__ __forceinline__ void init(uint32_t id) {
+        const uint32_t col = id * stride + base;
 #pragma unroll
         for (int s = 0; s < NS; ++s) {
-            prev[s] = *reinterpret_cast<const uint4*>(col + s * kRowsPerSlabR8);
+            prev[s] = lds128(col + s * kRowsPerSlabR8);
             acc[s] = prev[s];
         }
     }
-#define EBIC_STEP_R8(ID)                                                                   \
-    {                                                                                      \
-        const uint8_t* col = base + (ID) * T;                                              \
-        _Pragma("unroll") for (int s = 0; s < NS; ++s) {                                   \
-            const uint4 cur = *reinterpret_cast<const uint4*>(col + s * kRowsPerSlabR8);   \
-            acc[s].x &= (cur.x - prev[s].x + H) & cur.x;                                   \
-            acc[s].y &= (cur.y - prev[s].y + H) & cur.y;                                   \
-            acc[s].z &= (cur.z - prev[s].z + H) & cur.z;                                   \
-            acc[s].w &= (cur.w - prev[s].w + H) & cur.w;                                   \
-            prev[s] = cur;                                                                 \
-        }                                                                                  \
-    }
-    EBIC_STEP_R8(g.y);
-    if (L > 2) {
-        EBIC_STEP_R8(g.z);
-        if (L > 3) EBIC_STEP_R8(g.w);
-    }
-    for (int32_t i = 4; i < L; i += 4) {
-        g = __ldg(++gp);
-        EBIC_STEP_R8(g.x);
-        if (i + 1 < L) {
-            EBIC_STEP_R8(g.y);
-            if (i + 2 < L) {
-                EBIC_STEP_R8(g.z);
-                if (i + 3 < L) EBIC_STEP_R8(g.w);
-            }
+    __device__ __forceinline__ void step(uint32_t id) {
+        const uint32_t col = id * stride + base;
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const uint4 cur = lds128(col + s * kRowsPerSlabR8);
+            acc[s].x &= (cur.x - prev[s].x + H) & cur.x;
+            acc[s].y &= (cur.y - prev[s].y + H) & cur.y;
+            acc[s].z &= (cur.z - prev[s].z + H) & cur.z;
+            acc[s].w &= (cur.w - prev[s].w + H) & cur.w;
+            prev[s] = cur;
         }
     }
-#undef EBIC_STEP_R8
-    int total = 0;
+    __device__ __forceinline__ bool alive() const {
+        unsigned int any = 0;
 #pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        const unsigned int m = (acc[s].x & H) | ((acc[s].y & H) >> 1) | ((acc[s].z & H) >> 2) | ((acc[s].w & H) >> 3);
-        total += __popc(m);
+        for (int s = 0; s < NS; ++s) any |= acc[s].x | acc[s].y | acc[s].z | acc[s].w;
+        return (any & H) != 0;
     }
-    return total;
+    __device__ __forceinline__ int count() const {
+        int total = 0;
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const unsigned int m = (acc[s].x & H) | ((acc[s].y & H) >> 1) | ((acc[s].z & H) >> 2) | ((acc[s].w & H) >> 3);
+            total += __popc(m);
+        }
+        return total;
+    }
+};
+
+// One chromosome on one slab group.  ids arrive four per word; w0 = first word (already loaded),
+// idw points at it.  Full words run branch-free; the (at most two) ragged words go byte by byte.
+// Returns the number of matching rows; adds the number of columns actually visited to `steps`.
+template <class C>
+__device__ __forceinline__ int run_chain(C& c, const uint32_t* __restrict__ idw, uint32_t w0, int32_t L,
+                                         bool early_exit, int32_t& steps)
+{
+    uint32_t w = w0;
+    uint32_t wn = (L > 4) ? __ldg(idw + 1) : 0u;
+    c.init(id_byte(w, 0));
+    int32_t rem = L - 1;                                  // steps still to do; L >= 2
+    int32_t done = 1;
+    {                                                     // bytes 1..3 of word 0
+        c.step(id_byte(w, 1));
+        if (rem >= 2) c.step(id_byte(w, 2));
+        if (rem >= 3) c.step(id_byte(w, 3));
+        const int32_t n0 = min(rem, 3);
+        rem -= n0;
+        done += n0;
+    }
+    int32_t j = 1;
+    while (rem > 0) {
+        if (early_exit && !__any_sync(0xffffffffu, c.alive())) break;
+        w = wn;
+        if (rem > 4) wn = __ldg(idw + j + 1);
+        ++j;
+        if (rem >= 4) {
+            c.step(id_byte(w, 0));
+            c.step(id_byte(w, 1));
+            c.step(id_byte(w, 2));
+            c.step(id_byte(w, 3));
+            rem -= 4;
+            done += 4;
+        } else {
+            c.step(id_byte(w, 0));
+            if (rem >= 2) c.step(id_byte(w, 1));
+            if (rem >= 3) c.step(id_byte(w, 2));
+            done += rem;
+            rem = 0;
+        }
+    }
+    steps += done;
+    return c.count();
 }
 
 struct ElemF32 {
     using type = float;
     static constexpr int kSlabRows = kRowsPerSlabF32;
-    static constexpr int kLaneElems = 4;
 };
 struct ElemR8 {
     using type = uint8_t;
     static constexpr int kSlabRows = kRowsPerSlabR8;
-    static constexpr int kLaneElems = 16;
 };
 
+// All slabs of the tile for one individual.  Returns matches; `visited` += rows * columns actually visited.
 template <class E>
-__device__ __forceinline__ int eval_individual_on_tile(const typename E::type* tile, int32_t T, int32_t nslabs,
-                                                        int lane, int4 g0, const int4* gp, int32_t L);
+__device__ __forceinline__ int eval_individual_on_tile(const typename E::type* tile, int32_t T, int32_t nslabs, int lane,
+                                                        const uint32_t* idw, uint32_t w0, int32_t L, bool early_exit,
+                                                        unsigned long long& visited);
 
 template <>
-__device__ __forceinline__ int eval_individual_on_tile<ElemF32>(const float* tile, int32_t T, int32_t nslabs,
-                                                                int lane, int4 g0, const int4* gp, int32_t L)
+__device__ __forceinline__ int eval_individual_on_tile<ElemF32>(const float* tile, int32_t T, int32_t nslabs, int lane,
+                                                                const uint32_t* idw, uint32_t w0, int32_t L,
+                                                                bool early_exit, unsigned long long& visited)
 {
     int cnt = 0;
-    const float* base = tile + lane * 4;
-    for (int32_t s = 0; s < nslabs; ++s) cnt += chain_f32(base + s * kRowsPerSlabF32, T, g0, gp, L);
+    int32_t steps = 0;
+    for (int32_t s = 0; s < nslabs; ++s) {
+        ChainF32 c;
+        c.base = smem_u32(tile) + (s * kRowsPerSlabF32 + lane * 4) * 4;
+        c.stride = static_cast<uint32_t>(T) * 4;
+        cnt += run_chain(c, idw, w0, L, early_exit, steps);
+    }
+    visited += static_cast<unsigned long long>(steps) * kRowsPerSlabF32;
     return cnt;
 }
 
 template <>
-__device__ __forceinline__ int eval_individual_on_tile<ElemR8>(const uint8_t* tile, int32_t T, int32_t nslabs,
-                                                               int lane, int4 g0, const int4* gp, int32_t L)
+__device__ __forceinline__ int eval_individual_on_tile<ElemR8>(const uint8_t* tile, int32_t T, int32_t nslabs, int lane,
+                                                               const uint32_t* idw, uint32_t w0, int32_t L,
+                                                               bool early_exit, unsigned long long& visited)
 {
     int cnt = 0;
-    const uint8_t* base = tile + lane * 16;
     int32_t s = 0;
-    for (; s + 4 <= nslabs; s += 4) cnt += chain_r8<4>(base + s * kRowsPerSlabR8, T, g0, gp, L);
-    for (; s + 2 <= nslabs; s += 2) cnt += chain_r8<2>(base + s * kRowsPerSlabR8, T, g0, gp, L);
-    for (; s < nslabs; ++s) cnt += chain_r8<1>(base + s * kRowsPerSlabR8, T, g0, gp, L);
+    int32_t steps4 = 0, steps2 = 0, steps1 = 0;
+    for (; s + 4 <= nslabs; s += 4) {
+        ChainR8<4> c;
+        c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
+        c.stride = static_cast<uint32_t>(T);
+        cnt += run_chain(c, idw, w0, L, early_exit, steps4);
+    }
+    for (; s + 2 <= nslabs; s += 2) {
+        ChainR8<2> c;
+        c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
+        c.stride = static_cast<uint32_t>(T);
+        cnt += run_chain(c, idw, w0, L, early_exit, steps2);
+    }
+    for (; s < nslabs; ++s) {
+        ChainR8<1> c;
+        c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
+        c.stride = static_cast<uint32_t>(T);
+        cnt += run_chain(c, idw, w0, L, early_exit, steps1);
+    }
+    visited += static_cast<unsigned long long>(4 * steps4 + 2 * steps2 + steps1) * kRowsPerSlabR8;
     return cnt;
 }
 
@@ -307,6 +375,7 @@ fitness_tiled_kernel(const TiledParams p)
     } else {
         // ---------------- consumer warps (a5, a6) ----------------
         unsigned long long visited = 0;
+        const bool early_exit = p.early_exit != 0;
         for (int32_t j = 0; j < ntl; ++j) {
             const int buf = j & 1;
             const int64_t r0 = (t0 + j) * p.T;
@@ -315,16 +384,26 @@ fitness_tiled_kernel(const TiledParams p)
             const int32_t ka = (j == 0) ? static_cast<int32_t>(pb - t0 * p.n_ind) : 0;
             const int32_t kb = (j == ntl - 1) ? static_cast<int32_t>(pe - t1 * p.n_ind) : p.n_ind;
             const elem_t* tile = tiles + buf * tile_elems;
+            // software pipeline over this warp's individuals: meta two ahead, first id word one ahead
+            int32_t k = ka + warp;
+            int2 m_cur = make_int2(0, 0), m_next = make_int2(0, 0);
+            uint32_t w_cur = 0;
+            if (k < kb) {
+                m_cur = __ldg(&p.meta[k]);
+                w_cur = __ldg(p.idw + m_cur.x);
+            }
+            if (k + NCONS < kb) m_next = __ldg(&p.meta[k + NCONS]);
             mbar_wait(&full[buf], (j >> 1) & 1);
-            for (int32_t k = ka + warp; k < kb; k += NCONS) {
-                const int2 m = __ldg(&p.meta[k]);
+            for (; k < kb; k += NCONS) {
+                const int2 m = m_cur;
+                const uint32_t w0 = w_cur;
+                m_cur = m_next;
+                if (k + NCONS < kb) w_cur = __ldg(p.idw + m_cur.x);
+                if (k + 2 * NCONS < kb) m_next = __ldg(&p.meta[k + 2 * NCONS]);
                 if (m.y < 2) continue;
-                const int4* gp = p.pids4 + m.x;
-                const int4 g0 = __ldg(gp);
-                int cnt = eval_individual_on_tile<E>(tile, p.T, nslabs, lane, g0, gp, m.y);
+                int cnt = eval_individual_on_tile<E>(tile, p.T, nslabs, lane, p.idw + m.x, w0, m.y, early_exit, visited);
                 cnt = __reduce_add_sync(0xffffffffu, cnt);
                 if (lane == 0 && cnt) atomicAdd(&s_cnt[k], static_cast<unsigned int>(cnt));
-                visited += static_cast<unsigned long long>(m.y) * nrows;
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[buf]);

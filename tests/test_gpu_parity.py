@@ -72,9 +72,12 @@ def check_all(B, oracle_mod, matrix, mode, off, ids, chosen=None, expect_status=
     assert st == expect_status
     with B.Ebic(matrix, mode) as eb:
         for kern in kernels_for(eb, B):
-            got = gpu_counts(eb, B, off, ids, kern)
-            assert (got == want).all(), (B.KERNEL_NAMES[kern], np.flatnonzero(got != want)[:10])
-            assert eb.status() == expect_status
+            for early_exit in ((True, False) if kern != B.EBIC_KERNEL_DIRECT else (True,)):
+                eb.set_early_exit(early_exit)
+                got = gpu_counts(eb, B, off, ids, kern)
+                assert (got == want).all(), (B.KERNEL_NAMES[kern], early_exit, np.flatnonzero(got != want)[:10])
+                assert eb.status() == expect_status
+        eb.set_early_exit(True)
         n_ind = off.size - 1
         if chosen is None:
             chosen = np.arange(n_ind, dtype=np.int32)
@@ -257,16 +260,21 @@ def test_host_pointers_and_streams(B, oracle_mod):
         assert (host.numpy().view(np.uint64) == want).all()
 
 
-def test_instrumentation_counts_nominal_visits(B):
+def test_instrumentation_counts_executed_visits(B):
     w = W.make_workload(2, rows=20_000, n_ind=200)
     with B.Ebic(w.matrix, w.missing_mode) as eb:
+        nominal = eb.ld * int(w.lengths.sum())
         for kern in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8):
             eb.set_kernel(kern)
-            eb.set_instrumentation(True)
-            eb.eval_fitness(dev(w.offsets), dev(w.col_ids))
-            visits = eb.info(10)
-            eb.set_instrumentation(False)
-            assert visits == eb.ld * int(w.lengths.sum())          # no work skipped: executed == nominal
+            seen = {}
+            for early_exit in (False, True):
+                eb.set_early_exit(early_exit)
+                eb.set_instrumentation(1)
+                eb.eval_fitness(dev(w.offsets), dev(w.col_ids))
+                seen[early_exit] = eb.info(10)
+                eb.set_instrumentation(0)
+            assert seen[False] == nominal                          # plain work: executed == nominal
+            assert 2 * eb.ld * w.n_ind <= seen[True] <= nominal    # early exit only ever skips columns
 
 
 # ------------------------------------------------------------------------- full-size C5 (bench config)
