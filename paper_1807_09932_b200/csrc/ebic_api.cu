@@ -111,6 +111,12 @@ bool is_device_pointer(const void* p) {
 constexpr int kConsF32 = 31;   // consumer warps of the TILED_F32 kernel (+1 producer = 1024 threads)
 constexpr int kConsR8 = 15;    // consumer warps of the RANK8 kernel     (+1 producer =  512 threads)
 
+// Experiment knob (not part of the ABI): EBIC_R8_CONS=23 selects the 24-warp RANK8 build.
+int env_int(const char* name, int dflt) {
+    const char* v = std::getenv(name);
+    return v ? std::atoi(v) : dflt;
+}
+
 // Rows per tile: largest multiple of `quantum` that double-buffers into shared memory, <= cap.
 int32_t pick_tile_rows(const ebic_ctx* ctx, int32_t elem, int32_t quantum, int32_t cap, int32_t n_ind_launch) {
     const int64_t cnt = (static_cast<int64_t>(n_ind_launch) * 4 + 127) & ~127ll;
@@ -204,7 +210,11 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         if (kernel == EBIC_KERNEL_RANK8) {
             const int32_t T = tile_rows_r8(ctx, n);
             if (T <= 0) return EBIC_ERR_ARG;
-            st = launch_tiled<ElemR8, kConsR8>(ctx, ctx->Rk, T, ctx->meta + k0, n, counts + k0, stream);
+            static const int r8_cons = env_int("EBIC_R8_CONS", kConsR8);
+            if (r8_cons == 23)
+                st = launch_tiled<ElemR8, 23>(ctx, ctx->Rk, T, ctx->meta + k0, n, counts + k0, stream);
+            else
+                st = launch_tiled<ElemR8, kConsR8>(ctx, ctx->Rk, T, ctx->meta + k0, n, counts + k0, stream);
         } else if (kernel == EBIC_KERNEL_TILED_F32) {
             const int32_t T = tile_rows_f32(ctx, n);
             if (T <= 0) return EBIC_ERR_ARG;

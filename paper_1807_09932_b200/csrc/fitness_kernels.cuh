@@ -171,10 +171,14 @@ struct ChainF32 {
 };
 
 // ---- a5 on rank codes: 16 rows per lane and slab, NS slabs per id fetch -------------------------
-// code = 0x80|rank (rank <= 126) or 0x7F (missing).  Per byte: cur - prev + 0x80 stays in [1, 255] for
-// every code pair, so the 32-bit IADD3 never carries between bytes, and its bit 7 is set iff
-// rank(cur) >= rank(prev) when both are values.  AND-ing with `cur` clears bit 7 when cur is missing; a
-// missing prev was already cleared one step earlier (acc starts as the first column's code).
+// code = 0x80|rank (rank <= 126) or 0x7F (missing).  Per byte t = cur - prev + 0x80 stays in [1, 255] for
+// every code pair, so the 32-bit IADD3 never carries between bytes.  Bit 7 of t:
+//   value, value   : 0x80 + rank(cur) - rank(prev)      -> set iff rank(cur) >= rank(prev)
+//   missing, value : 0x7F - rank(prev) in [1, 127]       -> clear (the pair fails, as an ordered >= does)
+//   value, missing : 0x81 + rank(cur)                    -> set, but the chain has already failed:
+//   missing,missing: 0x80                                -> set,  the FIRST missing column of a chain is
+//                    either column 0 (acc starts as its code, bit 7 clear) or follows a value (case 2).
+// acc = AND of all t (and the first code): bit 7 of each byte = ok(k, r) for that row.
 template <int NS>
 struct ChainR8 {
     static constexpr unsigned int H = 0x80808080u;
@@ -194,10 +198,10 @@ struct ChainR8 {
 #pragma unroll
         for (int s = 0; s < NS; ++s) {
             const uint4 cur = lds128(col + s * kRowsPerSlabR8);
-            acc[s].x &= (cur.x - prev[s].x + H) & cur.x;
-            acc[s].y &= (cur.y - prev[s].y + H) & cur.y;
-            acc[s].z &= (cur.z - prev[s].z + H) & cur.z;
-            acc[s].w &= (cur.w - prev[s].w + H) & cur.w;
+            acc[s].x &= cur.x - prev[s].x + H;
+            acc[s].y &= cur.y - prev[s].y + H;
+            acc[s].z &= cur.z - prev[s].z + H;
+            acc[s].w &= cur.w - prev[s].w + H;
             prev[s] = cur;
         }
     }
