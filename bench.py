@@ -41,7 +41,7 @@ METRIC = "row_pair_comparisons_per_s"
 UNIT = "comparisons/s"
 N_CHOSEN = 8
 WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4}
-KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3}
+KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "pairbits_smem": 5}
 
 
 def log(*a):
@@ -123,7 +123,7 @@ def pick_chosen(w):
 def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None):
     f_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     smem_peak_gbs = sm_count * 128 * f_hz / 1e9            # 128 B / clk / SM shared-memory data pipe
-    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "direct": 4}[kernel_name]
+    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "direct": 4, "pairbits": 0.125, "pairbits_smem": 0.125}[kernel_name]
     achieved = visits_executed * bytes_per_visit / kernel_s / 1e9
     return {"bound": "alu", "resource": "shared-memory data pipe (128 B/clk/SM) == ALU pipe at 0.5 op/visit"
             if kernel_name == "rank8" else "shared-memory data pipe (128 B/clk/SM)",
@@ -378,7 +378,8 @@ def run_table(args):
         chosen = pick_chosen(w)
         d_chosen = torch.from_numpy(chosen).cuda()
         d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
-        for kname, ee in (("rank8", 0), ("rank8", 1), ("tiled_f32", 0), ("tiled_f32", 1), ("direct", 0)):
+        for kname, ee in (("pairbits_smem", 0), ("pairbits", 0), ("pairbits", 1), ("rank8", 0), ("rank8", 1),
+                          ("tiled_f32", 0), ("tiled_f32", 1), ("direct", 0)):
             if kname == "direct" and w.comparisons > 2e10:
                 continue
             try:
@@ -392,6 +393,7 @@ def run_table(args):
             eb.set_instrumentation(1)
             eb.eval_fitness(d_off, d_ids, counts=d_counts)
             visits = eb.info(10) if kname != "direct" else eb.ld * int(w.lengths.sum())
+            nominal = eb.ld * int((w.lengths - 1).sum() if kname.startswith("pairbits") else w.lengths.sum())
             eb.set_instrumentation(2)
             call_ms = []
             for _ in range(reps):
@@ -427,7 +429,7 @@ def run_table(args):
                 torch.cuda.synchronize()
             roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7))
             rows_out.append({"workload": w.cfg.name, "kernel": kname, "early_exit": ee,
-                             "executed_over_nominal_visits": visits / (eb.ld * int(w.lengths.sum())),
+                             "executed_over_nominal_visits": visits / nominal,
                              "call_ms_median": statistics.median(call_ms),
                              "kernel_ms": kernel_ms, "graph_replay_ms": graph_ms,
                              "comparisons_per_s": w.comparisons / (statistics.median(call_ms) * 1e-3),

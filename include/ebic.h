@@ -49,10 +49,13 @@ enum { EBIC_MISSING_OFF = 0, EBIC_MISSING_ON = 1 };
 
 /* Kernel selection for ebic_eval_fitness (all give bit-identical counts). */
 enum {
-    EBIC_KERNEL_AUTO = 0,    /* fastest applicable: RANK8 if cols <= 127, else TILED_F32, else DIRECT */
+    EBIC_KERNEL_AUTO = 0,    /* fastest applicable: PAIRBITS_SMEM, PAIRBITS, RANK8, TILED_F32, DIRECT */
     EBIC_KERNEL_DIRECT = 1,  /* one thread per row, column-major global loads (any shape)          */
     EBIC_KERNEL_TILED_F32 = 2, /* float32 row tiles staged in shared memory by TMA bulk copies    */
-    EBIC_KERNEL_RANK8 = 3    /* per-row order-preserving 8-bit rank tiles (cols <= 127)           */
+    EBIC_KERNEL_RANK8 = 3,   /* per-row order-preserving 8-bit rank tiles (cols <= 127)           */
+    EBIC_KERNEL_PAIRBITS = 4, /* AND of pair-relation bitmasks streamed through L2 (pair table built) */
+    EBIC_KERNEL_PAIRBITS_SMEM = 5 /* the same, pair table of a 1024-row tile staged in shared memory
+                                     (cols^2 * 128 B must fit: cols <= about 42)                  */
 };
 
 /*
@@ -61,8 +64,10 @@ enum {
  *   rows          1 .. 2^31-1.        cols  1 .. 2^31-1 (memory permitting).
  *   missing_mode  EBIC_MISSING_OFF / EBIC_MISSING_ON.
  *   out           receives the context.
- * Transposes to column-major, builds the packed NaN bitmask and per-column non-missing counts and,
- * when cols <= 127, the 8-bit rank tiles.  Synchronous: `matrix` may be freed on return.
+ * Transposes to column-major, builds the packed NaN bitmask and per-column non-missing counts,
+ * when cols <= 127 the 8-bit rank tiles and, when it takes at most 8 GiB and half of the free device
+ * memory, the pair-relation table (cols^2 bits per padded row; see ebic_set_pairbits).
+ * Synchronous: `matrix` may be freed on return.
  * Errors: EBIC_ERR_ARG, EBIC_ERR_OOM, EBIC_ERR_CUDA (then *out == NULL).
  */
 int ebic_create(const float *matrix, int64_t rows, int32_t cols, int32_t missing_mode,
@@ -113,6 +118,17 @@ int ebic_status(ebic_ctx *ctx, void *cuda_stream);
 int ebic_set_kernel(ebic_ctx *ctx, int32_t kernel);
 
 /*
+ * Pair-relation table: bit r of pair (a,b) = ( M[r][b] >= M[r][a] ), cols^2 * ceil(rows/1024) * 128
+ * bytes of device memory.  With it an L >= 2 chromosome is the AND of its L-1 pair bitmasks (the
+ * PAIRBITS kernels; extraction reads it too).  on != 0 builds it if absent (EBIC_ERR_OOM if it does
+ * not fit; EBIC_ERR_ARG if cols > 46340), on == 0 frees it.  Synchronises the device.
+ */
+int ebic_set_pairbits(ebic_ctx *ctx, int32_t on);
+
+/* Extraction source: 1 (default) = the pair table when it exists, 0 = always the float32 columns. */
+int ebic_set_extract_source(ebic_ctx *ctx, int32_t use_pairbits);
+
+/*
  * Early exit (default on): a warp stops walking a chromosome once none of the rows it holds can still
  * match.  Results are identical; only the number of executed column visits changes (on random
  * populations most rows fail within the first few columns).  Off = every column of every chromosome
@@ -123,7 +139,8 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
 /*
  * Instrumentation for roofline accounting.  `on` is a bit set:
  *   bit 0  the tiled fitness kernels add the number of (row, column-visit) operand fetches they
- *          actually executed to a device counter (one extra global atomic per warp);
+ *          actually executed -- the PAIRBITS kernels the number of (row, pair) bit fetches -- to a
+ *          device counter (one extra global atomic per warp);
  *          ebic_get_info(ctx, 10) synchronises the device, returns the counter and resets it.
  *          Never on inside a timed region.
  *   bit 1  every ebic_eval_fitness brackets its fitness kernel launch(es) -- not the ingest kernel --
@@ -140,7 +157,7 @@ int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
  *   use, 5 rows per shared-memory tile of that kernel, 6 CTAs of its last launch, 7 SM count,
  *   8 kernels launched by this context so far, 9 bytes of device memory the context owns,
  *   10 executed column visits since the last read, 11 mean fitness-kernel time in ns, 12 evals
- *   timed (see ebic_set_instrumentation), 13 early exit on/off.
+ *   timed (see ebic_set_instrumentation), 13 early exit on/off, 14 bytes of the pair table (0 = absent).
  * Returns -1 for NULL / unknown `what`.
  */
 int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);
@@ -149,7 +166,8 @@ int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);
  * Read-back of loader products for parity tests (synchronous D2H copies on the legacy stream).
  *   ebic_debug_read(ctx, what, dst, dst_bytes): what = 0 column-major matrix float32 [cols][ld];
  *   1 NaN bitmask uint32 [cols][ld/32]; 2 per-column non-missing counts uint64 [cols];
- *   3 rank tiles uint8 [cols][ld] (EBIC_ERR_ARG if not built).
+ *   3 rank tiles uint8 [cols][ld] (EBIC_ERR_ARG if not built);
+ *   4 pair table uint32 [ld/1024][cols*cols][32] (EBIC_ERR_ARG if not built).
  *   dst_bytes must equal the product's size.
  */
 int ebic_debug_read(const ebic_ctx *ctx, int32_t what, void *dst, int64_t dst_bytes);

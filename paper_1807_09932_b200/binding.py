@@ -29,7 +29,9 @@ EBIC_KERNEL_AUTO = 0
 EBIC_KERNEL_DIRECT = 1
 EBIC_KERNEL_TILED_F32 = 2
 EBIC_KERNEL_RANK8 = 3
-KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8"}
+EBIC_KERNEL_PAIRBITS = 4
+EBIC_KERNEL_PAIRBITS_SMEM = 5
+KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits", 5: "pairbits_smem"}
 
 LIB_PATH = Path(__file__).resolve().parent / "libebic.so"
 
@@ -43,6 +45,8 @@ SYMBOLS = {
     "ebic_mask_words": (_i64, [_vp]),
     "ebic_status": (ctypes.c_int, [_vp, _vp]),
     "ebic_set_kernel": (ctypes.c_int, [_vp, _i32]),
+    "ebic_set_pairbits": (ctypes.c_int, [_vp, _i32]),
+    "ebic_set_extract_source": (ctypes.c_int, [_vp, _i32]),
     "ebic_set_early_exit": (ctypes.c_int, [_vp, _i32]),
     "ebic_set_instrumentation": (ctypes.c_int, [_vp, _i32]),
     "ebic_get_info": (_i64, [_vp, _i32]),
@@ -121,6 +125,16 @@ def ebic_set_kernel(ctx, kernel: int) -> None:
     st = load_library().ebic_set_kernel(ctx, kernel)
     if st != EBIC_OK:
         raise EbicError(st, "ebic_set_kernel")
+
+
+def ebic_set_pairbits(ctx, on: bool) -> None:
+    st = load_library().ebic_set_pairbits(ctx, 1 if on else 0)
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_set_pairbits")
+
+
+def ebic_set_extract_source(ctx, use_pairbits: bool) -> None:
+    load_library().ebic_set_extract_source(ctx, 1 if use_pairbits else 0)
 
 
 def ebic_set_early_exit(ctx, on: bool) -> None:
@@ -259,6 +273,12 @@ class Ebic:
     def set_kernel(self, kernel: int) -> None:
         ebic_set_kernel(self._ctx, kernel)
 
+    def set_pairbits(self, on: bool) -> None:
+        ebic_set_pairbits(self._ctx, on)
+
+    def set_extract_source(self, use_pairbits: bool) -> None:
+        ebic_set_extract_source(self._ctx, use_pairbits)
+
     def set_early_exit(self, on: bool) -> None:
         ebic_set_early_exit(self._ctx, on)
 
@@ -286,6 +306,8 @@ class Ebic:
             dst = np.empty(cols, dtype=np.uint64)
         elif what == 3:
             dst = np.empty((cols, ld), dtype=np.uint8)
+        elif what == 4:
+            dst = np.empty((ld // 1024, cols * cols, 32), dtype=np.uint32)
         else:
             raise ValueError(what)
         ebic_debug_read(self._ctx, what, dst)

@@ -29,6 +29,8 @@ struct ebic_ctx {
     uint32_t* nanmask = nullptr;            // [cols][ld/32]
     unsigned long long* nonmissing = nullptr;  // [cols]
     uint8_t* Rk = nullptr;                  // [cols][ld] or nullptr
+    uint32_t* PB = nullptr;                 // pair bitmasks [ld/1024][cols*cols][32] or nullptr
+    int64_t pb_bytes = 0;
     int32_t* d_err = nullptr;               // sticky device error
     unsigned long long* d_visits = nullptr; // executed-visit counter (instrumentation)
     int32_t count_visits = 0;
@@ -40,7 +42,12 @@ struct ebic_ctx {
     int64_t pids_cap = 0;
     uint8_t* pids8 = nullptr;               // packed byte ids for the tiled kernels (cols <= 256)
     int64_t pids8_cap = 0;
+    int32_t* ppair = nullptr;               // pair indices for the pair-bit kernels
+    int64_t ppair_cap = 0;
+    int32_t* prec = nullptr;                // 128-byte per-individual records for the pair-bit kernels
+    int64_t prec_cap = 0;
     int32_t early_exit = 1;
+    int32_t extract_pairbits = 1;           // extraction reads the pair table when it exists
     // staging for host-pointer calls
     void* stage[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     int64_t stage_cap[5] = {0, 0, 0, 0, 0};
@@ -108,6 +115,8 @@ bool is_device_pointer(const void* p) {
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
+constexpr int kConsPair = 15;  // consumer warps of the PAIRBITS_SMEM kernel (+1 producer = 512 threads)
+constexpr int64_t kPairbitsAutoMaxBytes = 8ll << 30;   // ebic_create builds the pair table up to this size
 constexpr int kConsF32 = 31;   // consumer warps of the TILED_F32 kernel (+1 producer = 1024 threads)
 constexpr int kConsR8 = 15;    // consumer warps of the RANK8 kernel     (+1 producer =  512 threads)
 
@@ -140,9 +149,22 @@ int32_t tile_rows_r8(const ebic_ctx* ctx, int32_t n_ind_launch) {
     return T;
 }
 
+// tile buffers (1 or 2) of the PAIRBITS_SMEM kernel that fit next to the counters; 0 = does not fit
+int32_t pairsmem_nbuf(const ebic_ctx* ctx, int32_t n_ind_launch) {
+    if (!ctx->PB) return 0;
+    const int32_t npairs = ctx->cols * ctx->cols;
+    for (int32_t nbuf = 2; nbuf >= 1; --nbuf)
+        if (pairsmem_bytes(npairs, nbuf, n_ind_launch) <= static_cast<size_t>(ctx->smem_optin)) return nbuf;
+    return 0;
+}
+
 int32_t resolve_kernel(const ebic_ctx* ctx, int32_t n_ind_launch) {
     int32_t want = ctx->kernel_request;
     if (want == EBIC_KERNEL_AUTO) {
+        if (ctx->PB) {
+            if (ctx->cols <= 46 && pairsmem_nbuf(ctx, n_ind_launch) > 0) return EBIC_KERNEL_PAIRBITS_SMEM;
+            return EBIC_KERNEL_PAIRBITS;
+        }
         if (tile_rows_r8(ctx, n_ind_launch) > 0) return EBIC_KERNEL_RANK8;
         if (tile_rows_f32(ctx, n_ind_launch) > 0) return EBIC_KERNEL_TILED_F32;
         return EBIC_KERNEL_DIRECT;
@@ -178,6 +200,86 @@ int launch_tiled(ebic_ctx* ctx, const void* M, int32_t T, const int2* meta, int3
     return cuda_status(cudaGetLastError());
 }
 
+int launch_pairbits(ebic_ctx* ctx, int32_t k0, int32_t n_ind, unsigned long long* counts, cudaStream_t stream) {
+    PairbitsParams p;
+    p.PB = ctx->PB;
+    p.n_tiles = ctx->ld / kPairTileRows;
+    p.npairs = ctx->cols * ctx->cols;
+    // about 4 tasks per resident warp slot (4 CTAs / SM), 8..64 tiles (8,192..65,536 rows) per task
+    static const int64_t tasks_per_slot = env_int("EBIC_PB_TASKS_PER_SLOT", 4);
+    const int64_t want_tasks = tasks_per_slot * ctx->sm_count * 4 * kPairbitsWarps;
+    int64_t gt = p.n_tiles * n_ind / want_tasks;
+    gt = std::max<int64_t>(8, std::min<int64_t>(64, gt / 8 * 8));
+    p.group_tiles = static_cast<int32_t>(gt);
+    p.prec = ctx->prec + 32ll * k0;
+    p.ppair = ctx->ppair;
+    p.n_ind = n_ind;
+    p.counts = counts;
+    p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
+    const int64_t n_groups = (p.n_tiles + gt - 1) / gt;
+    const int64_t tasks = n_groups * n_ind;
+    const int64_t grid = (tasks + kPairbitsWarps - 1) / kPairbitsWarps;
+    if (grid > 0x7fffffffll) return EBIC_ERR_ARG;
+    ctx->last_grid = static_cast<int32_t>(grid);
+    ctx->last_T = static_cast<int32_t>(gt * kPairTileRows);
+    if (ctx->early_exit)
+        fitness_pairbits_kernel<true><<<static_cast<unsigned>(grid), kPairbitsWarps * 32, 0, stream>>>(p);
+    else
+        fitness_pairbits_kernel<false><<<static_cast<unsigned>(grid), kPairbitsWarps * 32, 0, stream>>>(p);
+    ctx->launches++;
+    return cuda_status(cudaGetLastError());
+}
+
+int launch_pairsmem(ebic_ctx* ctx, const int2* meta, int32_t n_ind, unsigned long long* counts, cudaStream_t stream) {
+    PairSmemParams p;
+    p.PB = ctx->PB;
+    p.n_tiles = ctx->ld / kPairTileRows;
+    p.npairs = ctx->cols * ctx->cols;
+    p.nbuf = pairsmem_nbuf(ctx, n_ind);
+    if (p.nbuf <= 0) return EBIC_ERR_ARG;
+    p.meta = meta;
+    p.ppair = ctx->ppair;
+    p.n_ind = n_ind;
+    p.early_exit = ctx->early_exit;
+    p.counts = counts;
+    p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
+    const size_t smem = pairsmem_bytes(p.npairs, p.nbuf, n_ind);
+    auto kern = fitness_pairsmem_kernel<kConsPair>;
+    EBIC_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+    const int64_t P = p.n_tiles * n_ind;
+    const int64_t grid = std::min<int64_t>(ctx->sm_count, std::max<int64_t>(1, P / kConsPair));
+    ctx->last_grid = static_cast<int32_t>(grid);
+    ctx->last_T = kPairTileRows;
+    kern<<<static_cast<unsigned>(grid), (kConsPair + 1) * 32, smem, stream>>>(p);
+    ctx->launches++;
+    return cuda_status(cudaGetLastError());
+}
+
+// a2": (re)build the pair-relation bitmasks.  Synchronous.
+int build_pairbits(ebic_ctx* ctx) {
+    if (ctx->PB) return EBIC_OK;
+    if (ctx->cols > 46340) return EBIC_ERR_ARG;                  // cols^2 must fit int32
+    const int64_t bytes = static_cast<int64_t>(ctx->cols) * ctx->cols * (ctx->ld / 8);
+    int st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->PB), bytes);
+    if (st) return st;
+    ctx->pb_bytes = bytes;
+    const dim3 grid(static_cast<unsigned>(ctx->ld / kPairTileRows), static_cast<unsigned>((ctx->cols + 7) / 8));
+    if (grid.y > 65535u) return EBIC_ERR_ARG;
+    pairbits_kernel<<<grid, 256>>>(ctx->Mc, ctx->ld, ctx->cols, ctx->PB);
+    ctx->launches++;
+    st = cuda_status(cudaGetLastError());
+    if (!st) st = cuda_status(cudaDeviceSynchronize());
+    return st;
+}
+
+void free_pairbits(ebic_ctx* ctx) {
+    if (!ctx->PB) return;
+    cudaFree(ctx->PB);
+    ctx->bytes_owned -= ctx->pb_bytes;
+    ctx->PB = nullptr;
+    ctx->pb_bytes = 0;
+}
+
 // Population already on the device: ingest + chain kernels.
 int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, int32_t n_ind, int64_t n_ids,
                 unsigned long long* counts, cudaStream_t stream) {
@@ -190,9 +292,17 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         if (st) return st;
     }
 
+    if (ctx->PB) {
+        st = grow(ctx, reinterpret_cast<void**>(&ctx->ppair), &ctx->ppair_cap, (n_ids + 3ll * n_ind + 8) * 4);
+        if (st) return st;
+        st = grow(ctx, reinterpret_cast<void**>(&ctx->prec), &ctx->prec_cap, 128ll * n_ind);
+        if (st) return st;
+    }
+
     ingest_population_kernel<<<(n_ind + 255) / 256, 256, 0, stream>>>(
         offsets, col_ids, n_ind, n_ids, ctx->cols, ctx->rows, ctx->missing_mode == EBIC_MISSING_ON,
-        ctx->nonmissing, ctx->meta, ctx->pids, ctx->cols <= 256 ? ctx->pids8 : nullptr, counts, ctx->d_err);
+        ctx->nonmissing, ctx->meta, ctx->pids, ctx->cols <= 256 ? ctx->pids8 : nullptr,
+        ctx->PB ? ctx->ppair : nullptr, ctx->PB ? ctx->prec : nullptr, counts, ctx->d_err);
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());
 
@@ -204,10 +314,18 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         }
         EBIC_TRY(cudaEventRecord(ctx->ev_begin[slot], stream));
     }
-    for (int32_t k0 = 0; k0 < n_ind; k0 += kMaxIndPerLaunch) {
-        const int32_t n = std::min<int32_t>(kMaxIndPerLaunch, n_ind - k0);
-        const int32_t kernel = resolve_kernel(ctx, n);
-        if (kernel == EBIC_KERNEL_RANK8) {
+    const bool whole = resolve_kernel(ctx, std::min<int32_t>(kMaxIndPerLaunch, n_ind)) == EBIC_KERNEL_PAIRBITS;
+    const int32_t per_launch = whole ? n_ind : kMaxIndPerLaunch;   // PAIRBITS has no per-CTA counters
+    for (int32_t k0 = 0; k0 < n_ind; k0 += per_launch) {
+        const int32_t n = std::min<int32_t>(per_launch, n_ind - k0);
+        const int32_t kernel = whole ? EBIC_KERNEL_PAIRBITS : resolve_kernel(ctx, n);
+        if (kernel == EBIC_KERNEL_PAIRBITS) {
+            if (!ctx->PB) return EBIC_ERR_ARG;
+            st = launch_pairbits(ctx, k0, n, counts + k0, stream);
+        } else if (kernel == EBIC_KERNEL_PAIRBITS_SMEM) {
+            if (!ctx->PB) return EBIC_ERR_ARG;
+            st = launch_pairsmem(ctx, ctx->meta + k0, n, counts + k0, stream);
+        } else if (kernel == EBIC_KERNEL_RANK8) {
             const int32_t T = tile_rows_r8(ctx, n);
             if (T <= 0) return EBIC_ERR_ARG;
             static const int r8_cons = env_int("EBIC_R8_CONS", kConsR8);
@@ -245,6 +363,15 @@ int extract_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids
                    cudaStream_t stream) {
     const int64_t words32 = 2 * ((ctx->rows + 63) / 64);
     if (counts) EBIC_TRY(cudaMemsetAsync(counts, 0, static_cast<size_t>(n_chosen) * 8, stream));
+    if (ctx->PB && ctx->extract_pairbits) {
+        const dim3 grid(static_cast<unsigned>((words32 + 255) / 256), static_cast<unsigned>(std::min<int32_t>(n_chosen, 65535)));
+        extract_rows_pairbits_kernel<<<grid, 256, 0, stream>>>(
+            ctx->PB, ctx->ld, ctx->rows, ctx->cols, ctx->missing_mode == EBIC_MISSING_ON, ctx->nanmask, offsets,
+            col_ids, n_ind, n_ids, chosen, n_chosen, reinterpret_cast<uint32_t*>(masks), words32,
+            reinterpret_cast<unsigned long long*>(counts), ctx->d_err);
+        ctx->launches++;
+        return cuda_status(cudaGetLastError());
+    }
     const int64_t gx = (words32 * 32 + kExtractRowsPerBlock - 1) / kExtractRowsPerBlock;
     dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>(std::min<int32_t>(n_chosen, 65535)));
     extract_rows_kernel<<<grid, 256, 0, stream>>>(
@@ -337,7 +464,21 @@ int ebic_create(const float* matrix, int64_t rows, int32_t cols, int32_t missing
             ctx->launches++;
             if ((st = cuda_status(cudaGetLastError()))) break;
         }
-        st = cuda_status(cudaDeviceSynchronize());
+        if ((st = cuda_status(cudaDeviceSynchronize()))) break;
+        // a2": pair-relation bitmasks, when they fit comfortably (otherwise the rank / float kernels serve)
+        if (cols <= 46340) {
+            const int64_t pb = static_cast<int64_t>(cols) * cols * (ctx->ld / 8);
+            size_t free_b = 0, total_b = 0;
+            if ((st = cuda_status(cudaMemGetInfo(&free_b, &total_b)))) break;
+            if (pb <= kPairbitsAutoMaxBytes && pb <= static_cast<int64_t>(free_b / 2)) {
+                st = build_pairbits(ctx);
+                if (st == EBIC_ERR_OOM) {
+                    free_pairbits(ctx);
+                    st = EBIC_OK;
+                }
+                if (st) break;
+            }
+        }
     } while (0);
     if (staging) cudaFree(staging);
     if (st != EBIC_OK) {
@@ -354,6 +495,9 @@ int ebic_destroy(ebic_ctx* ctx) {
     cudaFree(ctx->nanmask);
     cudaFree(ctx->nonmissing);
     cudaFree(ctx->Rk);
+    cudaFree(ctx->PB);
+    cudaFree(ctx->ppair);
+    cudaFree(ctx->prec);
     cudaFree(ctx->d_err);
     cudaFree(ctx->meta);
     cudaFree(ctx->pids);
@@ -469,10 +613,36 @@ int ebic_set_kernel(ebic_ctx* ctx, int32_t kernel) {
         case EBIC_KERNEL_RANK8:
             if (tile_rows_r8(ctx, 1) <= 0) return EBIC_ERR_ARG;
             break;
+        case EBIC_KERNEL_PAIRBITS:
+            if (!ctx->PB) return EBIC_ERR_ARG;
+            break;
+        case EBIC_KERNEL_PAIRBITS_SMEM:
+            if (pairsmem_nbuf(ctx, 1) <= 0) return EBIC_ERR_ARG;
+            break;
         default:
             return EBIC_ERR_ARG;
     }
     ctx->kernel_request = kernel;
+    return EBIC_OK;
+}
+
+int ebic_set_pairbits(ebic_ctx* ctx, int32_t on) {
+    if (!ctx) return EBIC_ERR_ARG;
+    if (cudaDeviceSynchronize() != cudaSuccess) return cuda_status(cudaGetLastError());
+    if (on == 0) {
+        free_pairbits(ctx);
+        if (ctx->kernel_request == EBIC_KERNEL_PAIRBITS || ctx->kernel_request == EBIC_KERNEL_PAIRBITS_SMEM)
+            ctx->kernel_request = EBIC_KERNEL_AUTO;
+        return EBIC_OK;
+    }
+    int st = build_pairbits(ctx);
+    if (st) free_pairbits(ctx);
+    return st;
+}
+
+int ebic_set_extract_source(ebic_ctx* ctx, int32_t use_pairbits) {
+    if (!ctx) return EBIC_ERR_ARG;
+    ctx->extract_pairbits = use_pairbits ? 1 : 0;
     return EBIC_OK;
 }
 
@@ -532,6 +702,7 @@ int64_t ebic_get_info(ebic_ctx* ctx, int32_t what) {
         }
         case 12: return ctx->timed_evals;
         case 13: return ctx->early_exit;
+        case 14: return ctx->pb_bytes;
         default: return -1;
     }
 }
@@ -546,6 +717,7 @@ int ebic_debug_read(const ebic_ctx* ctx, int32_t what, void* dst, int64_t dst_by
         case 1: src = ctx->nanmask; bytes = n / 8; break;
         case 2: src = ctx->nonmissing; bytes = static_cast<int64_t>(ctx->cols) * 8; break;
         case 3: src = ctx->Rk; bytes = n; break;
+        case 4: src = ctx->PB; bytes = ctx->pb_bytes; break;
         default: return EBIC_ERR_ARG;
     }
     if (!src || bytes != dst_bytes) return EBIC_ERR_ARG;

@@ -6,7 +6,8 @@
 
 namespace ebic {
 
-constexpr int kLdAlign = 512;          // leading dimension (padded rows) is a multiple of this
+constexpr int kLdAlign = 1024;         // leading dimension (padded rows) is a multiple of this (= one pair-bit tile)
+constexpr int kPairTileRows = 1024;    // rows per pair-bit tile: one pair-row of a tile = 32 words = 128 B
 constexpr int kRowsPerSlabF32 = 128;   // one warp, 4 float32 rows per lane  (one LDS.128 per column)
 constexpr int kRowsPerSlabR8 = 512;    // one warp, 16 uint8 ranks per lane  (one LDS.128 per column)
 constexpr unsigned kRankNaN = 0x7Fu;   // rank code of a missing value; real ranks are 0x80 | rank
@@ -62,6 +63,12 @@ __device__ __forceinline__ void bulk_copy_g2s(void* smem_dst, const void* gmem_s
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     uint4 v;
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
     return v;
 }
 

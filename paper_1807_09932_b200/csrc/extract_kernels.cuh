@@ -108,4 +108,96 @@ extract_rows_kernel(const float* __restrict__ Mc, int64_t ld, int64_t rows, int3
     }
 }
 
+// Extraction from the pair-relation bitmasks (loader_kernels.cuh): for L >= 2 the mask IS the AND of the
+// individual's L-1 pair-rows, so a chosen individual costs (L-1) * rows / 8 bytes of HBM reads instead of
+// 4 * L * rows -- 32x less.  One thread per 32-bit mask word; a warp reads one 128 B pair-row of one
+// tile per pair.  Padding rows are NaN, so bits >= rows are already zero.  L <= 1 as above.
+// grid.x over blocks of 256 words, grid.y over chosen (strided).
+__global__ void __launch_bounds__(256)
+extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_t rows, int32_t cols,
+                             int32_t missing_on, const uint32_t* __restrict__ nanmask,
+                             const int32_t* __restrict__ offsets, const int32_t* __restrict__ col_ids,
+                             int32_t n_ind, int64_t n_ids, const int32_t* __restrict__ chosen, int32_t n_chosen,
+                             uint32_t* __restrict__ masks32, int64_t words32,
+                             unsigned long long* __restrict__ counts, int32_t* __restrict__ err)
+{
+    __shared__ int32_t s_pair[kExtractMaxSmemIds];
+    __shared__ int32_t s_bad;
+    __shared__ unsigned int s_cnt;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int64_t ldw = ld / 32;
+    const int64_t w = static_cast<int64_t>(blockIdx.x) * 256 + tid;      // this thread's mask word
+    const int64_t npairs = static_cast<int64_t>(cols) * cols;
+    const uint32_t* wbase = PB + (w >> 5) * npairs * 32 + (w & 31);        // + pair * 32
+
+    for (int32_t j = blockIdx.y; j < n_chosen; j += gridDim.y) {
+        if (tid == 0) {
+            s_bad = 0;
+            s_cnt = 0;
+        }
+        __syncthreads();
+        const int32_t k = chosen[j];
+        int32_t b = 0, L = -1;
+        int bad = 0;
+        if (k < 0 || k >= n_ind) {
+            bad = 5;
+        } else {
+            b = offsets[k];
+            const int32_t e = offsets[k + 1];
+            if (b < 0 || e < b || static_cast<int64_t>(e) > n_ids) bad = 5;
+            else L = e - b;
+        }
+        if (!bad) {
+            for (int32_t i = tid; i < L; i += 256) {
+                const int32_t id = col_ids[b + i];
+                if (id < 0 || id >= cols) s_bad = 4;             // benign race: same value
+                else if (i + 1 < L && i < kExtractMaxSmemIds) {
+                    const int32_t nx = col_ids[b + i + 1];
+                    s_pair[i] = (nx >= 0 && nx < cols) ? id * cols + nx : 0;
+                }
+            }
+        }
+        __syncthreads();
+        if (!bad) bad = s_bad;
+        if (bad && tid == 0 && blockIdx.x == 0) atomicMax(err, bad);
+
+        unsigned int word = 0;
+        if (w < words32 && !bad) {
+            if (L >= 2) {
+                word = 0xffffffffu;
+                const int32_t npr = L - 1;
+                const int32_t ns = min(npr, kExtractMaxSmemIds);
+                int32_t i = 0;
+                for (; i + 4 <= ns; i += 4) {
+                    const unsigned int v0 = __ldg(wbase + static_cast<int64_t>(s_pair[i]) * 32);
+                    const unsigned int v1 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 1]) * 32);
+                    const unsigned int v2 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 2]) * 32);
+                    const unsigned int v3 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 3]) * 32);
+                    word &= v0 & v1 & v2 & v3;
+                }
+                for (; i < ns; ++i) word &= __ldg(wbase + static_cast<int64_t>(s_pair[i]) * 32);
+                for (; i < npr; ++i) {                          // very long chromosomes: ids from global
+                    const int64_t pr = static_cast<int64_t>(__ldg(&col_ids[b + i])) * cols + __ldg(&col_ids[b + i + 1]);
+                    word &= __ldg(wbase + pr * 32);
+                }
+            } else {
+                const int64_t left = rows - w * 32;
+                const unsigned int valid = left >= 32 ? 0xffffffffu : left <= 0 ? 0u : ((1u << left) - 1u);
+                if (L == 1 && missing_on && w < ldw)
+                    word = ~nanmask[static_cast<int64_t>(__ldg(&col_ids[b])) * ldw + w] & valid;
+                else
+                    word = valid;
+            }
+        }
+        if (w < words32) masks32[static_cast<int64_t>(j) * words32 + w] = word;
+        if (counts != nullptr) {                                 // warp -> block -> one global atomic per block
+            const unsigned int local = __reduce_add_sync(0xffffffffu, __popc(word));
+            if (lane == 0 && local) atomicAdd(&s_cnt, local);
+            __syncthreads();
+            if (tid == 0 && s_cnt) atomicAdd(&counts[j], static_cast<unsigned long long>(s_cnt));
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace ebic

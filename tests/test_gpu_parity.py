@@ -28,7 +28,7 @@ def B():
 
 def kernels_for(eb, B):
     ks = [B.EBIC_KERNEL_DIRECT]
-    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8):
+    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_PAIRBITS_SMEM):
         try:
             eb.set_kernel(k)
             ks.append(k)
@@ -83,10 +83,12 @@ def check_all(B, oracle_mod, matrix, mode, off, ids, chosen=None, expect_status=
             chosen = np.arange(n_ind, dtype=np.int32)
         if len(chosen):
             st, wm, wc = oracle_mod.extract_rows(matrix, mode, off, ids, chosen)
-            gm, gc = gpu_masks(eb, off, ids, chosen)
-            assert (gm == wm).all()
-            assert (gc == wc).all()
-            assert eb.status() == st
+            for use_pairbits in (True, False):                 # pair-table source and float32 source
+                eb.set_extract_source(use_pairbits)
+                gm, gc = gpu_masks(eb, off, ids, chosen)
+                assert (gm == wm).all(), use_pairbits
+                assert (gc == wc).all(), use_pairbits
+                assert eb.status() == st
     return want
 
 
@@ -100,7 +102,7 @@ def test_loader_products(B, rows, cols, nan_rate):
     for src in (m, dev(m)):                                    # host pointer and device pointer
         with B.Ebic(src, ON) as eb:
             ld = eb.ld
-            assert ld % 512 == 0 and ld >= rows and ld - rows < 512
+            assert ld % 1024 == 0 and ld >= rows and ld - rows < 1024
             mc = eb.debug_read(0)
             assert (mc[:, :rows].view(np.uint32) == m.T.view(np.uint32)).all()   # bit-exact transpose
             assert np.isnan(mc[:, rows:]).all()                                   # padding = missing
@@ -112,6 +114,16 @@ def test_loader_products(B, rows, cols, nan_rate):
             below = (m[:, None, :] < m[:, :, None]).sum(axis=2)                   # [rows][cols]
             code = np.where(np.isnan(m), 0x7F, 0x80 | below).astype(np.uint8)
             assert (rk[:, :rows] == code.T).all() and (rk[:, rows:] == 0x7F).all()
+            # pair table [tile][a*cols+b][32 words]: bit r = (m[r][b] >= m[r][a]); padding rows 0
+            pb = eb.debug_read(4)
+            assert eb.info(14) == pb.nbytes
+            mp = np.full((ld, cols), np.nan, dtype=np.float32)
+            mp[:rows] = m
+            with np.errstate(invalid="ignore"):
+                ge = mp[:, None, :] >= mp[:, :, None]                              # [ld][a][b]
+            want = np.ascontiguousarray(np.packbits(ge.reshape(ld // 1024, 1024, cols * cols).transpose(0, 2, 1),
+                                                    axis=2, bitorder="little")).view(np.uint32)
+            assert (pb == want).all()
 
 
 # ------------------------------------------------------------------------- hand fixtures on the GPU
@@ -190,14 +202,26 @@ def test_long_and_degenerate_chromosomes(B, oracle_mod):
 
 
 def test_wide_matrix_falls_back(B, oracle_mod):
-    """cols > 127: no rank tiles; cols so large that no float tile double-buffers: DIRECT only."""
+    """cols > 127: no rank tiles; cols so large that no float tile double-buffers: DIRECT only.  The pair
+    table still serves (PAIRBITS); without it AUTO falls back to TILED_F32 / DIRECT."""
     for cols in (128, 200, 500):
         m, off, ids = W.random_case(cols, 700, cols, 50, (0, 9), 0.02, False, True)
         with B.Ebic(m, ON) as eb:
             with pytest.raises(B.EbicError):
                 eb.set_kernel(B.EBIC_KERNEL_RANK8)
+            with pytest.raises(B.EbicError):
+                eb.set_kernel(B.EBIC_KERNEL_PAIRBITS_SMEM)
+            assert eb.kernel == B.EBIC_KERNEL_PAIRBITS
+            eb.set_pairbits(False)
+            assert eb.info(14) == 0
             expected = B.EBIC_KERNEL_TILED_F32 if cols <= 200 else B.EBIC_KERNEL_DIRECT
             assert eb.kernel == expected
+            with pytest.raises(B.EbicError):
+                eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)
+            st, want = oracle_mod.eval_fitness(m, ON, off, ids)
+            assert (gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_AUTO) == want).all()
+            eb.set_pairbits(True)
+            assert eb.kernel == B.EBIC_KERNEL_PAIRBITS
         check_all(B, oracle_mod, m, ON, off, ids, np.arange(0, 50, 7, dtype=np.int32))
 
 
@@ -261,7 +285,7 @@ def test_host_pointers_and_streams(B, oracle_mod):
 
 
 def test_instrumentation_counts_executed_visits(B):
-    w = W.make_workload(2, rows=20_000, n_ind=200)
+    w = W.make_workload(4, rows=20_000, n_ind=200)
     with B.Ebic(w.matrix, w.missing_mode) as eb:
         nominal = eb.ld * int(w.lengths.sum())
         for kern in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8):
@@ -275,6 +299,21 @@ def test_instrumentation_counts_executed_visits(B):
                 eb.set_instrumentation(0)
             assert seen[False] == nominal                          # plain work: executed == nominal
             assert 2 * eb.ld * w.n_ind <= seen[True] <= nominal    # early exit only ever skips columns
+        nominal_pairs = eb.ld * int((w.lengths - 1).sum())         # pair kernels count (row, pair) fetches
+        for kern in (B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_PAIRBITS_SMEM):
+            if kern not in kernels_for(eb, B):
+                continue
+            eb.set_kernel(kern)
+            for early_exit in (False, True):
+                eb.set_early_exit(early_exit)
+                eb.set_instrumentation(1)
+                eb.eval_fitness(dev(w.offsets), dev(w.col_ids))
+                seen = eb.info(10)
+                eb.set_instrumentation(0)
+                if early_exit and kern == B.EBIC_KERNEL_PAIRBITS:
+                    assert eb.ld * w.n_ind <= seen <= nominal_pairs
+                else:
+                    assert seen == nominal_pairs
 
 
 # ------------------------------------------------------------------------- full-size C5 (bench config)
@@ -291,13 +330,16 @@ def test_c5_full_size_sampled(B, oracle_mod):
     with B.Ebic(w.matrix, w.missing_mode) as eb:
         import torch
         results = {}
-        for kern in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32):
+        for kern in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_PAIRBITS_SMEM):
             eb.set_kernel(kern)
-            c = eb.eval_fitness(d_off, d_ids)
-            torch.cuda.synchronize()
-            results[kern] = c.cpu().numpy().view(np.uint64)
-            assert (results[kern][sample] == want).all(), B.KERNEL_NAMES[kern]
-        assert (results[B.EBIC_KERNEL_RANK8] == results[B.EBIC_KERNEL_TILED_F32]).all()
+            for early_exit in (False, True):
+                eb.set_early_exit(early_exit)
+                c = eb.eval_fitness(d_off, d_ids)
+                torch.cuda.synchronize()
+                results[kern] = c.cpu().numpy().view(np.uint64)
+                assert (results[kern][sample] == want).all(), (B.KERNEL_NAMES[kern], early_exit)
+        for kern in results:
+            assert (results[kern] == results[B.EBIC_KERNEL_RANK8]).all(), B.KERNEL_NAMES[kern]
         counts = results[B.EBIC_KERNEL_RANK8]
         # properties: planted rows are a subset; popcount(mask) == count; tail bits zero
         chosen = np.array([k for k, _ in w.planted_individuals][:4], dtype=np.int32)
