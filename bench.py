@@ -41,7 +41,7 @@ METRIC = "row_pair_comparisons_per_s"
 UNIT = "comparisons/s"
 N_CHOSEN = 8
 WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4}
-KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "pairbits_smem": 5}
+KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4}
 
 
 def log(*a):
@@ -123,7 +123,7 @@ def pick_chosen(w):
 def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None):
     f_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     smem_peak_gbs = sm_count * 128 * f_hz / 1e9            # 128 B / clk / SM shared-memory data pipe
-    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "direct": 4, "pairbits": 0.125, "pairbits_smem": 0.125}[kernel_name]
+    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "direct": 4, "pairbits": 0.125}[kernel_name]
     achieved = visits_executed * bytes_per_visit / kernel_s / 1e9
     return {"bound": "alu", "resource": "shared-memory data pipe (128 B/clk/SM) == ALU pipe at 0.5 op/visit"
             if kernel_name == "rank8" else "shared-memory data pipe (128 B/clk/SM)",
@@ -378,7 +378,7 @@ def run_table(args):
         chosen = pick_chosen(w)
         d_chosen = torch.from_numpy(chosen).cuda()
         d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
-        for kname, ee in (("pairbits_smem", 0), ("pairbits", 0), ("pairbits", 1), ("rank8", 0), ("rank8", 1),
+        for kname, ee in (("pairbits", 0), ("pairbits", 1), ("rank8", 0), ("rank8", 1),
                           ("tiled_f32", 0), ("tiled_f32", 1), ("direct", 0)):
             if kname == "direct" and w.comparisons > 2e10:
                 continue

@@ -49,13 +49,11 @@ enum { EBIC_MISSING_OFF = 0, EBIC_MISSING_ON = 1 };
 
 /* Kernel selection for ebic_eval_fitness (all give bit-identical counts). */
 enum {
-    EBIC_KERNEL_AUTO = 0,    /* fastest applicable: PAIRBITS_SMEM, PAIRBITS, RANK8, TILED_F32, DIRECT */
+    EBIC_KERNEL_AUTO = 0,    /* fastest applicable: PAIRBITS, RANK8, TILED_F32, DIRECT              */
     EBIC_KERNEL_DIRECT = 1,  /* one thread per row, column-major global loads (any shape)          */
     EBIC_KERNEL_TILED_F32 = 2, /* float32 row tiles staged in shared memory by TMA bulk copies    */
     EBIC_KERNEL_RANK8 = 3,   /* per-row order-preserving 8-bit rank tiles (cols <= 127)           */
-    EBIC_KERNEL_PAIRBITS = 4, /* AND of pair-relation bitmasks streamed through L2 (pair table built) */
-    EBIC_KERNEL_PAIRBITS_SMEM = 5 /* the same, pair table of a 1024-row tile staged in shared memory
-                                     (cols^2 * 128 B must fit: cols <= about 42)                  */
+    EBIC_KERNEL_PAIRBITS = 4 /* AND of pair-relation bit columns gathered by TMA bulk copies (pair table built) */
 };
 
 /*
@@ -119,8 +117,8 @@ int ebic_set_kernel(ebic_ctx *ctx, int32_t kernel);
 
 /*
  * Pair-relation table: bit r of pair (a,b) = ( M[r][b] >= M[r][a] ), cols^2 * ceil(rows/1024) * 128
- * bytes of device memory.  With it an L >= 2 chromosome is the AND of its L-1 pair bitmasks (the
- * PAIRBITS kernels; extraction reads it too).  on != 0 builds it if absent (EBIC_ERR_OOM if it does
+ * bytes of device memory, one contiguous bit column per ordered pair.  With it an L >= 2 chromosome is
+ * the AND of its L-1 bit columns (the PAIRBITS kernel; extraction reads it too).  on != 0 builds it if absent (EBIC_ERR_OOM if it does
  * not fit; EBIC_ERR_ARG if cols > 46340), on == 0 frees it.  Synchronises the device.
  */
 int ebic_set_pairbits(ebic_ctx *ctx, int32_t on);
@@ -139,7 +137,7 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
 /*
  * Instrumentation for roofline accounting.  `on` is a bit set:
  *   bit 0  the tiled fitness kernels add the number of (row, column-visit) operand fetches they
- *          actually executed -- the PAIRBITS kernels the number of (row, pair) bit fetches -- to a
+ *          actually executed -- the PAIRBITS kernel the number of (row, pair) bit fetches -- to a
  *          device counter (one extra global atomic per warp);
  *          ebic_get_info(ctx, 10) synchronises the device, returns the counter and resets it.
  *          Never on inside a timed region.
@@ -167,7 +165,7 @@ int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);
  *   ebic_debug_read(ctx, what, dst, dst_bytes): what = 0 column-major matrix float32 [cols][ld];
  *   1 NaN bitmask uint32 [cols][ld/32]; 2 per-column non-missing counts uint64 [cols];
  *   3 rank tiles uint8 [cols][ld] (EBIC_ERR_ARG if not built);
- *   4 pair table uint32 [ld/1024][cols*cols][32] (EBIC_ERR_ARG if not built).
+ *   4 pair table uint32 [cols*cols][ld/32], pair (a,b) = a*cols + b (EBIC_ERR_ARG if not built).
  *   dst_bytes must equal the product's size.
  */
 int ebic_debug_read(const ebic_ctx *ctx, int32_t what, void *dst, int64_t dst_bytes);

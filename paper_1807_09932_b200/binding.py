@@ -30,8 +30,7 @@ EBIC_KERNEL_DIRECT = 1
 EBIC_KERNEL_TILED_F32 = 2
 EBIC_KERNEL_RANK8 = 3
 EBIC_KERNEL_PAIRBITS = 4
-EBIC_KERNEL_PAIRBITS_SMEM = 5
-KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits", 5: "pairbits_smem"}
+KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits"}
 
 LIB_PATH = Path(__file__).resolve().parent / "libebic.so"
 
@@ -307,7 +306,7 @@ class Ebic:
         elif what == 3:
             dst = np.empty((cols, ld), dtype=np.uint8)
         elif what == 4:
-            dst = np.empty((ld // 1024, cols * cols, 32), dtype=np.uint32)
+            dst = np.empty((cols * cols, ld // 32), dtype=np.uint32)
         else:
             raise ValueError(what)
         ebic_debug_read(self._ctx, what, dst)

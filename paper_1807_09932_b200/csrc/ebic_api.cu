@@ -12,6 +12,7 @@
 #include "extract_kernels.cuh"
 #include "fitness_kernels.cuh"
 #include "loader_kernels.cuh"
+#include "pairbits_kernels.cuh"
 
 using namespace ebic;
 
@@ -29,7 +30,7 @@ struct ebic_ctx {
     uint32_t* nanmask = nullptr;            // [cols][ld/32]
     unsigned long long* nonmissing = nullptr;  // [cols]
     uint8_t* Rk = nullptr;                  // [cols][ld] or nullptr
-    uint32_t* PB = nullptr;                 // pair bitmasks [ld/1024][cols*cols][32] or nullptr
+    uint32_t* PB = nullptr;                 // pair bit columns [cols*cols][ld/32] or nullptr
     int64_t pb_bytes = 0;
     int32_t* d_err = nullptr;               // sticky device error
     unsigned long long* d_visits = nullptr; // executed-visit counter (instrumentation)
@@ -115,7 +116,6 @@ bool is_device_pointer(const void* p) {
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
-constexpr int kConsPair = 15;  // consumer warps of the PAIRBITS_SMEM kernel (+1 producer = 512 threads)
 constexpr int64_t kPairbitsAutoMaxBytes = 8ll << 30;   // ebic_create builds the pair table up to this size
 constexpr int kConsF32 = 31;   // consumer warps of the TILED_F32 kernel (+1 producer = 1024 threads)
 constexpr int kConsR8 = 15;    // consumer warps of the RANK8 kernel     (+1 producer =  512 threads)
@@ -149,22 +149,10 @@ int32_t tile_rows_r8(const ebic_ctx* ctx, int32_t n_ind_launch) {
     return T;
 }
 
-// tile buffers (1 or 2) of the PAIRBITS_SMEM kernel that fit next to the counters; 0 = does not fit
-int32_t pairsmem_nbuf(const ebic_ctx* ctx, int32_t n_ind_launch) {
-    if (!ctx->PB) return 0;
-    const int32_t npairs = ctx->cols * ctx->cols;
-    for (int32_t nbuf = 2; nbuf >= 1; --nbuf)
-        if (pairsmem_bytes(npairs, nbuf, n_ind_launch) <= static_cast<size_t>(ctx->smem_optin)) return nbuf;
-    return 0;
-}
-
 int32_t resolve_kernel(const ebic_ctx* ctx, int32_t n_ind_launch) {
     int32_t want = ctx->kernel_request;
     if (want == EBIC_KERNEL_AUTO) {
-        if (ctx->PB) {
-            if (ctx->cols <= 46 && pairsmem_nbuf(ctx, n_ind_launch) > 0) return EBIC_KERNEL_PAIRBITS_SMEM;
-            return EBIC_KERNEL_PAIRBITS;
-        }
+        if (ctx->PB) return EBIC_KERNEL_PAIRBITS;
         if (tile_rows_r8(ctx, n_ind_launch) > 0) return EBIC_KERNEL_RANK8;
         if (tile_rows_f32(ctx, n_ind_launch) > 0) return EBIC_KERNEL_TILED_F32;
         return EBIC_KERNEL_DIRECT;
@@ -200,57 +188,31 @@ int launch_tiled(ebic_ctx* ctx, const void* M, int32_t T, const int2* meta, int3
     return cuda_status(cudaGetLastError());
 }
 
-int launch_pairbits(ebic_ctx* ctx, int32_t k0, int32_t n_ind, unsigned long long* counts, cudaStream_t stream) {
+int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, unsigned long long* counts, cudaStream_t stream) {
     PairbitsParams p;
     p.PB = ctx->PB;
-    p.n_tiles = ctx->ld / kPairTileRows;
-    p.npairs = ctx->cols * ctx->cols;
-    // about 4 tasks per resident warp slot (4 CTAs / SM), 8..64 tiles (8,192..65,536 rows) per task
+    p.ldw = ctx->ld / 32;
+    // about `tasks_per_slot` tasks per resident warp slot (4 CTAs / SM), 256..2048 words (8,192..65,536 rows) per task
     static const int64_t tasks_per_slot = env_int("EBIC_PB_TASKS_PER_SLOT", 4);
     const int64_t want_tasks = tasks_per_slot * ctx->sm_count * 4 * kPairbitsWarps;
-    int64_t gt = p.n_tiles * n_ind / want_tasks;
-    gt = std::max<int64_t>(8, std::min<int64_t>(64, gt / 8 * 8));
-    p.group_tiles = static_cast<int32_t>(gt);
-    p.prec = ctx->prec + 32ll * k0;
+    int64_t cw = p.ldw * n_ind / want_tasks;
+    cw = std::max<int64_t>(kPairbitsStepWords, std::min<int64_t>(8 * kPairbitsStepWords, cw / kPairbitsStepWords * kPairbitsStepWords));
+    p.chunk_words = static_cast<int32_t>(cw);
+    p.n_chunks = static_cast<int32_t>((p.ldw + cw - 1) / cw);
+    p.prec = ctx->prec;
     p.ppair = ctx->ppair;
     p.n_ind = n_ind;
     p.counts = counts;
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
-    const int64_t n_groups = (p.n_tiles + gt - 1) / gt;
-    const int64_t tasks = n_groups * n_ind;
+    const int64_t tasks = static_cast<int64_t>(p.n_chunks) * n_ind;
     const int64_t grid = (tasks + kPairbitsWarps - 1) / kPairbitsWarps;
     if (grid > 0x7fffffffll) return EBIC_ERR_ARG;
     ctx->last_grid = static_cast<int32_t>(grid);
-    ctx->last_T = static_cast<int32_t>(gt * kPairTileRows);
+    ctx->last_T = static_cast<int32_t>(cw * 32);
     if (ctx->early_exit)
         fitness_pairbits_kernel<true><<<static_cast<unsigned>(grid), kPairbitsWarps * 32, 0, stream>>>(p);
     else
         fitness_pairbits_kernel<false><<<static_cast<unsigned>(grid), kPairbitsWarps * 32, 0, stream>>>(p);
-    ctx->launches++;
-    return cuda_status(cudaGetLastError());
-}
-
-int launch_pairsmem(ebic_ctx* ctx, const int2* meta, int32_t n_ind, unsigned long long* counts, cudaStream_t stream) {
-    PairSmemParams p;
-    p.PB = ctx->PB;
-    p.n_tiles = ctx->ld / kPairTileRows;
-    p.npairs = ctx->cols * ctx->cols;
-    p.nbuf = pairsmem_nbuf(ctx, n_ind);
-    if (p.nbuf <= 0) return EBIC_ERR_ARG;
-    p.meta = meta;
-    p.ppair = ctx->ppair;
-    p.n_ind = n_ind;
-    p.early_exit = ctx->early_exit;
-    p.counts = counts;
-    p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
-    const size_t smem = pairsmem_bytes(p.npairs, p.nbuf, n_ind);
-    auto kern = fitness_pairsmem_kernel<kConsPair>;
-    EBIC_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
-    const int64_t P = p.n_tiles * n_ind;
-    const int64_t grid = std::min<int64_t>(ctx->sm_count, std::max<int64_t>(1, P / kConsPair));
-    ctx->last_grid = static_cast<int32_t>(grid);
-    ctx->last_T = kPairTileRows;
-    kern<<<static_cast<unsigned>(grid), (kConsPair + 1) * 32, smem, stream>>>(p);
     ctx->launches++;
     return cuda_status(cudaGetLastError());
 }
@@ -263,7 +225,7 @@ int build_pairbits(ebic_ctx* ctx) {
     int st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->PB), bytes);
     if (st) return st;
     ctx->pb_bytes = bytes;
-    const dim3 grid(static_cast<unsigned>(ctx->ld / kPairTileRows), static_cast<unsigned>((ctx->cols + 7) / 8));
+    const dim3 grid(static_cast<unsigned>(ctx->ld / 1024), static_cast<unsigned>((ctx->cols + 7) / 8));
     if (grid.y > 65535u) return EBIC_ERR_ARG;
     pairbits_kernel<<<grid, 256>>>(ctx->Mc, ctx->ld, ctx->cols, ctx->PB);
     ctx->launches++;
@@ -321,10 +283,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         const int32_t kernel = whole ? EBIC_KERNEL_PAIRBITS : resolve_kernel(ctx, n);
         if (kernel == EBIC_KERNEL_PAIRBITS) {
             if (!ctx->PB) return EBIC_ERR_ARG;
-            st = launch_pairbits(ctx, k0, n, counts + k0, stream);
-        } else if (kernel == EBIC_KERNEL_PAIRBITS_SMEM) {
-            if (!ctx->PB) return EBIC_ERR_ARG;
-            st = launch_pairsmem(ctx, ctx->meta + k0, n, counts + k0, stream);
+            st = launch_pairbits(ctx, n, counts, stream);
         } else if (kernel == EBIC_KERNEL_RANK8) {
             const int32_t T = tile_rows_r8(ctx, n);
             if (T <= 0) return EBIC_ERR_ARG;
@@ -616,9 +575,6 @@ int ebic_set_kernel(ebic_ctx* ctx, int32_t kernel) {
         case EBIC_KERNEL_PAIRBITS:
             if (!ctx->PB) return EBIC_ERR_ARG;
             break;
-        case EBIC_KERNEL_PAIRBITS_SMEM:
-            if (pairsmem_nbuf(ctx, 1) <= 0) return EBIC_ERR_ARG;
-            break;
         default:
             return EBIC_ERR_ARG;
     }
@@ -631,8 +587,7 @@ int ebic_set_pairbits(ebic_ctx* ctx, int32_t on) {
     if (cudaDeviceSynchronize() != cudaSuccess) return cuda_status(cudaGetLastError());
     if (on == 0) {
         free_pairbits(ctx);
-        if (ctx->kernel_request == EBIC_KERNEL_PAIRBITS || ctx->kernel_request == EBIC_KERNEL_PAIRBITS_SMEM)
-            ctx->kernel_request = EBIC_KERNEL_AUTO;
+        if (ctx->kernel_request == EBIC_KERNEL_PAIRBITS) ctx->kernel_request = EBIC_KERNEL_AUTO;
         return EBIC_OK;
     }
     int st = build_pairbits(ctx);

@@ -108,10 +108,10 @@ extract_rows_kernel(const float* __restrict__ Mc, int64_t ld, int64_t rows, int3
     }
 }
 
-// Extraction from the pair-relation bitmasks (loader_kernels.cuh): for L >= 2 the mask IS the AND of the
-// individual's L-1 pair-rows, so a chosen individual costs (L-1) * rows / 8 bytes of HBM reads instead of
-// 4 * L * rows -- 32x less.  One thread per 32-bit mask word; a warp reads one 128 B pair-row of one
-// tile per pair.  Padding rows are NaN, so bits >= rows are already zero.  L <= 1 as above.
+// Extraction from the pair-relation bit columns (loader_kernels.cuh): for L >= 2 the mask IS the AND of
+// the individual's L-1 bit columns, so a chosen individual costs (L-1) * rows / 8 bytes of HBM reads
+// instead of 4 * L * rows -- 32x less.  One thread per 32-bit mask word; a warp reads 128 contiguous
+// bytes of a bit column per pair.  Padding rows are NaN, so bits >= rows are already zero.  L <= 1 as above.
 // grid.x over blocks of 256 words, grid.y over chosen (strided).
 __global__ void __launch_bounds__(256)
 extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_t rows, int32_t cols,
@@ -127,8 +127,7 @@ extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_
     const int tid = threadIdx.x, lane = tid & 31;
     const int64_t ldw = ld / 32;
     const int64_t w = static_cast<int64_t>(blockIdx.x) * 256 + tid;      // this thread's mask word
-    const int64_t npairs = static_cast<int64_t>(cols) * cols;
-    const uint32_t* wbase = PB + (w >> 5) * npairs * 32 + (w & 31);        // + pair * 32
+    const uint32_t* wbase = PB + min(w, ldw - 1);                          // + pair * ldw
 
     for (int32_t j = blockIdx.y; j < n_chosen; j += gridDim.y) {
         if (tid == 0) {
@@ -169,16 +168,16 @@ extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_
                 const int32_t ns = min(npr, kExtractMaxSmemIds);
                 int32_t i = 0;
                 for (; i + 4 <= ns; i += 4) {
-                    const unsigned int v0 = __ldg(wbase + static_cast<int64_t>(s_pair[i]) * 32);
-                    const unsigned int v1 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 1]) * 32);
-                    const unsigned int v2 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 2]) * 32);
-                    const unsigned int v3 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 3]) * 32);
+                    const unsigned int v0 = __ldg(wbase + static_cast<int64_t>(s_pair[i]) * ldw);
+                    const unsigned int v1 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 1]) * ldw);
+                    const unsigned int v2 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 2]) * ldw);
+                    const unsigned int v3 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 3]) * ldw);
                     word &= v0 & v1 & v2 & v3;
                 }
-                for (; i < ns; ++i) word &= __ldg(wbase + static_cast<int64_t>(s_pair[i]) * 32);
+                for (; i < ns; ++i) word &= __ldg(wbase + static_cast<int64_t>(s_pair[i]) * ldw);
                 for (; i < npr; ++i) {                          // very long chromosomes: ids from global
                     const int64_t pr = static_cast<int64_t>(__ldg(&col_ids[b + i])) * cols + __ldg(&col_ids[b + i + 1]);
-                    word &= __ldg(wbase + pr * 32);
+                    word &= __ldg(wbase + pr * ldw);
                 }
             } else {
                 const int64_t left = rows - w * 32;

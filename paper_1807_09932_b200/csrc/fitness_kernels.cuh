@@ -441,247 +441,4 @@ fitness_tiled_kernel(const TiledParams p)
     }
 }
 
-// ------------------------------------------------------------------------------------------------
-// PAIRBITS kernels (a5/a6 on the pair-relation bitmasks of loader_kernels.cuh):
-//   ok(k, r) = AND_{i < L-1} PB[(c_i, c_{i+1})] bit r          count[k] = popcount over rows.
-// 1 bit per (row, pair): 8x fewer operand bytes than RANK8 and one LOP3 per 32 rows instead of 1.5 ALU
-// ops per 4 rows.  Exact for every L >= 2 and both missing modes (an ordered >= is false on NaN).
-//
-// PAIRBITS (any cols): no staging; a warp task = (individual, group of `group_tiles` tiles).  Per 4 tiles
-// (4096 rows) and pair the warp issues one LDG.128 per lane: lane l reads words 4*(l%8).. of tile l/8 --
-// four fully used 128 B lines.  Tasks are ordered tile-group major, so the CTAs in flight walk the same
-// few tile groups and the table slice they touch (cols^2 * group rows / 8 bytes) stays in the 126 MB
-// L2; HBM sees the table once per evaluation.  Bound: L2 -> SM bandwidth.
-// ------------------------------------------------------------------------------------------------
-struct PairbitsParams {
-    const uint32_t* PB;              // [n_tiles][npairs][32]
-    int64_t n_tiles;
-    int32_t npairs;                  // cols * cols
-    int32_t group_tiles;             // tiles per warp task, multiple of 8
-    const int32_t* prec;             // [n_ind][32] records
-    const int32_t* ppair;            // padded pair-index slots (chromosomes with more than 31 columns)
-    int32_t n_ind;
-    unsigned long long* counts;
-    unsigned long long* visits;      // executed (row, pair) visits (instrumented) or nullptr
-};
-
-__device__ __forceinline__ void and4(uint4& a, const uint4& v) {
-    a.x &= v.x; a.y &= v.y; a.z &= v.z; a.w &= v.w;
-}
-__device__ __forceinline__ bool any4(const uint4& a) { return (a.x | a.y | a.z | a.w) != 0u; }
-
-constexpr int kPairbitsWarps = 8;
-
-// One warp task.  Per step the warp covers 8 tiles (two chunks of 4) and, per batch, 4 pairs: 8 independent
-// LDG.128 per lane in flight before the first AND -- the kernel is bound by L2 latency x bandwidth, so the
-// loads in flight per SM are what matters.
-template <bool EARLY_EXIT>
-__global__ void __launch_bounds__(kPairbitsWarps * 32)
-fitness_pairbits_kernel(const PairbitsParams p)
-{
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t task = static_cast<int64_t>(blockIdx.x) * kPairbitsWarps + warp;
-    const int64_t g = task / p.n_ind;
-    const int32_t k = static_cast<int32_t>(task - g * p.n_ind);
-    const int64_t t_begin = g * p.group_tiles;
-    if (t_begin >= p.n_tiles) return;                            // warp-uniform
-    const int32_t rec = __ldg(p.prec + 32ll * k + lane);         // the individual: one coalesced 128 B load
-    const int32_t L = __shfl_sync(0xffffffffu, rec, 0);
-    if (L < 2) return;
-    const int32_t npr = L - 1;
-    const int32_t n0 = min(npr, kRecPairs);
-    const int32_t* pp = p.ppair + 4ll * __shfl_sync(0xffffffffu, rec, 1);
-    const int64_t t_end = min(p.n_tiles, t_begin + p.group_tiles);
-    const int sub = lane >> 3, q = lane & 7;
-    const int64_t tile_words = static_cast<int64_t>(p.npairs) * 32;
-
-    unsigned int cnt = 0;
-    unsigned long long executed = 0;
-    for (int64_t t0 = t_begin; t0 < t_end; t0 += 8) {
-        const int64_t ta = t0 + sub, tb = t0 + 4 + sub;
-        const bool va = ta < t_end, vb = tb < t_end;
-        const uint4* base_a = reinterpret_cast<const uint4*>(p.PB + (va ? ta : t0) * tile_words) + q;
-        const uint4* base_b = reinterpret_cast<const uint4*>(p.PB + (vb ? tb : t0) * tile_words) + q;
-        uint4 acc_a = va ? make_uint4(~0u, ~0u, ~0u, ~0u) : make_uint4(0u, 0u, 0u, 0u);
-        uint4 acc_b = vb ? make_uint4(~0u, ~0u, ~0u, ~0u) : make_uint4(0u, 0u, 0u, 0u);
-        int32_t done = 0;
-        int32_t i = 0;
-        for (; i + 4 <= n0; i += 4) {
-            const int32_t p0 = __shfl_sync(0xffffffffu, rec, i + 2) * 8, p1 = __shfl_sync(0xffffffffu, rec, i + 3) * 8;
-            const int32_t p2 = __shfl_sync(0xffffffffu, rec, i + 4) * 8, p3 = __shfl_sync(0xffffffffu, rec, i + 5) * 8;
-            const uint4 a0 = __ldg(base_a + p0), a1 = __ldg(base_a + p1), a2 = __ldg(base_a + p2), a3 = __ldg(base_a + p3);
-            const uint4 b0 = __ldg(base_b + p0), b1 = __ldg(base_b + p1), b2 = __ldg(base_b + p2), b3 = __ldg(base_b + p3);
-            and4(acc_a, a0); and4(acc_a, a1); and4(acc_a, a2); and4(acc_a, a3);
-            and4(acc_b, b0); and4(acc_b, b1); and4(acc_b, b2); and4(acc_b, b3);
-            done += 4;
-            if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) goto step_done;
-        }
-        if (i < n0) {                                            // 1..3 pairs left: the record is padded with
-            const int32_t r = n0 - i;                            // the last pair, so loading 4 is harmless
-            const int32_t p0 = __shfl_sync(0xffffffffu, rec, i + 2) * 8, p1 = __shfl_sync(0xffffffffu, rec, i + 3) * 8;
-            const int32_t p2 = __shfl_sync(0xffffffffu, rec, min(i + 4, 31)) * 8;
-            const uint4 a0 = __ldg(base_a + p0), b0 = __ldg(base_b + p0);
-            and4(acc_a, a0); and4(acc_b, b0);
-            if (r >= 2) {
-                const uint4 a1 = __ldg(base_a + p1), b1 = __ldg(base_b + p1);
-                and4(acc_a, a1); and4(acc_b, b1);
-            }
-            if (r >= 3) {
-                const uint4 a2 = __ldg(base_a + p2), b2 = __ldg(base_b + p2);
-                and4(acc_a, a2); and4(acc_b, b2);
-            }
-            done += r;
-        }
-        for (int32_t seg = kRecPairs; seg < npr; seg += 32) {    // chromosomes with more than 31 columns
-            if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) break;
-            const int32_t n = min(32, npr - seg);
-            const int32_t mine = __ldg(pp + seg + min(lane, n - 1));
-            for (int32_t j = 0; j < n; ++j) {
-                const int32_t p0 = __shfl_sync(0xffffffffu, mine, j) * 8;
-                const uint4 a0 = __ldg(base_a + p0), b0 = __ldg(base_b + p0);
-                and4(acc_a, a0); and4(acc_b, b0);
-            }
-            done += n;
-        }
-    step_done:
-        cnt += __popc(acc_a.x) + __popc(acc_a.y) + __popc(acc_a.z) + __popc(acc_a.w);
-        cnt += __popc(acc_b.x) + __popc(acc_b.y) + __popc(acc_b.z) + __popc(acc_b.w);
-        executed += static_cast<unsigned long long>(done) * (min(t_end - t0, static_cast<int64_t>(8)) * kPairTileRows);
-    }
-    cnt = __reduce_add_sync(0xffffffffu, cnt);
-    if (lane == 0) {
-        if (cnt) atomicAdd(&p.counts[k], static_cast<unsigned long long>(cnt));
-        if (p.visits != nullptr) atomicAdd(p.visits, executed);
-    }
-}
-
-// ------------------------------------------------------------------------------------------------
-// PAIRBITS_SMEM (cols <= 40): the whole pair table of a 1024-row tile (cols^2 * 128 B <= 200 KB) is
-// staged in shared memory by TMA bulk copies and reused by the whole population, exactly like the
-// tiled kernels above (persistent CTAs, flat (tile, individual) split, producer warp, mbarriers).
-// A consumer warp evaluates one individual on the tile with one conflict-free 128 B LDS.32 wavefront
-// per pair (lane = word = 32 rows) and one LOP3 per two pairs.  NBUF = 2 when two tiles fit, else 1.
-// ------------------------------------------------------------------------------------------------
-struct PairSmemParams {
-    const uint32_t* PB;
-    int64_t n_tiles;
-    int32_t npairs;
-    int32_t nbuf;                    // 1 or 2 tile buffers
-    const int2* meta;
-    const int32_t* ppair;
-    int32_t n_ind;
-    int32_t early_exit;              // unused: a tile is one wavefront per pair, nothing to skip cheaply
-    unsigned long long* counts;
-    unsigned long long* visits;
-};
-
-__host__ __device__ inline size_t pairsmem_bytes(int32_t npairs, int32_t nbuf, int32_t n_ind) {
-    size_t cnt = (static_cast<size_t>(n_ind) * 4 + 127) & ~static_cast<size_t>(127);
-    return kSmemHeader + cnt + static_cast<size_t>(nbuf) * npairs * 128;
-}
-
-template <int NCONS>
-__global__ void __launch_bounds__((NCONS + 1) * 32, 1)
-fitness_pairsmem_kernel(const PairSmemParams p)
-{
-    extern __shared__ __align__(128) unsigned char smem[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem);          // [2]
-    uint64_t* empty = full + 2;                                  // [2]
-    uint32_t* s_cnt = reinterpret_cast<uint32_t*>(smem + kSmemHeader);
-    const size_t cnt_bytes = (static_cast<size_t>(p.n_ind) * 4 + 127) & ~static_cast<size_t>(127);
-    unsigned char* tiles = smem + kSmemHeader + cnt_bytes;
-    const uint32_t tile_bytes = static_cast<uint32_t>(p.npairs) * 128u;
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int64_t P = p.n_tiles * p.n_ind;
-    const int64_t pb = P * blockIdx.x / gridDim.x;
-    const int64_t pe = P * (blockIdx.x + 1) / gridDim.x;
-    if (pb >= pe) return;
-    const int64_t t0 = pb / p.n_ind, t1 = (pe - 1) / p.n_ind;
-    const int32_t ntl = static_cast<int32_t>(t1 - t0 + 1);
-    const int nbuf = p.nbuf;
-
-    for (int32_t k = tid; k < p.n_ind; k += blockDim.x) s_cnt[k] = 0;
-    if (tid == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
-        mbar_init(&empty[0], NCONS);
-        mbar_init(&empty[1], NCONS);
-        fence_mbar_init();
-    }
-    __syncthreads();
-
-    if (warp == NCONS) {
-        // producer: the tile is one contiguous block of npairs * 128 B; 4 KB pieces, lane-strided
-        for (int32_t j = 0; j < ntl; ++j) {
-            const int buf = (nbuf == 2) ? (j & 1) : 0;
-            const int32_t use = (nbuf == 2) ? (j >> 1) : j;      // how often this buffer was filled before
-            mbar_wait(&empty[buf], (use & 1) ^ 1);               // passes immediately on first use
-            if (lane == 0) mbar_arrive_expect_tx(&full[buf], tile_bytes);
-            __syncwarp();
-            const unsigned char* src = reinterpret_cast<const unsigned char*>(p.PB) + (t0 + j) * static_cast<int64_t>(tile_bytes);
-            unsigned char* dst = tiles + static_cast<size_t>(buf) * tile_bytes;
-            for (uint32_t off = lane * 4096u; off < tile_bytes; off += 32u * 4096u)
-                bulk_copy_g2s(dst + off, src + off, min(4096u, tile_bytes - off), &full[buf]);
-        }
-    } else {
-        unsigned long long visited = 0;
-        for (int32_t j = 0; j < ntl; ++j) {
-            const int buf = (nbuf == 2) ? (j & 1) : 0;
-            const int32_t use = (nbuf == 2) ? (j >> 1) : j;
-            const int32_t ka = (j == 0) ? static_cast<int32_t>(pb - t0 * p.n_ind) : 0;
-            const int32_t kb = (j == ntl - 1) ? static_cast<int32_t>(pe - t1 * p.n_ind) : p.n_ind;
-            const uint32_t lb = smem_u32(tiles + static_cast<size_t>(buf) * tile_bytes) + lane * 4;
-            int32_t k = ka + warp;
-            int2 m_cur = make_int2(0, 0), m_next = make_int2(0, 0);
-            int4 q_cur = make_int4(0, 0, 0, 0);
-            if (k < kb) {
-                m_cur = __ldg(&p.meta[k]);
-                q_cur = __ldg(reinterpret_cast<const int4*>(p.ppair) + m_cur.x);
-            }
-            if (k + NCONS < kb) m_next = __ldg(&p.meta[k + NCONS]);
-            mbar_wait(&full[buf], use & 1);
-            for (; k < kb; k += NCONS) {
-                const int2 m = m_cur;
-                int4 q = q_cur;
-                m_cur = m_next;
-                if (k + NCONS < kb) q_cur = __ldg(reinterpret_cast<const int4*>(p.ppair) + m_cur.x);
-                if (k + 2 * NCONS < kb) m_next = __ldg(&p.meta[k + 2 * NCONS]);
-                if (m.y < 2) continue;
-                const int32_t npr = m.y - 1;
-                const int4* qp = reinterpret_cast<const int4*>(p.ppair) + m.x;
-                unsigned int acc = 0xffffffffu;
-                int32_t i = 0;
-                for (; i + 4 < npr; i += 4) {                    // full quads with more to come
-                    const int4 qn = __ldg(qp + (i >> 2) + 1);
-                    const unsigned int v0 = lds32(lb + q.x * 128), v1 = lds32(lb + q.y * 128);
-                    const unsigned int v2 = lds32(lb + q.z * 128), v3 = lds32(lb + q.w * 128);
-                    acc &= v0 & v1;
-                    acc &= v2 & v3;
-                    q = qn;
-                }
-                {                                                // last quad: 1..4 real pairs, padded with the last
-                    const int32_t rem = npr - i;
-                    const unsigned int v0 = lds32(lb + q.x * 128);
-                    acc &= v0;
-                    if (rem >= 2) acc &= lds32(lb + q.y * 128);
-                    if (rem >= 3) acc &= lds32(lb + q.z * 128);
-                    if (rem >= 4) acc &= lds32(lb + q.w * 128);
-                }
-                visited += static_cast<unsigned long long>(npr) * kPairTileRows;
-                const int cnt = __reduce_add_sync(0xffffffffu, __popc(acc));
-                if (lane == 0 && cnt) atomicAdd(&s_cnt[k], static_cast<unsigned int>(cnt));
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&empty[buf]);
-        }
-        if (p.visits != nullptr && lane == 0 && visited) atomicAdd(p.visits, visited);
-    }
-    __syncthreads();
-    for (int32_t k = tid; k < p.n_ind; k += blockDim.x) {
-        const unsigned int c = s_cnt[k];
-        if (c) atomicAdd(&p.counts[k], static_cast<unsigned long long>(c));
-    }
-}
-
 }  // namespace ebic

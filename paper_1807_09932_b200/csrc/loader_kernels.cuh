@@ -7,11 +7,11 @@
 //       0x7F for NaN.  a >= b on float32 (ordered)  <=>  both codes have bit 7 set and
 //       code(a) >= code(b): the trend predicate depends only on the within-row order, so the
 //       fitness kernel can compare 4 rows per 32-bit word.
-//   a2" pair-relation bitmasks PB[tile][pair][32 words], tile = 1024 rows, pair (a,b) = a*cols + b:
-//       bit (r % 32) of word (r % 1024) / 32 of tile r / 1024 = ( M[r][b] >= M[r][a] ), ordered float32 >=.
-//       An L >= 2 chromosome matches row r iff all its L-1 consecutive pair bits are set, so the fitness
-//       kernel ANDs pair-rows: 1 bit per (row, pair) instead of an 8-bit rank per (row, column).
-//       The diagonal (a,a) is "not NaN"; padding rows are NaN, so their bits are 0.
+//   a2" pair-relation bit columns PB[pair][ld/32 words], pair (a,b) = a*cols + b (pair-major: the bit
+//       column of a pair is contiguous): bit (r % 32) of word r / 32 = ( M[r][b] >= M[r][a] ), ordered
+//       float32 >=.  An L >= 2 chromosome matches row r iff all its L-1 consecutive pair bits are set, so
+//       the fitness kernel ANDs bit columns: 1 bit per (row, pair) instead of an 8-bit rank per (row,
+//       column).  The diagonal (a,a) is "not NaN"; padding rows are NaN, so their bits are 0.
 // All HBM-bound, run once per ebic_create.
 #pragma once
 #include "ebic_device.cuh"
@@ -106,11 +106,11 @@ rank8_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint8_t* __
     }
 }
 
-// Pair bitmasks.  Block = 8 warps; warp w of block (t, y) owns column a = 8*y + w on tile t: it keeps the
-// tile's 1024 values of column a in registers (32 per lane, lane = row % 32) and walks every column b
-// (coalesced 128 B loads, served by L1 for the other 7 warps of the block), turning each 32-row
-// comparison into one ballot word; lane j keeps word j and the 32 words go out as one 128 B store.
-// grid = (ld / 1024, ceil(cols / 8)).
+// Pair bit columns.  Block = 8 warps; warp w of block (t, y) owns column a = 8*y + w on the 1024-row
+// tile t: it keeps the tile's 1024 values of column a in registers (32 per lane, lane = row % 32) and
+// walks every column b (coalesced 128 B loads, served by L1 for the other 7 warps of the block), turning
+// each 32-row comparison into one ballot word; lane j keeps word j and the 32 words go out as one 128 B
+// store into the bit column of pair (a, b).  grid = (ld / 1024, ceil(cols / 8)).
 __global__ void __launch_bounds__(256)
 pairbits_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint32_t* __restrict__ PB)
 {
@@ -123,7 +123,8 @@ pairbits_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint32_t
     const float* ca = tile + static_cast<int64_t>(a) * ld;
 #pragma unroll
     for (int j = 0; j < 32; ++j) va[j] = ca[32 * j];
-    uint32_t* out = PB + (t * cols * cols + static_cast<int64_t>(a) * cols) * 32 + lane;
+    const int64_t ldw = ld / 32;
+    uint32_t* out = PB + static_cast<int64_t>(a) * cols * ldw + t * 32 + lane;
     for (int32_t b = 0; b < cols; ++b) {
         const float* cb = tile + static_cast<int64_t>(b) * ld;
         unsigned int mine = 0;
@@ -132,7 +133,7 @@ pairbits_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint32_t
             const unsigned int w = __ballot_sync(0xffffffffu, cb[32 * j] >= va[j]);
             if (lane == j) mine = w;
         }
-        out[static_cast<int64_t>(b) * 32] = mine;
+        out[static_cast<int64_t>(b) * ldw] = mine;
     }
 }
 

@@ -28,7 +28,7 @@ def B():
 
 def kernels_for(eb, B):
     ks = [B.EBIC_KERNEL_DIRECT]
-    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_PAIRBITS_SMEM):
+    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_PAIRBITS):
         try:
             eb.set_kernel(k)
             ks.append(k)
@@ -114,15 +114,15 @@ def test_loader_products(B, rows, cols, nan_rate):
             below = (m[:, None, :] < m[:, :, None]).sum(axis=2)                   # [rows][cols]
             code = np.where(np.isnan(m), 0x7F, 0x80 | below).astype(np.uint8)
             assert (rk[:, :rows] == code.T).all() and (rk[:, rows:] == 0x7F).all()
-            # pair table [tile][a*cols+b][32 words]: bit r = (m[r][b] >= m[r][a]); padding rows 0
+            # pair table [a*cols+b][ld/32 words]: bit r = (m[r][b] >= m[r][a]); padding rows 0
             pb = eb.debug_read(4)
             assert eb.info(14) == pb.nbytes
             mp = np.full((ld, cols), np.nan, dtype=np.float32)
             mp[:rows] = m
             with np.errstate(invalid="ignore"):
                 ge = mp[:, None, :] >= mp[:, :, None]                              # [ld][a][b]
-            want = np.ascontiguousarray(np.packbits(ge.reshape(ld // 1024, 1024, cols * cols).transpose(0, 2, 1),
-                                                    axis=2, bitorder="little")).view(np.uint32)
+            want = np.ascontiguousarray(np.packbits(ge.reshape(ld, cols * cols).T, axis=1,
+                                                    bitorder="little")).view(np.uint32)
             assert (pb == want).all()
 
 
@@ -209,8 +209,6 @@ def test_wide_matrix_falls_back(B, oracle_mod):
         with B.Ebic(m, ON) as eb:
             with pytest.raises(B.EbicError):
                 eb.set_kernel(B.EBIC_KERNEL_RANK8)
-            with pytest.raises(B.EbicError):
-                eb.set_kernel(B.EBIC_KERNEL_PAIRBITS_SMEM)
             assert eb.kernel == B.EBIC_KERNEL_PAIRBITS
             eb.set_pairbits(False)
             assert eb.info(14) == 0
@@ -300,20 +298,17 @@ def test_instrumentation_counts_executed_visits(B):
             assert seen[False] == nominal                          # plain work: executed == nominal
             assert 2 * eb.ld * w.n_ind <= seen[True] <= nominal    # early exit only ever skips columns
         nominal_pairs = eb.ld * int((w.lengths - 1).sum())         # pair kernels count (row, pair) fetches
-        for kern in (B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_PAIRBITS_SMEM):
-            if kern not in kernels_for(eb, B):
-                continue
-            eb.set_kernel(kern)
-            for early_exit in (False, True):
-                eb.set_early_exit(early_exit)
-                eb.set_instrumentation(1)
-                eb.eval_fitness(dev(w.offsets), dev(w.col_ids))
-                seen = eb.info(10)
-                eb.set_instrumentation(0)
-                if early_exit and kern == B.EBIC_KERNEL_PAIRBITS:
-                    assert eb.ld * w.n_ind <= seen <= nominal_pairs
-                else:
-                    assert seen == nominal_pairs
+        eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)
+        for early_exit in (False, True):
+            eb.set_early_exit(early_exit)
+            eb.set_instrumentation(1)
+            eb.eval_fitness(dev(w.offsets), dev(w.col_ids))
+            seen = eb.info(10)
+            eb.set_instrumentation(0)
+            if early_exit:
+                assert eb.ld * w.n_ind <= seen <= nominal_pairs
+            else:
+                assert seen == nominal_pairs
 
 
 # ------------------------------------------------------------------------- full-size C5 (bench config)
@@ -330,7 +325,7 @@ def test_c5_full_size_sampled(B, oracle_mod):
     with B.Ebic(w.matrix, w.missing_mode) as eb:
         import torch
         results = {}
-        for kern in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_PAIRBITS_SMEM):
+        for kern in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_PAIRBITS):
             eb.set_kernel(kern)
             for early_exit in (False, True):
                 eb.set_early_exit(early_exit)
