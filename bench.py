@@ -120,17 +120,42 @@ def pick_chosen(w):
 # ----------------------------------------------------------------------------------------------------
 # roofline of the fitness kernel
 # ----------------------------------------------------------------------------------------------------
-def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None):
+L1_RESIDENT_BYTES = 192 << 10    # a 1,024-row slice of every pair column (cols^2 x 128 B) fits L1 below this
+
+
+def measure_l2_gbs(B):
+    """L2 -> SM read bandwidth measured live on this GPU (64 MiB buffer, L1 bypassed): ebic_probe_read_bandwidth."""
+    return B.ebic_probe_read_bandwidth(64 << 20, 40)
+
+
+def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None, cols=None, l2_gbs=None):
+    """each kernel against the data pipe its operands have to come through."""
     f_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
-    smem_peak_gbs = sm_count * 128 * f_hz / 1e9            # 128 B / clk / SM shared-memory data pipe
+    pipe_gbs = sm_count * 128 * f_hz / 1e9                 # 128 B / clk / SM: shared memory and L1 share this pipe
+    pipe_basis = f"{sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz ({peaks_kind} sm_max_mhz)"
     bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "direct": 4, "pairbits": 0.125}[kernel_name]
     achieved = visits_executed * bytes_per_visit / kernel_s / 1e9
-    return {"bound": "alu", "resource": "shared-memory data pipe (128 B/clk/SM) == ALU pipe at 0.5 op/visit"
-            if kernel_name == "rank8" else "shared-memory data pipe (128 B/clk/SM)",
-            "kernel": "fitness_" + kernel_name, "achieved": achieved, "peak": smem_peak_gbs, "unit": "GB/s",
-            "frac": achieved / smem_peak_gbs, "traffic": traffic,
-            "bytes_per_visit": bytes_per_visit, "visits_per_launch": visits_executed,
-            "kernel_ms": kernel_s * 1e3, "peak_basis": f"{sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz ({peaks_kind} sm_max_mhz)"}
+    bound, peak, basis = "alu", pipe_gbs, pipe_basis
+    resource = "shared-memory data pipe (128 B/clk/SM)"
+    if kernel_name == "rank8":
+        resource += " == INT ALU pipe at 0.5 op/visit"
+    elif kernel_name == "direct":
+        resource = "L1/LSU data pipe (128 B/clk/SM)"
+    elif kernel_name == "pairbits":
+        wide = cols is not None and cols * cols * 128 > L1_RESIDENT_BYTES
+        if wide and l2_gbs:
+            bound, peak = "l2", l2_gbs
+            resource = "L2 -> SM read bandwidth (bit columns gathered from L2; working set too wide for L1)"
+            basis = "ebic_probe_read_bandwidth(64 MiB, L1 bypassed), measured in this run"
+        else:
+            resource = "L1/LSU data pipe (128 B/clk/SM; bit columns gathered through L1)"
+    out = {"bound": bound, "resource": resource, "kernel": "fitness_" + kernel_name, "achieved": achieved,
+           "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+           "bytes_per_visit": bytes_per_visit, "visits_per_launch": visits_executed,
+           "kernel_ms": kernel_s * 1e3, "peak_basis": basis}
+    if bound == "l2":
+        out["frac_of_lsu_pipe"] = achieved / pipe_gbs      # the strict on-chip ceiling, for comparison
+    return out
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -262,12 +287,13 @@ def run_gpu(args):
     out = None
     if rank == 0:
         sm_count = eb.info(7)
+        l2_gbs = measure_l2_gbs(B) if kernel_name == "pairbits" else None
         roof = roofline(kernel_name, visits_exec, kernel_ns * 1e-9, peaks, peaks_kind, sm_count,
-                        traffic=args.traffic)
+                        traffic=args.traffic, cols=w.cols, l2_gbs=l2_gbs)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "u8" if kernel_name == "rank8" else "f32", "data": "synthetic",
+            "vs_baseline": None, "dtype": {"rank8": "u8", "pairbits": "u32"}.get(kernel_name, "f32"), "data": "synthetic",
             "config": {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind,
                        "sum_L": int(w.lengths.sum()), "missing_mode": w.missing_mode, "kernel": kernel_name,
                        "tile_rows": eb.info(5), "ctas": eb.info(6), "n_chosen": int(len(chosen)),
@@ -368,6 +394,8 @@ def run_table(args):
     peaks, peaks_kind = measured_peaks()
     torch.cuda.set_device(0)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    l2_gbs = measure_l2_gbs(B)
+    log(f"L2 -> SM read bandwidth (probe): {l2_gbs:.0f} GB/s")
     rows_out = []
     names = args.table_workloads.split(",")
     for name in names:
@@ -427,7 +455,7 @@ def run_table(args):
             except Exception as ex:                              # noqa: BLE001
                 log("graph replay unavailable:", ex)
                 torch.cuda.synchronize()
-            roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7))
+            roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7), cols=w.cols, l2_gbs=l2_gbs)
             rows_out.append({"workload": w.cfg.name, "kernel": kname, "early_exit": ee,
                              "executed_over_nominal_visits": visits / nominal,
                              "call_ms_median": statistics.median(call_ms),
@@ -438,24 +466,33 @@ def run_table(args):
                              "roofline_frac": roof["frac"], "achieved_gbs": roof["achieved"], "tile_rows": eb.info(5),
                              "ctas": eb.info(6)})
             log(json.dumps(rows_out[-1]))
-        # extraction (a7): HBM-bound
+        # extraction (a7): HBM-bound.  Two sources: the pair table's bit columns (default when it exists;
+        # (L-1) * ld/8 bytes read per individual) and the float32 columns (4 * L * ld bytes read).
         eb.set_kernel(0)
-        ex_ms = []
-        for _ in range(10):
-            flush.zero_()
-            s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            s.record()
-            eb.extract_rows(d_off, d_ids, d_chosen, masks=d_masks, want_counts=False)
-            e.record()
-            torch.cuda.synchronize()
-            ex_ms.append(s.elapsed_time(e))
         Lsum = int(sum(w.lengths[k] for k in chosen))
-        ex_bytes = eb.ld * 4 * Lsum + len(chosen) * eb.mask_words * 8
-        rows_out.append({"workload": w.cfg.name, "kernel": "extract_rows", "call_ms_median": statistics.median(ex_ms),
-                         "hbm_gbs": ex_bytes / (statistics.median(ex_ms) * 1e-3) / 1e9,
-                         "hbm_frac": ex_bytes / (statistics.median(ex_ms) * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                         "n_chosen": int(len(chosen)), "bytes": ex_bytes})
-        log(json.dumps(rows_out[-1]))
+        Psum = int(sum(max(int(w.lengths[k]) - 1, 0) for k in chosen))
+        for source in ("pairbits", "float32"):
+            if source == "pairbits" and eb.info(14) == 0:
+                continue
+            eb.set_extract_source(source == "pairbits")
+            ex_ms = []
+            for _ in range(10):
+                flush.zero_()
+                s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                s.record()
+                eb.extract_rows(d_off, d_ids, d_chosen, masks=d_masks, want_counts=False)
+                e.record()
+                torch.cuda.synchronize()
+                ex_ms.append(s.elapsed_time(e))
+            read_bytes = eb.ld // 8 * Psum if source == "pairbits" else eb.ld * 4 * Lsum
+            ex_bytes = read_bytes + len(chosen) * eb.mask_words * 8
+            rows_out.append({"workload": w.cfg.name, "kernel": "extract_rows", "source": source,
+                             "call_ms_median": statistics.median(ex_ms),
+                             "hbm_gbs": ex_bytes / (statistics.median(ex_ms) * 1e-3) / 1e9,
+                             "hbm_frac": ex_bytes / (statistics.median(ex_ms) * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                             "n_chosen": int(len(chosen)), "bytes": ex_bytes})
+            log(json.dumps(rows_out[-1]))
+        eb.set_extract_source(True)
         if not args.no_cpu_baseline:
             rows_out.append({"workload": w.cfg.name, "kernel": "cpu_oracle", **cpu_baseline(w, budget_s=args.cpu_budget)})
             log(json.dumps(rows_out[-1]))

@@ -170,6 +170,17 @@ int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);
  */
 int ebic_debug_read(const ebic_ctx *ctx, int32_t what, void *dst, int64_t dst_bytes);
 
+/*
+ * Measurement utility (not a step of the path): read bandwidth, in GB/s, that all SMs together get
+ * from a freshly allocated device buffer of `buffer_bytes` (>= 1 MiB) streamed `reps` times with
+ * coalesced 128-bit loads that bypass L1 (best of 3 passes after a warm-up pass, CUDA events on the
+ * legacy stream).  A buffer that fits the L2 (e.g. 64 MiB) gives the L2 -> SM bandwidth -- the
+ * roofline bench.py uses for the PAIRBITS kernel on matrices too wide for L1 residency --, one far
+ * larger than the L2 gives HBM read bandwidth.  Synchronous; allocates and frees its own memory.
+ * Errors: EBIC_ERR_ARG, EBIC_ERR_OOM, EBIC_ERR_CUDA (*gb_per_s = 0).
+ */
+int ebic_probe_read_bandwidth(int64_t buffer_bytes, int32_t reps, double *gb_per_s);
+
 /* Static string for a status code. */
 const char *ebic_strerror(int status);
 

@@ -50,6 +50,7 @@ SYMBOLS = {
     "ebic_set_instrumentation": (ctypes.c_int, [_vp, _i32]),
     "ebic_get_info": (_i64, [_vp, _i32]),
     "ebic_debug_read": (ctypes.c_int, [_vp, _i32, _vp, _i64]),
+    "ebic_probe_read_bandwidth": (ctypes.c_int, [_i64, _i32, ctypes.POINTER(ctypes.c_double)]),
     "ebic_strerror": (ctypes.c_char_p, [ctypes.c_int]),
 }
 
@@ -155,6 +156,14 @@ def ebic_debug_read(ctx, what: int, dst: np.ndarray) -> None:
 
 
 # ---------------------------------------------------------------- convenience wrapper
+def ebic_probe_read_bandwidth(buffer_bytes: int, reps: int) -> float:
+    out = ctypes.c_double(0.0)
+    st = load_library().ebic_probe_read_bandwidth(int(buffer_bytes), int(reps), ctypes.byref(out))
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_probe_read_bandwidth")
+    return out.value
+
+
 def _require_cuda():
     import torch
     if not torch.cuda.is_available():

@@ -13,6 +13,7 @@
 #include "fitness_kernels.cuh"
 #include "loader_kernels.cuh"
 #include "pairbits_kernels.cuh"
+#include "probe_kernels.cuh"
 
 using namespace ebic;
 
@@ -193,7 +194,7 @@ int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, unsigned long long* counts, cu
     p.PB = ctx->PB;
     p.ldw = ctx->ld / 32;
     // about `tasks_per_slot` tasks per resident warp slot (4 CTAs / SM), 256..2048 words (8,192..65,536 rows) per task
-    static const int64_t tasks_per_slot = env_int("EBIC_PB_TASKS_PER_SLOT", 4);
+    static const int64_t tasks_per_slot = env_int("EBIC_PB_TASKS_PER_SLOT", 8);
     const int64_t want_tasks = tasks_per_slot * ctx->sm_count * 4 * kPairbitsWarps;
     int64_t cw = p.ldw * n_ind / want_tasks;
     cw = std::max<int64_t>(kPairbitsStepWords, std::min<int64_t>(8 * kPairbitsStepWords, cw / kPairbitsStepWords * kPairbitsStepWords));
@@ -204,6 +205,9 @@ int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, unsigned long long* counts, cu
     p.n_ind = n_ind;
     p.counts = counts;
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
+    p.n_pairs = ctx->cols * ctx->cols;
+    static const int prefetch_dist = env_int("EBIC_PB_PREFETCH", 1);
+    p.prefetch_dist = prefetch_dist;
     const int64_t tasks = static_cast<int64_t>(p.n_chunks) * n_ind;
     const int64_t grid = (tasks + kPairbitsWarps - 1) / kPairbitsWarps;
     if (grid > 0x7fffffffll) return EBIC_ERR_ARG;
@@ -677,6 +681,46 @@ int ebic_debug_read(const ebic_ctx* ctx, int32_t what, void* dst, int64_t dst_by
     }
     if (!src || bytes != dst_bytes) return EBIC_ERR_ARG;
     return cuda_status(cudaMemcpy(dst, src, static_cast<size_t>(bytes), cudaMemcpyDeviceToHost));
+}
+
+int ebic_probe_read_bandwidth(int64_t buffer_bytes, int32_t reps, double* gb_per_s) {
+    if (!gb_per_s || buffer_bytes < (1ll << 20) || reps < 1) return EBIC_ERR_ARG;
+    *gb_per_s = 0.0;
+    int dev = 0, sms = 0;
+    EBIC_TRY(cudaGetDevice(&dev));
+    EBIC_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int64_t n_vec = buffer_bytes / 16;
+    if (n_vec / (8ll * sms * 8 * 256) <= 0) return EBIC_ERR_ARG;
+    uint4* buf = nullptr;
+    unsigned int* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    int st = cuda_status(cudaMalloc(&buf, static_cast<size_t>(n_vec) * 16));
+    if (!st) st = cuda_status(cudaMalloc(&sink, 4));
+    if (!st) st = cuda_status(cudaMemset(buf, 0x5a, static_cast<size_t>(n_vec) * 16));
+    if (!st) st = cuda_status(cudaEventCreate(&e0));
+    if (!st) st = cuda_status(cudaEventCreate(&e1));
+    double best = 0.0;
+    for (int per_sm = 2; per_sm <= 8 && !st; per_sm *= 2) {        // 2, 4, 8 CTAs of 256 threads per SM: keep the best
+        const int grid = sms * per_sm;
+        const int64_t stride = static_cast<int64_t>(grid) * 256;
+        const int64_t span = n_vec / (8 * stride) * (8 * stride);
+        for (int pass = 0; pass < 4 && !st; ++pass) {            // pass 0 warms the cache; best of the next 3
+            cudaEventRecord(e0, nullptr);
+            probe_read_kernel<<<grid, 256>>>(buf, n_vec, reps, sink);
+            cudaEventRecord(e1, nullptr);
+            st = cuda_status(cudaEventSynchronize(e1));
+            float ms = 0.f;
+            if (!st) st = cuda_status(cudaEventElapsedTime(&ms, e0, e1));
+            if (!st && pass > 0 && ms > 0.f)
+                best = std::max(best, static_cast<double>(span) * 16.0 * reps / (ms * 1e-3) / 1e9);
+        }
+    }
+    if (!st) *gb_per_s = best;
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(sink);
+    cudaFree(buf);
+    return st;
 }
 
 const char* ebic_strerror(int status) {

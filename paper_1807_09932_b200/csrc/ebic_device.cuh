@@ -58,6 +58,12 @@ __device__ __forceinline__ void bulk_copy_g2s(void* smem_dst, const void* gmem_s
         : "memory");
 }
 
+// L2 prefetch of `bytes` (multiple of 16) at a 16-byte aligned global address; no register or shared-memory
+// destination, no completion to wait for (SASS: UBLKPF).
+__device__ __forceinline__ void bulk_prefetch_l2(const void* gmem_src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
+}
+
 // 128-bit shared-memory load from a 32-bit shared-window address (SASS: LDS.128 [R+imm]): the address
 // comes straight out of one IMAD (id * column stride + lane base), no generic-pointer arithmetic.
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {

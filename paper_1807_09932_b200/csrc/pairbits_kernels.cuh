@@ -32,6 +32,8 @@ struct PairbitsParams {
     int32_t n_ind;
     unsigned long long* counts;
     unsigned long long* visits;      // executed (row, pair) visits (instrumented) or nullptr
+    int32_t n_pairs;                 // cols * cols bit columns in PB
+    int32_t prefetch_dist;           // CTAs of chunk g prefetch a slice of the bit columns of chunk g + dist into L2 (0 = off)
 };
 
 __device__ __forceinline__ void and4(uint4& a, const uint4& v) {
@@ -49,6 +51,23 @@ fitness_pairbits_kernel(const PairbitsParams p)
     const int32_t k = static_cast<int32_t>(task - g * p.n_ind);
     const int64_t w_begin = g * p.chunk_words;
     if (w_begin >= p.ldw) return;                                // warp-uniform
+    if (p.prefetch_dist > 0 && warp == 0) {
+        // Every bit column of a later chunk is requested from HBM exactly once, by one lane of one CTA of
+        // this chunk, `prefetch_dist` chunks before the demand loads arrive: those then hit L2.
+        const int64_t ctas_per_chunk = (static_cast<int64_t>(p.n_ind) + kPairbitsWarps - 1) / kPairbitsWarps;
+        const int64_t j = blockIdx.x - g * p.n_ind / kPairbitsWarps; // position of this CTA inside its chunk (approx.)
+        const int32_t per_cta = static_cast<int32_t>((p.n_pairs + ctas_per_chunk - 1) / ctas_per_chunk);
+        const int64_t first = (g == 0) ? 1 : p.prefetch_dist;        // chunk 0 also covers the cold start
+        for (int64_t d = first; d <= p.prefetch_dist; ++d) {
+            const int64_t pw = (g + d) * p.chunk_words;
+            if (pw >= p.ldw) break;
+            const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.chunk_words), p.ldw - pw)) * 4u;
+            for (int32_t q = lane; q < per_cta; q += 32) {
+                const int64_t pair = j * per_cta + q;
+                if (pair >= 0 && pair < p.n_pairs) bulk_prefetch_l2(p.PB + pair * p.ldw + pw, bytes);
+            }
+        }
+    }
     const int32_t rec = __ldg(p.prec + 32ll * k + lane);         // the individual: one coalesced 128 B load
     const int32_t L = __shfl_sync(0xffffffffu, rec, 0);
     if (L < 2) return;
