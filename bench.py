@@ -120,11 +120,14 @@ def pick_chosen(w):
 # ----------------------------------------------------------------------------------------------------
 # roofline of the fitness kernel
 # ----------------------------------------------------------------------------------------------------
-L1_RESIDENT_BYTES = 192 << 10    # a 1,024-row slice of every pair column (cols^2 x 128 B) fits L1 below this
+# L2 -> crossbar peak of this B200 as ncu states it: derived__lts__lts2xbar_bytes.sum.peak_sustained = 11,776 B/clk
+# (184 L2 slices x 64 B/clk; profiles/r01_fitness_pairbits_c4_ncu_full.txt), at the L2 clock == sm_max_mhz.
+L2_XBAR_BYTES_PER_CLK = 184 * 64
 
 
 def measure_l2_gbs(B):
-    """L2 -> SM read bandwidth measured live on this GPU (64 MiB buffer, L1 bypassed): ebic_probe_read_bandwidth."""
+    """What a plain streaming read of an L2-resident buffer reaches on this GPU (64 MiB, L1 bypassed):
+    ebic_probe_read_bandwidth.  Context for the L2 roofline, not its denominator."""
     return B.ebic_probe_read_bandwidth(64 << 20, 40)
 
 
@@ -142,19 +145,17 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
     elif kernel_name == "direct":
         resource = "L1/LSU data pipe (128 B/clk/SM)"
     elif kernel_name == "pairbits":
-        wide = cols is not None and cols * cols * 128 > L1_RESIDENT_BYTES
-        if wide and l2_gbs:
-            bound, peak = "l2", l2_gbs
-            resource = "L2 -> SM read bandwidth (bit columns gathered from L2; working set too wide for L1)"
-            basis = "ebic_probe_read_bandwidth(64 MiB, L1 bypassed), measured in this run"
-        else:
-            resource = "L1/LSU data pipe (128 B/clk/SM; bit columns gathered through L1)"
+        bound, peak = "l2", L2_XBAR_BYTES_PER_CLK * f_hz / 1e9
+        resource = "L2 -> SM read bandwidth (bit columns gathered from L2 with 128-bit loads)"
+        basis = (f"184 L2 slices x 64 B/clk x {f_hz/1e6:.0f} MHz (ncu lts2xbar peak_sustained; a plain L2-resident "
+                 f"streaming read reaches {l2_gbs:.0f} GB/s in this run)" if l2_gbs else
+                 f"184 L2 slices x 64 B/clk x {f_hz/1e6:.0f} MHz (ncu lts2xbar peak_sustained)")
     out = {"bound": bound, "resource": resource, "kernel": "fitness_" + kernel_name, "achieved": achieved,
            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
            "bytes_per_visit": bytes_per_visit, "visits_per_launch": visits_executed,
            "kernel_ms": kernel_s * 1e3, "peak_basis": basis}
     if bound == "l2":
-        out["frac_of_lsu_pipe"] = achieved / pipe_gbs      # the strict on-chip ceiling, for comparison
+        out["l2_probe_gbs"] = l2_gbs
     return out
 
 
@@ -194,12 +195,14 @@ def run_gpu(args):
     create_ms = (time.time() - t0) * 1e3
     eb.set_kernel(KERNELS[args.kernel])
     eb.set_early_exit(args.early_exit)
-    kernel_name = B.KERNEL_NAMES[eb.kernel]
 
     d_off = torch.from_numpy(w.offsets).cuda()
     d_ids = torch.from_numpy(w.col_ids).cuda()
     d_chosen = torch.from_numpy(chosen).cuda()
     d_counts = torch.empty(w.n_ind, dtype=torch.int64, device="cuda")
+    eb.eval_fitness(d_off, d_ids, counts=d_counts)             # AUTO picks by shape and population size
+    torch.cuda.synchronize()
+    kernel_name = B.KERNEL_NAMES[eb.last_kernel]
     d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
     d_mcnt = torch.empty(len(chosen), dtype=torch.int64, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
@@ -421,7 +424,7 @@ def run_table(args):
             eb.set_instrumentation(1)
             eb.eval_fitness(d_off, d_ids, counts=d_counts)
             visits = eb.info(10) if kname != "direct" else eb.ld * int(w.lengths.sum())
-            nominal = eb.ld * int((w.lengths - 1).sum() if kname.startswith("pairbits") else w.lengths.sum())
+            nominal = eb.ld * int((w.lengths - 1).sum() if kname.startswith("pair") else w.lengths.sum())
             eb.set_instrumentation(2)
             call_ms = []
             for _ in range(reps):

@@ -53,7 +53,7 @@ enum {
     EBIC_KERNEL_DIRECT = 1,  /* one thread per row, column-major global loads (any shape)          */
     EBIC_KERNEL_TILED_F32 = 2, /* float32 row tiles staged in shared memory by TMA bulk copies    */
     EBIC_KERNEL_RANK8 = 3,   /* per-row order-preserving 8-bit rank tiles (cols <= 127)           */
-    EBIC_KERNEL_PAIRBITS = 4 /* AND of pair-relation bit columns gathered by TMA bulk copies (pair table built) */
+    EBIC_KERNEL_PAIRBITS = 4 /* AND of pair-relation bit columns streamed through L2 (pair table built)    */
 };
 
 /*
@@ -119,7 +119,7 @@ int ebic_set_kernel(ebic_ctx *ctx, int32_t kernel);
  * Pair-relation table: bit r of pair (a,b) = ( M[r][b] >= M[r][a] ), cols^2 * ceil(rows/1024) * 128
  * bytes of device memory, one contiguous bit column per ordered pair.  With it an L >= 2 chromosome is
  * the AND of its L-1 bit columns (the PAIRBITS kernel; extraction reads it too).  on != 0 builds it if absent (EBIC_ERR_OOM if it does
- * not fit; EBIC_ERR_ARG if cols > 46340), on == 0 frees it.  Synchronises the device.
+ * not fit; EBIC_ERR_ARG if cols > 46340 or the table would exceed 64 GiB), on == 0 frees it.  Synchronises the device.
  */
 int ebic_set_pairbits(ebic_ctx *ctx, int32_t on);
 
@@ -155,7 +155,8 @@ int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
  *   use, 5 rows per shared-memory tile of that kernel, 6 CTAs of its last launch, 7 SM count,
  *   8 kernels launched by this context so far, 9 bytes of device memory the context owns,
  *   10 executed column visits since the last read, 11 mean fitness-kernel time in ns, 12 evals
- *   timed (see ebic_set_instrumentation), 13 early exit on/off, 14 bytes of the pair table (0 = absent).
+ *   timed (see ebic_set_instrumentation), 13 early exit on/off, 14 bytes of the pair table (0 = absent), 15 kernel (EBIC_KERNEL_*)
+ *   of the last fitness launch (0 = none yet).
  * Returns -1 for NULL / unknown `what`.
  */
 int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);

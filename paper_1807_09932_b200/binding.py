@@ -304,6 +304,11 @@ class Ebic:
     def kernel(self) -> int:
         return self.info(4)
 
+    @property
+    def last_kernel(self) -> int:
+        """Kernel of the last fitness launch 0 = none yet."""
+        return self.info(15)
+
     def debug_read(self, what: int) -> np.ndarray:
         ld, cols = self.ld, self.cols
         if what == 0:

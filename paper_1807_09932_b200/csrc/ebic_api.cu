@@ -65,6 +65,7 @@ struct ebic_ctx {
     int64_t launches = 0;
     int32_t last_grid = 0;
     int32_t last_T = 0;
+    int32_t last_kernel = 0;                // kernel of the last fitness launch (0 = none yet)
 };
 
 namespace {
@@ -195,7 +196,7 @@ int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, unsigned long long* counts, cu
     p.ldw = ctx->ld / 32;
     // about `tasks_per_slot` tasks per resident warp slot (4 CTAs / SM), 256..2048 words (8,192..65,536 rows) per task
     static const int64_t tasks_per_slot = env_int("EBIC_PB_TASKS_PER_SLOT", 8);
-    const int64_t want_tasks = tasks_per_slot * ctx->sm_count * 4 * kPairbitsWarps;
+    const int64_t want_tasks = tasks_per_slot * ctx->sm_count * 32;
     int64_t cw = p.ldw * n_ind / want_tasks;
     cw = std::max<int64_t>(kPairbitsStepWords, std::min<int64_t>(8 * kPairbitsStepWords, cw / kPairbitsStepWords * kPairbitsStepWords));
     p.chunk_words = static_cast<int32_t>(cw);
@@ -209,14 +210,25 @@ int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, unsigned long long* counts, cu
     static const int prefetch_dist = env_int("EBIC_PB_PREFETCH", 1);
     p.prefetch_dist = prefetch_dist;
     const int64_t tasks = static_cast<int64_t>(p.n_chunks) * n_ind;
-    const int64_t grid = (tasks + kPairbitsWarps - 1) / kPairbitsWarps;
+    static const int nw = env_int("EBIC_PB_WARPS", 2);
+    const int64_t grid = (tasks + nw - 1) / nw;
     if (grid > 0x7fffffffll) return EBIC_ERR_ARG;
     ctx->last_grid = static_cast<int32_t>(grid);
     ctx->last_T = static_cast<int32_t>(cw * 32);
-    if (ctx->early_exit)
-        fitness_pairbits_kernel<true><<<static_cast<unsigned>(grid), kPairbitsWarps * 32, 0, stream>>>(p);
-    else
-        fitness_pairbits_kernel<false><<<static_cast<unsigned>(grid), kPairbitsWarps * 32, 0, stream>>>(p);
+    const unsigned g = static_cast<unsigned>(grid);
+#define EBIC_PB_LAUNCH(NW)                                                              \
+    do {                                                                                \
+        if (ctx->early_exit) fitness_pairbits_kernel<true, NW><<<g, NW * 32, 0, stream>>>(p);  \
+        else fitness_pairbits_kernel<false, NW><<<g, NW * 32, 0, stream>>>(p);                 \
+    } while (0)
+    switch (nw) {
+        case 1: EBIC_PB_LAUNCH(1); break;
+        case 2: EBIC_PB_LAUNCH(2); break;
+        case 4: EBIC_PB_LAUNCH(4); break;
+        case 8: EBIC_PB_LAUNCH(8); break;
+        default: EBIC_PB_LAUNCH(2); break;
+    }
+#undef EBIC_PB_LAUNCH
     ctx->launches++;
     return cuda_status(cudaGetLastError());
 }
@@ -226,6 +238,7 @@ int build_pairbits(ebic_ctx* ctx) {
     if (ctx->PB) return EBIC_OK;
     if (ctx->cols > 46340) return EBIC_ERR_ARG;                  // cols^2 must fit int32
     const int64_t bytes = static_cast<int64_t>(ctx->cols) * ctx->cols * (ctx->ld / 8);
+    if (bytes > (64ll << 30)) return EBIC_ERR_ARG;               // bit-column offsets are uint32 in 16-byte units
     int st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->PB), bytes);
     if (st) return st;
     ctx->pb_bytes = bytes;
@@ -265,10 +278,11 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         if (st) return st;
     }
 
-    ingest_population_kernel<<<(n_ind + 255) / 256, 256, 0, stream>>>(
+    ingest_population_kernel<<<(n_ind + 7) / 8, 256, 0, stream>>>(
         offsets, col_ids, n_ind, n_ids, ctx->cols, ctx->rows, ctx->missing_mode == EBIC_MISSING_ON,
         ctx->nonmissing, ctx->meta, ctx->pids, ctx->cols <= 256 ? ctx->pids8 : nullptr,
-        ctx->PB ? ctx->ppair : nullptr, ctx->PB ? ctx->prec : nullptr, counts, ctx->d_err);
+        ctx->PB ? ctx->ppair : nullptr, ctx->PB ? ctx->prec : nullptr, static_cast<uint32_t>(ctx->ld / 128), counts,
+        ctx->d_err);
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());
 
@@ -285,6 +299,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     for (int32_t k0 = 0; k0 < n_ind; k0 += per_launch) {
         const int32_t n = std::min<int32_t>(per_launch, n_ind - k0);
         const int32_t kernel = whole ? EBIC_KERNEL_PAIRBITS : resolve_kernel(ctx, n);
+        ctx->last_kernel = kernel;
         if (kernel == EBIC_KERNEL_PAIRBITS) {
             if (!ctx->PB) return EBIC_ERR_ARG;
             st = launch_pairbits(ctx, n, counts, stream);
@@ -662,6 +677,7 @@ int64_t ebic_get_info(ebic_ctx* ctx, int32_t what) {
         case 12: return ctx->timed_evals;
         case 13: return ctx->early_exit;
         case 14: return ctx->pb_bytes;
+        case 15: return ctx->last_kernel;
         default: return -1;
     }
 }

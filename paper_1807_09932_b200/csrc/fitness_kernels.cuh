@@ -13,7 +13,7 @@ namespace ebic {
 constexpr int kRecPairs = 30;        // pair indices held in an individual's 128-byte record
 
 // ------------------------------------------------------------------------------------------------
-// a3  Population ingest + validation.  One thread per individual.
+// a3  Population ingest + validation.  One warp per individual.
 //   meta[k] = { slot4, L }   slot4 = index, in 4-entry groups, of the individual's id slot; L = chromosome
 //                            length, or -1 if the individual is invalid.
 //   pids    = int32 ids copied to the slot (entries 4*slot4 ..), padded to a multiple of 4 with the last id
@@ -22,10 +22,11 @@ constexpr int kRecPairs = 30;        // pair indices held in an individual's 128
 //             four ids with one warp-uniform 32-bit load.
 //   The slot of individual k starts at entry (offsets[k] + 3k) & ~3: 4-aligned and disjoint from its
 //   neighbours without a prefix sum.
-//   ppair   = (pair-bit kernels) the L-1 pair indices id_i * cols + id_{i+1} in the same slot (entries
-//             4*slot4 ..), padded to a multiple of 4 with the last pair (AND is idempotent).
+//   ppair   = (pair-bit kernels) for each of the L-1 pairs (id_i, id_{i+1}) the offset of its bit column in
+//             the pair table in 16-byte units, (id_i * cols + id_{i+1}) * pair_stride16 as uint32, in the same
+//             slot (entries 4*slot4 ..), padded to a multiple of 4 with the last pair (AND is idempotent).
 //   prec    = (pair-bit kernels) one 128-byte record per individual, read by a warp with ONE coalesced
-//             load: [0] = L (-1 = invalid), [1] = slot4, [2..31] = the first 30 pair indices, padded with
+//             load: [0] = L (-1 = invalid), [1] = slot4, [2..31] = the first 30 pair offsets, padded with
 //             the last pair.
 //   counts[k] is initialised: rows (L = 0, or L = 1 in mode OFF), non-missing rows of the column
 //             (L = 1, mode ON), else 0 -- the chain kernels then add to it.
@@ -35,49 +36,62 @@ ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __r
                          int32_t n_ind, int64_t n_ids, int32_t cols, int64_t rows, int32_t missing_on,
                          const unsigned long long* __restrict__ nonmissing, int2* __restrict__ meta,
                          int32_t* __restrict__ pids, uint8_t* __restrict__ pids8, int32_t* __restrict__ ppair,
-                         int32_t* __restrict__ prec, unsigned long long* __restrict__ counts,
-                         int32_t* __restrict__ err)
+                         int32_t* __restrict__ prec, uint32_t pair_stride16,
+                         unsigned long long* __restrict__ counts, int32_t* __restrict__ err)
 {
-    const int32_t k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n_ind) return;
+    // one warp per individual, lane i takes ids i, i + 32, ...: the id loads and the slot stores run in parallel
+    const int lane = threadIdx.x & 31;
+    const int32_t k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (k >= n_ind) return;                                      // warp-uniform
     const int32_t b = offsets[k], e = offsets[k + 1];
     if (b < 0 || e < b || static_cast<int64_t>(e) > n_ids) {
-        meta[k] = make_int2(0, -1);
-        if (prec != nullptr) prec[32ll * k] = -1;
-        counts[k] = 0;
-        atomicMax(err, 5 /* EBIC_ERR_BAD_OFFSETS */);
+        if (lane == 0) {
+            meta[k] = make_int2(0, -1);
+            if (prec != nullptr) prec[32ll * k] = -1;
+            counts[k] = 0;
+            atomicMax(err, 5 /* EBIC_ERR_BAD_OFFSETS */);
+        }
         return;
     }
     const int32_t L = e - b;
+    const int32_t npr = max(L - 1, 0);
     const int64_t slot = (static_cast<int64_t>(b) + 3ll * k) & ~3ll;
     const bool bytes = pids8 != nullptr;
     bool bad = false;
-    int32_t last = 0, last_pair = 0;
-    for (int32_t i = 0; i < L; ++i) {
-        int32_t id = col_ids[b + i];
-        if (id < 0 || id >= cols) {
-            bad = true;
-            id = 0;
-        }
+    auto clean = [&](int32_t id) {                               // an id outside [0, cols) becomes 0 in the slots
+        const bool out = id < 0 || id >= cols;
+        bad |= out;
+        return out ? 0 : id;
+    };
+    auto pair_offset = [&](int32_t a, int32_t c) {
+        return static_cast<int32_t>(static_cast<uint32_t>(a * cols + c) * pair_stride16);
+    };
+    for (int32_t i = lane; i < L; i += 32) {
+        const int32_t id = clean(col_ids[b + i]);
         pids[slot + i] = id;
         if (bytes) pids8[slot + i] = static_cast<uint8_t>(id);
         if (ppair != nullptr && i > 0) {
-            last_pair = last * cols + id;
-            ppair[slot + i - 1] = last_pair;
-            if (i <= kRecPairs) prec[32ll * k + 1 + i] = last_pair;
+            const int32_t po = pair_offset(clean(col_ids[b + i - 1]), id);
+            ppair[slot + i - 1] = po;
+            if (i <= kRecPairs) prec[32ll * k + 1 + i] = po;
         }
-        last = id;
     }
-    for (int32_t i = L; i < ((L + 3) & ~3); ++i) {
+    bad = __any_sync(0xffffffffu, bad);
+    const int32_t last = (L > 0) ? clean(col_ids[b + L - 1]) : 0;
+    for (int32_t i = L + lane; i < ((L + 3) & ~3); i += 32) {
         pids[slot + i] = last;
         if (bytes) pids8[slot + i] = static_cast<uint8_t>(last);
     }
     if (ppair != nullptr) {
-        for (int32_t i = max(L - 1, 0); i < ((max(L - 1, 0) + 3) & ~3); ++i) ppair[slot + i] = last_pair;
-        for (int32_t i = max(L - 1, 0); i < kRecPairs; ++i) prec[32ll * k + 2 + i] = last_pair;
-        prec[32ll * k] = bad ? -1 : L;
-        prec[32ll * k + 1] = static_cast<int32_t>(slot >> 2);
+        const int32_t last_pair = (L > 1) ? pair_offset(clean(col_ids[b + L - 2]), last) : 0;
+        for (int32_t i = npr + lane; i < ((npr + 3) & ~3); i += 32) ppair[slot + i] = last_pair;
+        for (int32_t i = npr + lane; i < kRecPairs; i += 32) prec[32ll * k + 2 + i] = last_pair;
+        if (lane == 0) {
+            prec[32ll * k] = bad ? -1 : L;
+            prec[32ll * k + 1] = static_cast<int32_t>(slot >> 2);
+        }
     }
+    if (lane != 0) return;
     if (bad) {
         meta[k] = make_int2(static_cast<int32_t>(slot >> 2), -1);
         counts[k] = 0;

@@ -19,7 +19,6 @@
 namespace ebic {
 
 constexpr int kRecPairsPb = 30;      // pair indices held in an individual's 128-byte record (see ingest)
-constexpr int kPairbitsWarps = 8;
 constexpr int kPairbitsStepWords = 256;   // words (x32 rows) a warp covers per step: 2 x LDG.128 per lane and pair
 
 struct PairbitsParams {
@@ -27,8 +26,8 @@ struct PairbitsParams {
     int64_t ldw;                     // words per bit column = ld / 32
     int32_t chunk_words;             // words per warp task, multiple of kPairbitsStepWords
     int32_t n_chunks;                // ceil(ldw / chunk_words)
-    const int32_t* prec;             // [n_ind][32] records: L, slot4, 30 pair indices
-    const int32_t* ppair;            // padded pair-index slots (chromosomes with more than 31 columns)
+    const int32_t* prec;             // [n_ind][32] records: L, slot4, 30 pair offsets (pair * ldw / 4, uint32)
+    const int32_t* ppair;            // padded pair-offset slots (chromosomes with more than 31 columns)
     int32_t n_ind;
     unsigned long long* counts;
     unsigned long long* visits;      // executed (row, pair) visits (instrumented) or nullptr
@@ -41,10 +40,65 @@ __device__ __forceinline__ void and4(uint4& a, const uint4& v) {
 }
 __device__ __forceinline__ bool any4(const uint4& a) { return (a.x | a.y | a.z | a.w) != 0u; }
 
-template <bool EARLY_EXIT>
-__global__ void __launch_bounds__(kPairbitsWarps * 32)
+// One step of one chromosome: AND the 256-word slice [base_a, +128 words) / [base_b, +128 words) of each of its
+// bit columns into acc_a / acc_b.  FULL: base_b == base_a + 32 uint4, so the second load of a pair is the
+// first one's address + 512 bytes (an immediate).  Returns the number of pairs visited.
+template <bool EARLY_EXIT, bool FULL>
+__device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_a, const uint4* __restrict__ base_b,
+                                                 uint32_t rec, int32_t n0, int32_t npr, const uint32_t* __restrict__ pp,
+                                                 int lane, uint4& acc_a, uint4& acc_b)
+{
+    int32_t done = 0;
+    int32_t i = 0;
+    for (; i + 4 <= n0; i += 4) {
+        const uint32_t p0 = __shfl_sync(0xffffffffu, rec, i + 2), p1 = __shfl_sync(0xffffffffu, rec, i + 3);
+        const uint32_t p2 = __shfl_sync(0xffffffffu, rec, i + 4), p3 = __shfl_sync(0xffffffffu, rec, i + 5);
+        const uint4 *q0 = base_a + p0, *q1 = base_a + p1, *q2 = base_a + p2, *q3 = base_a + p3;
+        const uint4 *r0 = FULL ? q0 + 32 : base_b + p0, *r1 = FULL ? q1 + 32 : base_b + p1;
+        const uint4 *r2 = FULL ? q2 + 32 : base_b + p2, *r3 = FULL ? q3 + 32 : base_b + p3;
+        const uint4 a0 = __ldg(q0), a1 = __ldg(q1), a2 = __ldg(q2), a3 = __ldg(q3);
+        const uint4 b0 = __ldg(r0), b1 = __ldg(r1), b2 = __ldg(r2), b3 = __ldg(r3);
+        and4(acc_a, a0); and4(acc_a, a1); and4(acc_a, a2); and4(acc_a, a3);
+        and4(acc_b, b0); and4(acc_b, b1); and4(acc_b, b2); and4(acc_b, b3);
+        done += 4;
+        if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) return done;
+    }
+    if (i < n0) {                                                // 1..3 pairs left: the record is padded with
+        const int32_t r = n0 - i;                                // the last pair, so its entries are always valid
+        const uint32_t p0 = __shfl_sync(0xffffffffu, rec, i + 2), p1 = __shfl_sync(0xffffffffu, rec, i + 3);
+        const uint32_t p2 = __shfl_sync(0xffffffffu, rec, min(i + 4, 31));
+        const uint4 *q0 = base_a + p0, *q1 = base_a + p1, *q2 = base_a + p2;
+        const uint4 a0 = __ldg(q0), b0 = __ldg(FULL ? q0 + 32 : base_b + p0);
+        and4(acc_a, a0); and4(acc_b, b0);
+        if (r >= 2) {
+            const uint4 a1 = __ldg(q1), b1 = __ldg(FULL ? q1 + 32 : base_b + p1);
+            and4(acc_a, a1); and4(acc_b, b1);
+        }
+        if (r >= 3) {
+            const uint4 a2 = __ldg(q2), b2 = __ldg(FULL ? q2 + 32 : base_b + p2);
+            and4(acc_a, a2); and4(acc_b, b2);
+        }
+        done += r;
+    }
+    for (int32_t seg = kRecPairsPb; seg < npr; seg += 32) {      // chromosomes with more than 31 columns
+        if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) break;
+        const int32_t n = min(32, npr - seg);
+        const uint32_t mine = __ldg(pp + seg + min(lane, n - 1));
+        for (int32_t j = 0; j < n; ++j) {
+            const uint4* q0 = base_a + __shfl_sync(0xffffffffu, mine, j);
+            const uint4 a0 = __ldg(q0), b0 = __ldg(FULL ? q0 + 32 : base_b + __shfl_sync(0xffffffffu, mine, j));
+            and4(acc_a, a0); and4(acc_b, b0);
+        }
+        done += n;
+    }
+    return done;
+}
+
+template <bool EARLY_EXIT, int NW>
+__global__ void __launch_bounds__(NW * 32)
 fitness_pairbits_kernel(const PairbitsParams p)
 {
+    constexpr int kPairbitsWarps = NW;   // warps (= tasks) per CTA: a CTA's slot is held until its longest chromosome ends
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t task = static_cast<int64_t>(blockIdx.x) * kPairbitsWarps + warp;
     const int64_t g = task / p.n_ind;
@@ -68,68 +122,40 @@ fitness_pairbits_kernel(const PairbitsParams p)
             }
         }
     }
-    const int32_t rec = __ldg(p.prec + 32ll * k + lane);         // the individual: one coalesced 128 B load
-    const int32_t L = __shfl_sync(0xffffffffu, rec, 0);
+    const uint32_t rec = static_cast<uint32_t>(__ldg(p.prec + 32ll * k + lane));   // the individual: one coalesced 128 B load
+    const int32_t L = static_cast<int32_t>(__shfl_sync(0xffffffffu, rec, 0));
     if (L < 2) return;
     const int32_t npr = L - 1;
     const int32_t n0 = min(npr, kRecPairsPb);
-    const int32_t* pp = p.ppair + 4ll * __shfl_sync(0xffffffffu, rec, 1);
+    const uint32_t* pp = reinterpret_cast<const uint32_t*>(p.ppair) + 4ll * __shfl_sync(0xffffffffu, rec, 1);
     const int64_t w_end = min(p.ldw, w_begin + p.chunk_words);
-    const int64_t ldv = p.ldw / 4;                               // bit column length in uint4
+    const uint4* PB4 = reinterpret_cast<const uint4*>(p.PB);
 
     unsigned int cnt = 0;
     unsigned long long executed = 0;
-    for (int64_t w0 = w_begin; w0 < w_end; w0 += kPairbitsStepWords) {
-        const int64_t wa = w0 + lane * 4, wb = wa + 128;
-        const bool va = wa < w_end, vb = wb < w_end;             // ldw is a multiple of 32: a lane's 4 words are all in or all out
-        const uint4* base_a = reinterpret_cast<const uint4*>(p.PB + (va ? wa : w0));
-        const uint4* base_b = reinterpret_cast<const uint4*>(p.PB + (vb ? wb : w0));
-        uint4 acc_a = va ? make_uint4(~0u, ~0u, ~0u, ~0u) : make_uint4(0u, 0u, 0u, 0u);
-        uint4 acc_b = vb ? make_uint4(~0u, ~0u, ~0u, ~0u) : make_uint4(0u, 0u, 0u, 0u);
-        int32_t done = 0;
-        int32_t i = 0;
-        for (; i + 4 <= n0; i += 4) {
-            const int64_t p0 = __shfl_sync(0xffffffffu, rec, i + 2) * ldv, p1 = __shfl_sync(0xffffffffu, rec, i + 3) * ldv;
-            const int64_t p2 = __shfl_sync(0xffffffffu, rec, i + 4) * ldv, p3 = __shfl_sync(0xffffffffu, rec, i + 5) * ldv;
-            const uint4 a0 = __ldg(base_a + p0), a1 = __ldg(base_a + p1), a2 = __ldg(base_a + p2), a3 = __ldg(base_a + p3);
-            const uint4 b0 = __ldg(base_b + p0), b1 = __ldg(base_b + p1), b2 = __ldg(base_b + p2), b3 = __ldg(base_b + p3);
-            and4(acc_a, a0); and4(acc_a, a1); and4(acc_a, a2); and4(acc_a, a3);
-            and4(acc_b, b0); and4(acc_b, b1); and4(acc_b, b2); and4(acc_b, b3);
-            done += 4;
-            if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) goto step_done;
-        }
-        if (i < n0) {                                            // 1..3 pairs left: the record is padded with
-            const int32_t r = n0 - i;                            // the last pair, so its entries are always valid
-            const int64_t p0 = __shfl_sync(0xffffffffu, rec, i + 2) * ldv, p1 = __shfl_sync(0xffffffffu, rec, i + 3) * ldv;
-            const int64_t p2 = __shfl_sync(0xffffffffu, rec, min(i + 4, 31)) * ldv;
-            const uint4 a0 = __ldg(base_a + p0), b0 = __ldg(base_b + p0);
-            and4(acc_a, a0); and4(acc_b, b0);
-            if (r >= 2) {
-                const uint4 a1 = __ldg(base_a + p1), b1 = __ldg(base_b + p1);
-                and4(acc_a, a1); and4(acc_b, b1);
-            }
-            if (r >= 3) {
-                const uint4 a2 = __ldg(base_a + p2), b2 = __ldg(base_b + p2);
-                and4(acc_a, a2); and4(acc_b, b2);
-            }
-            done += r;
-        }
-        for (int32_t seg = kRecPairsPb; seg < npr; seg += 32) {  // chromosomes with more than 31 columns
-            if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) break;
-            const int32_t n = min(32, npr - seg);
-            const int32_t mine = __ldg(pp + seg + min(lane, n - 1));
-            for (int32_t j = 0; j < n; ++j) {
-                const int64_t p0 = __shfl_sync(0xffffffffu, mine, j) * ldv;
-                const uint4 a0 = __ldg(base_a + p0), b0 = __ldg(base_b + p0);
-                and4(acc_a, a0); and4(acc_b, b0);
-            }
-            done += n;
-        }
-    step_done:
+    // Lane l holds words 4l .. 4l+3 of the step's first 128 words (acc_a) and the same words of its second 128
+    // (acc_b).  Record / ppair entries are the bit columns' offsets into PB in uint4 units (< 2^32, host-checked).
+    const int64_t n_full = (w_end - w_begin) / kPairbitsStepWords;
+    const uint4* base = PB4 + (w_begin >> 2) + lane;
+    for (int64_t s = 0; s < n_full; ++s, base += kPairbitsStepWords / 4) {
+        uint4 acc_a = make_uint4(~0u, ~0u, ~0u, ~0u), acc_b = acc_a;
+        const int32_t done = pairbits_step<EARLY_EXIT, true>(base, base, rec, n0, npr, pp, lane, acc_a, acc_b);
         cnt += __popc(acc_a.x) + __popc(acc_a.y) + __popc(acc_a.z) + __popc(acc_a.w);
         cnt += __popc(acc_b.x) + __popc(acc_b.y) + __popc(acc_b.z) + __popc(acc_b.w);
-        executed += static_cast<unsigned long long>(done) *
-                    (min(w_end - w0, static_cast<int64_t>(kPairbitsStepWords)) * 32);
+        executed += static_cast<unsigned long long>(done) * (kPairbitsStepWords * 32);
+    }
+    const int64_t w0 = w_begin + n_full * kPairbitsStepWords;
+    if (w0 < w_end) {                                            // ragged last step of a column (ldw % 256 != 0)
+        const int64_t wa = w0 + lane * 4, wb = wa + 128;
+        const bool va = wa < w_end, vb = wb < w_end;             // ldw % 32 == 0: a lane's 4 words are all in or all out
+        const uint4* base_a = PB4 + ((va ? wa : w0) >> 2);
+        const uint4* base_b = PB4 + ((vb ? wb : w0) >> 2);
+        uint4 acc_a = va ? make_uint4(~0u, ~0u, ~0u, ~0u) : make_uint4(0u, 0u, 0u, 0u);
+        uint4 acc_b = vb ? make_uint4(~0u, ~0u, ~0u, ~0u) : make_uint4(0u, 0u, 0u, 0u);
+        const int32_t done = pairbits_step<EARLY_EXIT, false>(base_a, base_b, rec, n0, npr, pp, lane, acc_a, acc_b);
+        cnt += __popc(acc_a.x) + __popc(acc_a.y) + __popc(acc_a.z) + __popc(acc_a.w);
+        cnt += __popc(acc_b.x) + __popc(acc_b.y) + __popc(acc_b.z) + __popc(acc_b.w);
+        executed += static_cast<unsigned long long>(done) * ((w_end - w0) * 32);
     }
     cnt = __reduce_add_sync(0xffffffffu, cnt);
     if (lane == 0) {

@@ -1,7 +1,7 @@
 """Parity of the CUDA path (through the C ABI, via the thin binding) against the CPU oracle.
 
 Bar: bit-exact (integer counts and bitmasks from exact float32 comparisons; tolerance 0).
-Every fitness kernel (DIRECT, TILED_F32, RANK8) is compared with the oracle on the same seeded
+Every fitness kernel (DIRECT, TILED_F32, RANK8, PAIRBITS) is compared with the oracle on the same seeded
 inputs.  All tests here need the B200.
 """
 from __future__ import annotations
@@ -298,17 +298,18 @@ def test_instrumentation_counts_executed_visits(B):
             assert seen[False] == nominal                          # plain work: executed == nominal
             assert 2 * eb.ld * w.n_ind <= seen[True] <= nominal    # early exit only ever skips columns
         nominal_pairs = eb.ld * int((w.lengths - 1).sum())         # pair kernels count (row, pair) fetches
-        eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)
-        for early_exit in (False, True):
-            eb.set_early_exit(early_exit)
-            eb.set_instrumentation(1)
-            eb.eval_fitness(dev(w.offsets), dev(w.col_ids))
-            seen = eb.info(10)
-            eb.set_instrumentation(0)
-            if early_exit:
-                assert eb.ld * w.n_ind <= seen <= nominal_pairs
-            else:
-                assert seen == nominal_pairs
+        for kern in (B.EBIC_KERNEL_PAIRBITS,):
+            eb.set_kernel(kern)
+            for early_exit in (False, True):
+                eb.set_early_exit(early_exit)
+                eb.set_instrumentation(1)
+                eb.eval_fitness(dev(w.offsets), dev(w.col_ids))
+                seen = eb.info(10)
+                eb.set_instrumentation(0)
+                if early_exit:
+                    assert eb.ld * w.n_ind <= seen <= nominal_pairs, B.KERNEL_NAMES[kern]
+                else:
+                    assert seen == nominal_pairs, B.KERNEL_NAMES[kern]
 
 
 # ------------------------------------------------------------------------- full-size C5 (bench config)
@@ -325,6 +326,8 @@ def test_c5_full_size_sampled(B, oracle_mod):
     with B.Ebic(w.matrix, w.missing_mode) as eb:
         import torch
         results = {}
+        eb.eval_fitness(d_off, d_ids)
+        assert eb.last_kernel == B.EBIC_KERNEL_PAIRBITS          # what AUTO (and bench.py --workload c5) runs
         for kern in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_PAIRBITS):
             eb.set_kernel(kern)
             for early_exit in (False, True):
