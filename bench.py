@@ -40,7 +40,7 @@ from paper_1807_09932_b200 import workloads as W  # noqa: E402
 METRIC = "row_pair_comparisons_per_s"
 UNIT = "comparisons/s"
 N_CHOSEN = 8
-WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4}
+WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4, "p1": 5, "p2": 6, "p3": 7}
 KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4}
 
 
@@ -131,8 +131,26 @@ def measure_l2_gbs(B):
     return B.ebic_probe_read_bandwidth(64 << 20, 40)
 
 
-def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None, cols=None, l2_gbs=None):
-    """each kernel against the data pipe its operands have to come through."""
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fitness kernel, from the committed ncu --set full
+# captures (profiles/r01_fitness_<kernel>_<workload>_ncu_full.txt), full-size workloads only.
+NCU_TRAFFIC_BYTES = {("c4", "pairbits"): 224.34e6 + 4.32e6, ("c5", "pairbits"): 2153.09e6 + 4.58e6,
+                     ("c4", "rank8"): 28.03e6, ("c4", "tiled_f32"): 125.01e6 + 6.72e6}
+
+
+def pair_stats(w):
+    """Input statistics of a population (no method arithmetic): consecutive-pair uses and distinct ordered pairs."""
+    L = w.lengths
+    ids = w.col_ids.astype(np.int64)
+    start = np.zeros(ids.size, dtype=bool)
+    start[w.offsets[:-1][L > 0]] = True                    # position 0 of every chromosome starts no pair
+    nxt = np.flatnonzero(~start)                           # every other position closes the pair (i-1, i)
+    keys = ids[nxt - 1] * w.cols + ids[nxt]
+    return {"uses": int(keys.size), "unique": int(np.unique(keys).size)}
+
+
+def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None, l2_gbs=None,
+             pairs=None, ld=None):
+    """each kernel against the memory its operands have to come through."""
     f_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     pipe_gbs = sm_count * 128 * f_hz / 1e9                 # 128 B / clk / SM: shared memory and L1 share this pipe
     pipe_basis = f"{sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz ({peaks_kind} sm_max_mhz)"
@@ -140,22 +158,36 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
     achieved = visits_executed * bytes_per_visit / kernel_s / 1e9
     bound, peak, basis = "alu", pipe_gbs, pipe_basis
     resource = "shared-memory data pipe (128 B/clk/SM)"
+    extra = {}
     if kernel_name == "rank8":
         resource += " == INT ALU pipe at 0.5 op/visit"
     elif kernel_name == "direct":
         resource = "L1/LSU data pipe (128 B/clk/SM)"
     elif kernel_name == "pairbits":
-        bound, peak = "l2", L2_XBAR_BYTES_PER_CLK * f_hz / 1e9
-        resource = "L2 -> SM read bandwidth (bit columns gathered from L2 with 128-bit loads)"
-        basis = (f"184 L2 slices x 64 B/clk x {f_hz/1e6:.0f} MHz (ncu lts2xbar peak_sustained; a plain L2-resident "
-                 f"streaming read reaches {l2_gbs:.0f} GB/s in this run)" if l2_gbs else
-                 f"184 L2 slices x 64 B/clk x {f_hz/1e6:.0f} MHz (ncu lts2xbar peak_sustained)")
+        # two floors: the gathered bits through L2 -> SM, and the distinct bit columns once from HBM
+        l2_peak = L2_XBAR_BYTES_PER_CLK * f_hz / 1e9
+        hbm_peak = float(peaks["hbm_gbs"])
+        t_l2 = visits_executed * bytes_per_visit / (l2_peak * 1e9)
+        unique_bytes = pairs["unique"] * (ld // 8) if pairs and ld else 0
+        t_hbm = unique_bytes / (hbm_peak * 1e9)
+        extra = {"l2_floor_ms": t_l2 * 1e3, "hbm_floor_ms": t_hbm * 1e3, "pair_uses": pairs["uses"] if pairs else None,
+                 "distinct_pairs": pairs["unique"] if pairs else None, "l2_probe_gbs": l2_gbs}
+        if t_hbm > t_l2:
+            bound, peak, achieved = "hbm", hbm_peak, unique_bytes / kernel_s / 1e9
+            resource = "HBM read of the distinct bit columns the population uses (each once; little re-use)"
+            basis = f"{peaks_kind} hbm_gbs"
+            bytes_per_visit = unique_bytes / max(visits_executed, 1)
+        else:
+            bound, peak = "l2", l2_peak
+            resource = "L2 -> SM read bandwidth (bit columns gathered from L2 with 128-bit loads)"
+            basis = (f"184 L2 slices x 64 B/clk x {f_hz/1e6:.0f} MHz (ncu lts2xbar peak_sustained; a plain L2-resident "
+                     f"streaming read reaches {l2_gbs:.0f} GB/s in this run)" if l2_gbs else
+                     f"184 L2 slices x 64 B/clk x {f_hz/1e6:.0f} MHz (ncu lts2xbar peak_sustained)")
     out = {"bound": bound, "resource": resource, "kernel": "fitness_" + kernel_name, "achieved": achieved,
            "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
            "bytes_per_visit": bytes_per_visit, "visits_per_launch": visits_executed,
            "kernel_ms": kernel_s * 1e3, "peak_basis": basis}
-    if bound == "l2":
-        out["l2_probe_gbs"] = l2_gbs
+    out.update(extra)
     return out
 
 
@@ -291,8 +323,11 @@ def run_gpu(args):
     if rank == 0:
         sm_count = eb.info(7)
         l2_gbs = measure_l2_gbs(B) if kernel_name == "pairbits" else None
+        traffic = args.traffic
+        if traffic is None and args.rows is None and args.n_ind is None:
+            traffic = NCU_TRAFFIC_BYTES.get((args.workload, kernel_name))
         roof = roofline(kernel_name, visits_exec, kernel_ns * 1e-9, peaks, peaks_kind, sm_count,
-                        traffic=args.traffic, cols=w.cols, l2_gbs=l2_gbs)
+                        traffic=traffic, l2_gbs=l2_gbs, pairs=pair_stats(w), ld=eb.ld)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -402,13 +437,14 @@ def run_table(args):
     rows_out = []
     names = args.table_workloads.split(",")
     for name in names:
-        w = W.make_workload(WORKLOADS[name])
+        w = W.make_workload(WORKLOADS[name], rows=args.rows, n_ind=args.n_ind)
         eb = B.Ebic(w.matrix, w.missing_mode)
         d_off, d_ids = torch.from_numpy(w.offsets).cuda(), torch.from_numpy(w.col_ids).cuda()
         d_counts = torch.empty(w.n_ind, dtype=torch.int64, device="cuda")
         chosen = pick_chosen(w)
         d_chosen = torch.from_numpy(chosen).cuda()
         d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
+        pstats = pair_stats(w)
         for kname, ee in (("pairbits", 0), ("pairbits", 1), ("rank8", 0), ("rank8", 1),
                           ("tiled_f32", 0), ("tiled_f32", 1), ("direct", 0)):
             if kname == "direct" and w.comparisons > 2e10:
@@ -458,7 +494,8 @@ def run_table(args):
             except Exception as ex:                              # noqa: BLE001
                 log("graph replay unavailable:", ex)
                 torch.cuda.synchronize()
-            roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7), cols=w.cols, l2_gbs=l2_gbs)
+            roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7), l2_gbs=l2_gbs,
+                            pairs=pstats, ld=eb.ld)
             rows_out.append({"workload": w.cfg.name, "kernel": kname, "early_exit": ee,
                              "executed_over_nominal_visits": visits / nominal,
                              "call_ms_median": statistics.median(call_ms),
@@ -466,7 +503,8 @@ def run_table(args):
                              "comparisons_per_s": w.comparisons / (statistics.median(call_ms) * 1e-3),
                              "comparisons_per_s_kernel": w.comparisons / (kernel_ms * 1e-3),
                              "individuals_rows_per_s": w.n_ind * w.rows / (statistics.median(call_ms) * 1e-3),
-                             "roofline_frac": roof["frac"], "achieved_gbs": roof["achieved"], "tile_rows": eb.info(5),
+                             "roofline_bound": roof["bound"], "roofline_frac": roof["frac"], "achieved_gbs": roof["achieved"],
+                             "tile_rows": eb.info(5),
                              "ctas": eb.info(6)})
             log(json.dumps(rows_out[-1]))
         # extraction (a7): HBM-bound.  Two sources: the pair table's bit columns (default when it exists;

@@ -190,7 +190,7 @@ int launch_tiled(ebic_ctx* ctx, const void* M, int32_t T, const int2* meta, int3
     return cuda_status(cudaGetLastError());
 }
 
-int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, unsigned long long* counts, cudaStream_t stream) {
+int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, int64_t n_ids, unsigned long long* counts, cudaStream_t stream) {
     PairbitsParams p;
     p.PB = ctx->PB;
     p.ldw = ctx->ld / 32;
@@ -208,7 +208,10 @@ int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, unsigned long long* counts, cu
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
     p.n_pairs = ctx->cols * ctx->cols;
     static const int prefetch_dist = env_int("EBIC_PB_PREFETCH", 1);
-    p.prefetch_dist = prefetch_dist;
+    // The prefetch requests EVERY bit column of the next chunk once; that pays only when the population uses
+    // most of the cols^2 columns (n_ids - n_ind = number of pair uses).  A sparse population (wide matrix: P3
+    // uses 14 % of 96,100 columns) gathers straight from HBM instead -- measured 92 % of the HBM peak.
+    p.prefetch_dist = (n_ids - n_ind >= 2ll * p.n_pairs) ? prefetch_dist : 0;
     const int64_t tasks = static_cast<int64_t>(p.n_chunks) * n_ind;
     static const int nw = env_int("EBIC_PB_WARPS", 2);
     const int64_t grid = (tasks + nw - 1) / nw;
@@ -302,7 +305,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         ctx->last_kernel = kernel;
         if (kernel == EBIC_KERNEL_PAIRBITS) {
             if (!ctx->PB) return EBIC_ERR_ARG;
-            st = launch_pairbits(ctx, n, counts, stream);
+            st = launch_pairbits(ctx, n, n_ids, counts, stream);
         } else if (kernel == EBIC_KERNEL_RANK8) {
             const int32_t T = tile_rows_r8(ctx, n);
             if (T <= 0) return EBIC_ERR_ARG;

@@ -66,6 +66,19 @@ CONFIGS: Tuple[WorkloadConfig, ...] = (
                    MISSING_ON, 4_096, (2, 16)),
 )
 
+# stand-ins with the shapes of the paper's own datasets (Table 1, lines
+# 73-75: GDS1490 12,483 x 150, GSE65194 54,675 x 178, GSE84493 436,444 x 310) and its typical population
+# (1,600).  Wider than 127 columns: no rank tiles; a float tile of all columns no longer
+# double-buffers in shared memory at 310 columns.  `make_workload(5..7)`; not BASELINE.json configs.
+PAPER_SHAPES: Tuple[WorkloadConfig, ...] = (
+    WorkloadConfig(5, "P1-GDS1490-shaped", 12_483, 150, "normal", 5, (100, 500), (4, 10), 0.0,
+                   MISSING_OFF, 1_600, (2, 20)),
+    WorkloadConfig(6, "P2-GSE65194-shaped", 54_675, 178, "normal", 10, (200, 2_000), (4, 10), 0.01,
+                   MISSING_ON, 1_600, (2, 20)),
+    WorkloadConfig(7, "P3-GSE84493-shaped", 436_444, 310, "beta", 20, (500, 5_000), (4, 10), 0.01,
+                   MISSING_ON, 1_600, (2, 20)),
+)
+
 
 @dataclass
 class Bicluster:
@@ -137,8 +150,9 @@ def make_population(rng: np.random.Generator, cols: int, n_ind: int, len_range: 
 
 
 def make_workload(index: int, rows: Optional[int] = None, n_ind: Optional[int] = None) -> Workload:
-    """Build workload C(index+1).  `rows` / `n_ind` shrink it (same recipe) for parity tests."""
-    cfg = CONFIGS[index]
+    """Build workload C(index+1) (index 0..4) or a paper-shaped stand-in (index 5..7).  `rows` / `n_ind`
+    resize it (same recipe) for parity tests."""
+    cfg = (CONFIGS + PAPER_SHAPES)[index]
     rows = int(cfg.rows if rows is None else rows)
     n_ind = int(cfg.n_ind if n_ind is None else n_ind)
     cols = cfg.cols

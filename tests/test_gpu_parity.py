@@ -157,6 +157,16 @@ def test_workload_c5_scaled(B, oracle_mod):
     check_all(B, oracle_mod, w.matrix, w.missing_mode, w.offsets, w.col_ids, np.array(chosen, np.int32))
 
 
+@pytest.mark.parametrize("index,rows,n_ind", [(5, None, 1_600), (6, None, 400), (7, 40_001, 300)])
+def test_paper_shaped_workloads(B, oracle_mod, index, rows, n_ind):
+    """150 / 178 / 310 columns (Table 1 shapes): no rank tiles, at 310 columns
+    no float tile either; every kernel that applies, and both extraction sources, against the oracle.  P1 at
+    full size; P2 with a quarter of the population and P3 at 40,001 rows to keep the oracle to seconds."""
+    w = W.make_workload(index, rows=rows, n_ind=n_ind)
+    chosen = [k for k, _ in w.planted_individuals][:6] + [w.n_ind - 1]
+    check_all(B, oracle_mod, w.matrix, w.missing_mode, w.offsets, w.col_ids, np.array(chosen, np.int32))
+
+
 def test_planted_recovery_on_gpu(B):
     w = W.make_workload(0)
     with B.Ebic(w.matrix, w.missing_mode) as eb:

@@ -45,3 +45,11 @@ def test_scaled_down_variant_keeps_recipe():
     w = W.make_workload(4, rows=5000, n_ind=100)
     assert w.matrix.shape == (5000, 32) and w.n_ind == 100
     assert len(w.planted) == 50 and all(p.rows.size >= 2 for p in w.planted)
+
+
+def test_paper_shaped_configs():
+    """PAPER.md Table 1 (lines 73-75): the three dataset shapes; population 1,600."""
+    assert [(c.index, c.rows, c.cols, c.n_ind) for c in W.PAPER_SHAPES] == [
+        (5, 12_483, 150, 1_600), (6, 54_675, 178, 1_600), (7, 436_444, 310, 1_600)]
+    w = W.make_workload(5, rows=2_000, n_ind=50)
+    assert w.matrix.shape == (2_000, 150) and w.n_ind == 50 and w.col_ids.max() < 150
