@@ -169,6 +169,10 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
         hbm_peak = float(peaks["hbm_gbs"])
         t_l2 = visits_executed * bytes_per_visit / (l2_peak * 1e9)
         unique_bytes = pairs["unique"] * (ld // 8) if pairs and ld else 0
+        if pairs and ld and pairs["uses"]:
+            # early exit skips whole 8,192-row steps of the remaining columns: count only the executed share, so
+            # that skipping work can never push the fraction above 1
+            unique_bytes *= min(1.0, visits_executed / (pairs["uses"] * ld))
         t_hbm = unique_bytes / (hbm_peak * 1e9)
         extra = {"l2_floor_ms": t_l2 * 1e3, "hbm_floor_ms": t_hbm * 1e3, "pair_uses": pairs["uses"] if pairs else None,
                  "distinct_pairs": pairs["unique"] if pairs else None, "l2_probe_gbs": l2_gbs}
