@@ -43,13 +43,40 @@ __device__ __forceinline__ bool any4(const uint4& a) { return (a.x | a.y | a.z |
 // One step of one chromosome: AND the 256-word slice [base_a, +128 words) / [base_b, +128 words) of each of its
 // bit columns into acc_a / acc_b.  FULL: base_b == base_a + 32 uint4, so the second load of a pair is the
 // first one's address + 512 bytes (an immediate).  Returns the number of pairs visited.
-template <bool EARLY_EXIT, bool FULL>
+template <bool EARLY_EXIT, bool FULL, bool SMEM = false>
 __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_a, const uint4* __restrict__ base_b,
                                                  uint32_t rec, int32_t n0, int32_t npr, const uint32_t* __restrict__ pp,
-                                                 int lane, uint4& acc_a, uint4& acc_b)
+                                                 int lane, uint4& acc_a, uint4& acc_b, uint32_t ring = 0)
 {
     int32_t done = 0;
     int32_t i = 0;
+    if (FULL && SMEM) {
+        // 8 pairs per round: four land in registers (LDG.128), four in this lane's 16-byte cells of the warp's
+        // 4 KB shared-memory ring (LDGSTS) -- twice the bytes in flight per warp for the same registers.
+        for (; i + 8 <= n0; i += 8) {
+            const uint4* q[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) q[j] = base_a + __shfl_sync(0xffffffffu, rec, i + 2 + j);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                cp_async16(ring + j * 1024 + lane * 16, q[4 + j]);
+                cp_async16(ring + j * 1024 + 512 + lane * 16, q[4 + j] + 32);
+            }
+            cp_async_commit();
+            const uint4 a0 = __ldg(q[0]), a1 = __ldg(q[1]), a2 = __ldg(q[2]), a3 = __ldg(q[3]);
+            const uint4 b0 = __ldg(q[0] + 32), b1 = __ldg(q[1] + 32), b2 = __ldg(q[2] + 32), b3 = __ldg(q[3] + 32);
+            and4(acc_a, a0); and4(acc_a, a1); and4(acc_a, a2); and4(acc_a, a3);
+            and4(acc_b, b0); and4(acc_b, b1); and4(acc_b, b2); and4(acc_b, b3);
+            cp_async_wait_all();
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint4 a = lds128(ring + j * 1024 + lane * 16), b = lds128(ring + j * 1024 + 512 + lane * 16);
+                and4(acc_a, a); and4(acc_b, b);
+            }
+            done += 8;
+            if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) return done;
+        }
+    }
     for (; i + 4 <= n0; i += 4) {
         const uint32_t p0 = __shfl_sync(0xffffffffu, rec, i + 2), p1 = __shfl_sync(0xffffffffu, rec, i + 3);
         const uint32_t p2 = __shfl_sync(0xffffffffu, rec, i + 4), p3 = __shfl_sync(0xffffffffu, rec, i + 5);
@@ -94,10 +121,11 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
     return done;
 }
 
-template <bool EARLY_EXIT, int NW>
+template <bool EARLY_EXIT, int NW, bool SMEM = false>
 __global__ void __launch_bounds__(NW * 32)
 fitness_pairbits_kernel(const PairbitsParams p)
 {
+    extern __shared__ __align__(16) unsigned char pb_ring[];     // SMEM: NW x 4 KB landing ring
     constexpr int kPairbitsWarps = NW;   // warps (= tasks) per CTA: a CTA's slot is held until its longest chromosome ends
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t task = static_cast<int64_t>(blockIdx.x) * kPairbitsWarps + warp;
@@ -139,7 +167,8 @@ fitness_pairbits_kernel(const PairbitsParams p)
     const uint4* base = PB4 + (w_begin >> 2) + lane;
     for (int64_t s = 0; s < n_full; ++s, base += kPairbitsStepWords / 4) {
         uint4 acc_a = make_uint4(~0u, ~0u, ~0u, ~0u), acc_b = acc_a;
-        const int32_t done = pairbits_step<EARLY_EXIT, true>(base, base, rec, n0, npr, pp, lane, acc_a, acc_b);
+        const int32_t done = pairbits_step<EARLY_EXIT, true, SMEM>(base, base, rec, n0, npr, pp, lane, acc_a, acc_b,
+                                                                   SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u);
         cnt += __popc(acc_a.x) + __popc(acc_a.y) + __popc(acc_a.z) + __popc(acc_a.w);
         cnt += __popc(acc_b.x) + __popc(acc_b.y) + __popc(acc_b.z) + __popc(acc_b.w);
         executed += static_cast<unsigned long long>(done) * (kPairbitsStepWords * 32);
