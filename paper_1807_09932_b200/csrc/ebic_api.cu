@@ -224,7 +224,7 @@ int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, int64_t n_ids, unsigned long l
         if (ctx->early_exit) fitness_pairbits_kernel<true, NW><<<g, NW * 32, 0, stream>>>(p);  \
         else fitness_pairbits_kernel<false, NW><<<g, NW * 32, 0, stream>>>(p);                 \
     } while (0)
-    static const int use_smem = env_int("EBIC_PB_SMEM", 0);
+    static const int use_smem = env_int("EBIC_PB_SMEM", 1);
     if (use_smem && nw == 2) {
         if (ctx->early_exit) fitness_pairbits_kernel<true, 2, true><<<g, 64, 8192, stream>>>(p);
         else fitness_pairbits_kernel<false, 2, true><<<g, 64, 8192, stream>>>(p);

@@ -64,6 +64,13 @@ __device__ __forceinline__ void bulk_prefetch_l2(const void* gmem_src, uint32_t 
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
 }
 
+// 128-bit read-only global load that keeps its place among the other asm statements (SASS: LDG.E.128.CONSTANT).
+__device__ __forceinline__ uint4 ldg128_ordered(const void* p) {
+    uint4 v;
+    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+
 // 16-byte asynchronous copy global -> shared that bypasses registers and L1 (SASS: LDGSTS.E.BYPASS.128), and its
 // group fence.  A thread that only reads back what it copied itself needs no barrier after the wait.
 __device__ __forceinline__ void cp_async16(uint32_t smem_dst, const void* gmem_src) {

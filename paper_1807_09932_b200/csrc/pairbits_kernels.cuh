@@ -57,14 +57,16 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
             const uint4* q[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) q[j] = base_a + __shfl_sync(0xffffffffu, rec, i + 2 + j);
+            // all sixteen requests leave before anything waits: eight register loads, then eight LDGSTS
+            const uint4 a0 = ldg128_ordered(q[0]), a1 = ldg128_ordered(q[1]), a2 = ldg128_ordered(q[2]), a3 = ldg128_ordered(q[3]);
+            const uint4 b0 = ldg128_ordered(q[0] + 32), b1 = ldg128_ordered(q[1] + 32);
+            const uint4 b2 = ldg128_ordered(q[2] + 32), b3 = ldg128_ordered(q[3] + 32);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 cp_async16(ring + j * 1024 + lane * 16, q[4 + j]);
                 cp_async16(ring + j * 1024 + 512 + lane * 16, q[4 + j] + 32);
             }
             cp_async_commit();
-            const uint4 a0 = __ldg(q[0]), a1 = __ldg(q[1]), a2 = __ldg(q[2]), a3 = __ldg(q[3]);
-            const uint4 b0 = __ldg(q[0] + 32), b1 = __ldg(q[1] + 32), b2 = __ldg(q[2] + 32), b3 = __ldg(q[3] + 32);
             and4(acc_a, a0); and4(acc_a, a1); and4(acc_a, a2); and4(acc_a, a3);
             and4(acc_b, b0); and4(acc_b, b1); and4(acc_b, b2); and4(acc_b, b3);
             cp_async_wait_all();
@@ -74,6 +76,11 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
                 and4(acc_a, a); and4(acc_b, b);
             }
             done += 8;
+            // Ring reuse: the next round's LDGSTS must not be issued before this round's LDS data has arrived.
+            // `ring` is made to depend on all eight accumulator words (each holds the result of four of the LDS),
+            // so the in-order issue + scoreboard of the warp orders them; no instruction is emitted.
+            asm volatile("" : "+r"(ring) : "r"(acc_a.x), "r"(acc_a.y), "r"(acc_a.z), "r"(acc_a.w),
+                                           "r"(acc_b.x), "r"(acc_b.y), "r"(acc_b.z), "r"(acc_b.w) : "memory");
             if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) return done;
         }
     }
