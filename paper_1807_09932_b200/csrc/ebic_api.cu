@@ -190,15 +190,26 @@ int launch_tiled(ebic_ctx* ctx, const void* M, int32_t T, const int2* meta, int3
     return cuda_status(cudaGetLastError());
 }
 
+// Words of a bit column per PAIRBITS warp task: about `tasks_per_slot` tasks per resident warp slot (32 / SM),
+// 256..2048 words (8,192..65,536 rows) per task.
+int64_t pairbits_chunk_words(const ebic_ctx* ctx, int32_t n_ind) {
+    static const int64_t tasks_per_slot = env_int("EBIC_PB_TASKS_PER_SLOT", 8);
+    const int64_t want_tasks = tasks_per_slot * ctx->sm_count * 32;
+    const int64_t cw = (ctx->ld / 32) * n_ind / want_tasks;
+    return std::max<int64_t>(kPairbitsStepWords, std::min<int64_t>(8 * kPairbitsStepWords, cw / kPairbitsStepWords * kPairbitsStepWords));
+}
+// The L2 prefetches request EVERY bit column once; that pays only when the population uses most of the cols^2
+// columns (n_ids - n_ind = number of pair uses).  A sparse population (wide matrix: P3 uses 14 % of 96,100
+// columns) gathers straight from HBM instead -- measured 87 % of the HBM peak.
+bool pairbits_dense(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
+    return n_ids - n_ind >= 2ll * ctx->cols * ctx->cols;
+}
+
 int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, int64_t n_ids, unsigned long long* counts, cudaStream_t stream) {
     PairbitsParams p;
     p.PB = ctx->PB;
     p.ldw = ctx->ld / 32;
-    // about `tasks_per_slot` tasks per resident warp slot (4 CTAs / SM), 256..2048 words (8,192..65,536 rows) per task
-    static const int64_t tasks_per_slot = env_int("EBIC_PB_TASKS_PER_SLOT", 8);
-    const int64_t want_tasks = tasks_per_slot * ctx->sm_count * 32;
-    int64_t cw = p.ldw * n_ind / want_tasks;
-    cw = std::max<int64_t>(kPairbitsStepWords, std::min<int64_t>(8 * kPairbitsStepWords, cw / kPairbitsStepWords * kPairbitsStepWords));
+    const int64_t cw = pairbits_chunk_words(ctx, n_ind);
     p.chunk_words = static_cast<int32_t>(cw);
     p.n_chunks = static_cast<int32_t>((p.ldw + cw - 1) / cw);
     p.prec = ctx->prec;
@@ -208,10 +219,7 @@ int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, int64_t n_ids, unsigned long l
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
     p.n_pairs = ctx->cols * ctx->cols;
     static const int prefetch_dist = env_int("EBIC_PB_PREFETCH", 1);
-    // The prefetch requests EVERY bit column of the next chunk once; that pays only when the population uses
-    // most of the cols^2 columns (n_ids - n_ind = number of pair uses).  A sparse population (wide matrix: P3
-    // uses 14 % of 96,100 columns) gathers straight from HBM instead -- measured 92 % of the HBM peak.
-    p.prefetch_dist = (n_ids - n_ind >= 2ll * p.n_pairs) ? prefetch_dist : 0;
+    p.prefetch_dist = pairbits_dense(ctx, n_ind, n_ids) ? prefetch_dist : 0;
     const int64_t tasks = static_cast<int64_t>(p.n_chunks) * n_ind;
     static const int nw = env_int("EBIC_PB_WARPS", 2);
     const int64_t grid = (tasks + nw - 1) / nw;
@@ -288,11 +296,21 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         if (st) return st;
     }
 
+    // Experiment, OFF by default (EBIC_PB_WARM=3 turns it on): when PAIRBITS runs next on a dense population the
+    // ingest warps also request the first `warm` chunks of every bit column from HBM.  Measured on C4: the
+    // event-bracketed fitness kernel drops 63.4 -> 61.0 us but the step does not (83.2 -> 83.6..84.3 us): the
+    // cold-start HBM fetch only moves from inside the kernel's bracket to the ingest kernel before it.  It would
+    // raise the reported L2 fraction (0.59 -> 0.61) without making an evaluation faster, so it stays off.
+    static const int warm_chunks = env_int("EBIC_PB_WARM", 0);
+    uint32_t warm_bytes = 0;
+    if (warm_chunks > 0 && resolve_kernel(ctx, std::min<int32_t>(kMaxIndPerLaunch, n_ind)) == EBIC_KERNEL_PAIRBITS &&
+        pairbits_dense(ctx, n_ind, n_ids))
+        warm_bytes = static_cast<uint32_t>(std::min<int64_t>(warm_chunks * pairbits_chunk_words(ctx, n_ind), ctx->ld / 32) * 4);
     ingest_population_kernel<<<(n_ind + 7) / 8, 256, 0, stream>>>(
         offsets, col_ids, n_ind, n_ids, ctx->cols, ctx->rows, ctx->missing_mode == EBIC_MISSING_ON,
         ctx->nonmissing, ctx->meta, ctx->pids, ctx->cols <= 256 ? ctx->pids8 : nullptr,
         ctx->PB ? ctx->ppair : nullptr, ctx->PB ? ctx->prec : nullptr, static_cast<uint32_t>(ctx->ld / 128), counts,
-        ctx->d_err);
+        ctx->d_err, ctx->PB, ctx->cols * ctx->cols, warm_bytes);
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());
 

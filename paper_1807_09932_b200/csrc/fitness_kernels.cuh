@@ -37,12 +37,23 @@ ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __r
                          const unsigned long long* __restrict__ nonmissing, int2* __restrict__ meta,
                          int32_t* __restrict__ pids, uint8_t* __restrict__ pids8, int32_t* __restrict__ ppair,
                          int32_t* __restrict__ prec, uint32_t pair_stride16,
-                         unsigned long long* __restrict__ counts, int32_t* __restrict__ err)
+                         unsigned long long* __restrict__ counts, int32_t* __restrict__ err,
+                         const uint32_t* __restrict__ warm_PB, int32_t warm_pairs, uint32_t warm_bytes)
 {
     // one warp per individual, lane i takes ids i, i + 32, ...: the id loads and the slot stores run in parallel
     const int lane = threadIdx.x & 31;
     const int32_t k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (k >= n_ind) return;                                      // warp-uniform
+    if (warm_bytes != 0) {
+        // Cold start of the PAIRBITS kernel that follows on the stream: the first rows of every bit column (the
+        // chunks its first wave of CTAs will gather) are requested from HBM now, one slice of columns per warp.
+        const int32_t per = (warm_pairs + n_ind - 1) / n_ind;
+        for (int32_t q = lane; q < per; q += 32) {
+            const int64_t pair = static_cast<int64_t>(k) * per + q;
+            if (pair < warm_pairs)
+                bulk_prefetch_l2(reinterpret_cast<const uint4*>(warm_PB) + pair * pair_stride16, warm_bytes);
+        }
+    }
     const int32_t b = offsets[k], e = offsets[k + 1];
     if (b < 0 || e < b || static_cast<int64_t>(e) > n_ids) {
         if (lane == 0) {
