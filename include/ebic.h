@@ -43,7 +43,8 @@ enum {
     EBIC_ERR_OOM = 2,         /* cudaMalloc failed                                                */
     EBIC_ERR_CUDA = 3,        /* any other CUDA runtime error (no device, launch failure, ...)    */
     EBIC_ERR_BAD_COLUMN = 4,  /* a column id outside [0, cols) was found on the device            */
-    EBIC_ERR_BAD_OFFSETS = 5  /* offsets[k] < 0, offsets[k+1] < offsets[k] or offsets[k+1] > n_ids */
+    EBIC_ERR_BAD_OFFSETS = 5, /* offsets[k] < 0, offsets[k+1] < offsets[k] or offsets[k+1] > n_ids */
+    EBIC_ERR_IO = 6           /* ebic_read_delimited: cannot open / not a delimited matrix / ragged line */
 };
 enum { EBIC_MISSING_OFF = 0, EBIC_MISSING_ON = 1 };
 
@@ -70,6 +71,16 @@ enum {
  */
 int ebic_create(const float *matrix, int64_t rows, int32_t cols, int32_t missing_mode,
                 ebic_ctx **out);
+
+/*
+ * The same loader for matrices that mark missing cells with a numeric value instead of NaN (PAPER.md
+ * line 60: "a predefined numeric value, e.g. 0 or 999"): every element that compares equal to `sentinel`
+ * (float ==, so a sentinel of 0 also matches -0) becomes NaN while the matrix is transposed; elements
+ * that already are NaN stay missing.  `sentinel` must not be NaN (EBIC_ERR_ARG).  Everything else as
+ * ebic_create; with missing_mode OFF the mapped cells still fail every L >= 2 comparison (R4).
+ */
+int ebic_create_sentinel(const float *matrix, int64_t rows, int32_t cols, int32_t missing_mode,
+                         float sentinel, ebic_ctx **out);
 
 /* Frees everything the context owns.  NULL is allowed. */
 int ebic_destroy(ebic_ctx *ctx);
@@ -170,6 +181,27 @@ int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);
  *   dst_bytes must equal the product's size.
  */
 int ebic_debug_read(const ebic_ctx *ctx, int32_t what, void *dst, int64_t dst_bytes);
+
+/*
+ * Input files ("The data values might be separated by either comma, tabulator or
+ * semicolon. An upper left header is not required, which simplifies porting files between EBIC and R").
+ * Reads a text matrix on the HOST: line 1 = column names, every later line = a row name followed by the
+ * row's values.  `delimiter` is ',', '\t', ';' or 0 = detect from line 1 (a tab wins over a semicolon
+ * over a comma).  The upper-left corner label may be present (header has as many fields as a data line)
+ * or absent (one fewer, as R's write.table writes it).  Names are skipped and must not contain the
+ * delimiter; values are parsed with strtof (correctly rounded to float32; inf, exponents accepted), may
+ * be double-quoted, and an empty field, NA, N/A, NaN, nan or null is a missing cell = NaN (a numeric
+ * marker such as 999 is handled by ebic_create_sentinel).  "\n" and "\r\n" line ends; blank lines skipped.
+ *   *matrix  receives a malloc'ed ROW-MAJOR float32 [*rows][*cols] ready for ebic_create; the caller
+ *            releases it with ebic_free_host.
+ * Errors: EBIC_ERR_ARG (NULL, unknown delimiter), EBIC_ERR_IO (cannot open, fewer than two lines, no
+ * delimiter found, header/data field counts disagree, ragged line, a field that is not a number),
+ * EBIC_ERR_OOM.  On error *matrix == NULL.  No CUDA call is made.
+ */
+int ebic_read_delimited(const char *path, char delimiter, float **matrix, int64_t *rows, int32_t *cols);
+
+/* Releases a buffer returned by ebic_read_delimited.  NULL is allowed. */
+void ebic_free_host(void *p);
 
 /*
  * Measurement utility (not a step of the path): read bandwidth, in GB/s, that all SMs together get

@@ -23,6 +23,7 @@ EBIC_ERR_OOM = 2
 EBIC_ERR_CUDA = 3
 EBIC_ERR_BAD_COLUMN = 4
 EBIC_ERR_BAD_OFFSETS = 5
+EBIC_ERR_IO = 6
 EBIC_MISSING_OFF = 0
 EBIC_MISSING_ON = 1
 EBIC_KERNEL_AUTO = 0
@@ -38,6 +39,7 @@ LIB_PATH = Path(__file__).resolve().parent / "libebic.so"
 _vp, _i32, _i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
 SYMBOLS = {
     "ebic_create": (ctypes.c_int, [_vp, _i64, _i32, _i32, ctypes.POINTER(_vp)]),
+    "ebic_create_sentinel": (ctypes.c_int, [_vp, _i64, _i32, _i32, ctypes.c_float, ctypes.POINTER(_vp)]),
     "ebic_destroy": (ctypes.c_int, [_vp]),
     "ebic_eval_fitness": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _vp]),
     "ebic_extract_rows": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _i32, _vp, _vp, _vp]),
@@ -50,6 +52,9 @@ SYMBOLS = {
     "ebic_set_instrumentation": (ctypes.c_int, [_vp, _i32]),
     "ebic_get_info": (_i64, [_vp, _i32]),
     "ebic_debug_read": (ctypes.c_int, [_vp, _i32, _vp, _i64]),
+    "ebic_read_delimited": (ctypes.c_int, [ctypes.c_char_p, ctypes.c_char, ctypes.POINTER(ctypes.POINTER(ctypes.c_float)),
+                                           ctypes.POINTER(_i64), ctypes.POINTER(_i32)]),
+    "ebic_free_host": (None, [_vp]),
     "ebic_probe_read_bandwidth": (ctypes.c_int, [_i64, _i32, ctypes.POINTER(ctypes.c_double)]),
     "ebic_strerror": (ctypes.c_char_p, [ctypes.c_int]),
 }
@@ -92,6 +97,14 @@ def ebic_create(matrix_ptr: int, rows: int, cols: int, missing_mode: int) -> int
     st = load_library().ebic_create(matrix_ptr, rows, cols, missing_mode, ctypes.byref(out))
     if st != EBIC_OK:
         raise EbicError(st, "ebic_create")
+    return out.value
+
+
+def ebic_create_sentinel(matrix_ptr: int, rows: int, cols: int, missing_mode: int, sentinel: float) -> int:
+    out = _vp()
+    st = load_library().ebic_create_sentinel(matrix_ptr, rows, cols, missing_mode, float(sentinel), ctypes.byref(out))
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_create_sentinel")
     return out.value
 
 
@@ -155,6 +168,21 @@ def ebic_debug_read(ctx, what: int, dst: np.ndarray) -> None:
         raise EbicError(st, "ebic_debug_read")
 
 
+def ebic_read_delimited(path: str, delimiter: str = "") -> np.ndarray:
+    """ebic_read_delimited: float32 [rows][cols] copied out of the library's buffer (which is then freed)."""
+    lib = load_library()
+    m = ctypes.POINTER(ctypes.c_float)()
+    rows, cols = _i64(0), _i32(0)
+    d = delimiter.encode() if delimiter else b"\0"
+    st = lib.ebic_read_delimited(str(path).encode(), d, ctypes.byref(m), ctypes.byref(rows), ctypes.byref(cols))
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_read_delimited")
+    try:
+        return np.ctypeslib.as_array(m, shape=(rows.value, cols.value)).copy()
+    finally:
+        lib.ebic_free_host(ctypes.cast(m, _vp))
+
+
 # ---------------------------------------------------------------- convenience wrapper
 def ebic_probe_read_bandwidth(buffer_bytes: int, reps: int) -> float:
     out = ctypes.c_double(0.0)
@@ -198,7 +226,8 @@ def _stream_handle(stream) -> int:
 class Ebic:
     """One loaded matrix (ebic_ctx).  matrix: float32 [rows][cols], torch CUDA/CPU tensor or numpy."""
 
-    def __init__(self, matrix, missing_mode: int):
+    def __init__(self, matrix, missing_mode: int, sentinel: Optional[float] = None):
+        """`sentinel`: numeric value that marks missing cells in `matrix` (ebic_create_sentinel); None = NaN only."""
         torch = _require_cuda()
         load_library()
         if isinstance(matrix, np.ndarray):
@@ -213,7 +242,10 @@ class Ebic:
                 torch.cuda.current_stream().synchronize()      # ebic_create runs on the legacy stream
         self.rows, self.cols = int(matrix.shape[0]), int(matrix.shape[1])
         self.missing_mode = int(missing_mode)
-        self._ctx = ebic_create(_ptr(matrix), self.rows, self.cols, self.missing_mode)
+        if sentinel is None:
+            self._ctx = ebic_create(_ptr(matrix), self.rows, self.cols, self.missing_mode)
+        else:
+            self._ctx = ebic_create_sentinel(_ptr(matrix), self.rows, self.cols, self.missing_mode, sentinel)
         self.mask_words = ebic_mask_words(self._ctx)
 
     # -- lifetime

@@ -15,7 +15,7 @@ from pathlib import Path
 CSRC = Path(__file__).resolve().parent
 PKG = CSRC.parent
 LIB = PKG / "libebic.so"
-SOURCES = [CSRC / "ebic_api.cu"]
+SOURCES = [CSRC / "ebic_api.cu", CSRC / "ebic_reader.cu"]
 HEADERS = sorted(CSRC.glob("*.cuh")) + [PKG.parent / "include" / "ebic.h"]
 
 NVCC_FLAGS = [

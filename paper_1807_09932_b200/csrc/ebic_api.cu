@@ -400,10 +400,11 @@ int stage_in(ebic_ctx* ctx, int slot, const void* host, int64_t bytes, cudaStrea
 
 extern "C" {
 
-int ebic_create(const float* matrix, int64_t rows, int32_t cols, int32_t missing_mode, ebic_ctx** out) {
+static int create_impl(const float* matrix, int64_t rows, int32_t cols, int32_t missing_mode, int32_t use_sentinel,
+                       float sentinel, ebic_ctx** out) {
     if (out) *out = nullptr;
     if (!matrix || !out || rows <= 0 || rows > 2147483647ll || cols <= 0 ||
-        (missing_mode != EBIC_MISSING_OFF && missing_mode != EBIC_MISSING_ON))
+        (missing_mode != EBIC_MISSING_OFF && missing_mode != EBIC_MISSING_ON) || (use_sentinel && sentinel != sentinel))
         return EBIC_ERR_ARG;
     ebic_ctx* ctx = new (std::nothrow) ebic_ctx();
     if (!ctx) return EBIC_ERR_OOM;
@@ -431,7 +432,7 @@ int ebic_create(const float* matrix, int64_t rows, int32_t cols, int32_t missing
         const unsigned gy = static_cast<unsigned>(std::min<int64_t>((cols + 31) / 32, 65535));
         if (is_device_pointer(matrix)) {
             const dim3 grid(static_cast<unsigned>((rows + 31) / 32), gy);
-            transpose_pad_kernel<<<grid, tb>>>(matrix, ctx->Mc, 0, rows, cols, ctx->ld);
+            transpose_pad_kernel<<<grid, tb>>>(matrix, ctx->Mc, 0, rows, cols, ctx->ld, use_sentinel, sentinel);
             ctx->launches++;
             if ((st = cuda_status(cudaGetLastError()))) break;
         } else {
@@ -441,7 +442,7 @@ int ebic_create(const float* matrix, int64_t rows, int32_t cols, int32_t missing
                 const int64_t nr = std::min<int64_t>(chunk_rows, rows - r0);
                 if ((st = cuda_status(cudaMemcpy(staging, matrix + r0 * cols, static_cast<size_t>(nr) * cols * 4, cudaMemcpyHostToDevice)))) break;
                 const dim3 grid(static_cast<unsigned>((nr + 31) / 32), gy);
-                transpose_pad_kernel<<<grid, tb>>>(staging, ctx->Mc, r0, nr, cols, ctx->ld);
+                transpose_pad_kernel<<<grid, tb>>>(staging, ctx->Mc, r0, nr, cols, ctx->ld, use_sentinel, sentinel);
                 ctx->launches++;
                 st = cuda_status(cudaGetLastError());
             }
@@ -493,6 +494,15 @@ int ebic_create(const float* matrix, int64_t rows, int32_t cols, int32_t missing
     }
     *out = ctx;
     return EBIC_OK;
+}
+
+int ebic_create(const float* matrix, int64_t rows, int32_t cols, int32_t missing_mode, ebic_ctx** out) {
+    return create_impl(matrix, rows, cols, missing_mode, 0, 0.0f, out);
+}
+
+int ebic_create_sentinel(const float* matrix, int64_t rows, int32_t cols, int32_t missing_mode, float sentinel,
+                         ebic_ctx** out) {
+    return create_impl(matrix, rows, cols, missing_mode, 1, sentinel, out);
 }
 
 int ebic_destroy(ebic_ctx* ctx) {
@@ -775,6 +785,7 @@ const char* ebic_strerror(int status) {
         case EBIC_ERR_CUDA: return "CUDA runtime error";
         case EBIC_ERR_BAD_COLUMN: return "column id outside [0, cols) in the population";
         case EBIC_ERR_BAD_OFFSETS: return "bad population offsets or chosen index";
+        case EBIC_ERR_IO: return "cannot read the file as a delimited matrix";
         default: return "unknown status";
     }
 }

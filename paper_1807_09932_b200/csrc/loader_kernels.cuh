@@ -22,7 +22,7 @@ namespace ebic {
 // global row `row0`.  grid.x = ceil(chunk_rows / 32), grid.y = ceil(cols / 32).
 __global__ void __launch_bounds__(256)
 transpose_pad_kernel(const float* __restrict__ src, float* __restrict__ Mc, int64_t row0,
-                     int64_t chunk_rows, int32_t cols, int64_t ld)
+                     int64_t chunk_rows, int32_t cols, int64_t ld, int32_t use_sentinel, float sentinel)
 {
     __shared__ float tile[32][33];
     const int64_t r0 = static_cast<int64_t>(blockIdx.x) * 32;
@@ -31,7 +31,12 @@ transpose_pad_kernel(const float* __restrict__ src, float* __restrict__ Mc, int6
         for (int j = 0; j < 32; j += 8) {
             const int64_t r = r0 + threadIdx.y + j;
             const int32_t c = c0 + threadIdx.x;
-            if (r < chunk_rows && c < cols) tile[threadIdx.y + j][threadIdx.x] = src[r * cols + c];
+            if (r < chunk_rows && c < cols) {
+                // a file marks missing cells with a numeric value (e.g. 0 or 999); here it becomes
+                // NaN, the ABI's missing marker (float ==, so a sentinel of 0 also maps -0)
+                const float v = src[r * cols + c];
+                tile[threadIdx.y + j][threadIdx.x] = (use_sentinel && v == sentinel) ? __uint_as_float(0x7fc00000u) : v;
+            }
         }
         __syncthreads();
 #pragma unroll

@@ -233,6 +233,67 @@ def test_wide_matrix_falls_back(B, oracle_mod):
         check_all(B, oracle_mod, m, ON, off, ids, np.arange(0, 50, 7, dtype=np.int32))
 
 
+@pytest.mark.parametrize("sentinel", [999.0, 0.0, -1.5])
+def test_sentinel_marks_missing(B, oracle_mod, sentinel):
+    """missing cells carry a numeric marker ("e.g. 0 or 999"); ebic_create_sentinel maps it to
+    NaN in the loader.  Expected values: the oracle on the matrix with the marker replaced by NaN (input
+    preparation by numpy, no method arithmetic).  Cells that already are NaN stay missing; a 0 marker also
+    matches -0."""
+    m, off, ids = W.random_case(31, 3_001, 40, 120, (0, 8), 0.0, True, True)   # quantised: many 0.0 / -1.5 cells
+    rng = np.random.default_rng(5)
+    hit = rng.random(m.shape) < 0.03
+    m[hit] = np.float32(sentinel)
+    m[rng.random(m.shape) < 0.01] = np.float32(np.nan)
+    if sentinel == 0.0:
+        m[7, 3] = np.float32(-0.0)
+    as_nan = m.copy()
+    as_nan[m == np.float32(sentinel)] = np.float32(np.nan)
+    for mode in (ON, OFF):
+        st, want = oracle_mod.eval_fitness(as_nan, mode, off, ids)
+        chosen = np.arange(0, 120, 11, dtype=np.int32)
+        _, wm, wc = oracle_mod.extract_rows(as_nan, mode, off, ids, chosen)
+        for src in (m, dev(m)):                                   # host and device input
+            with B.Ebic(src, mode, sentinel=sentinel) as eb:
+                assert (eb.debug_read(1) == B.Ebic(as_nan, mode).debug_read(1)).all()      # NaN bitmask
+                for kern in kernels_for(eb, B):
+                    assert (gpu_counts(eb, B, off, ids, kern) == want).all(), B.KERNEL_NAMES[kern]
+                gm, gc = gpu_masks(eb, off, ids, chosen)
+                assert (gm == wm).all() and (gc == wc).all()
+    with pytest.raises(B.EbicError):
+        B.Ebic(m, ON, sentinel=float("nan"))
+
+
+def test_file_to_counts(B, oracle_mod, tmp_path):
+    """The whole ingest side: semicolon-separated file with R-style header (no corner), 999
+    as the missing marker -> ebic_read_delimited -> ebic_create_sentinel -> counts and masks equal the oracle's on
+    the matrix the file was written from."""
+    w = W.make_workload(1, rows=700, n_ind=150)
+    marked = w.matrix.copy()
+    marked[np.isnan(marked)] = np.float32(999.0)
+    lines = [";".join(f"s{c}" for c in range(w.cols))]
+    lines += [";".join([f"g{r}"] + [repr(float(v)) for v in marked[r]]) for r in range(w.rows)]
+    path = tmp_path / "expr.csv"
+    path.write_text("\n".join(lines) + "\n")
+    m = B.ebic_read_delimited(path)
+    assert m.shape == marked.shape and (m.view(np.uint32) == marked.view(np.uint32)).all()
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    chosen = np.array([k for k, _ in w.planted_individuals][:5], dtype=np.int32)
+    _, wm, wc = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
+    with B.Ebic(m, w.missing_mode, sentinel=999.0) as eb:
+        assert (gpu_counts(eb, B, w.offsets, w.col_ids, B.EBIC_KERNEL_AUTO) == want).all()
+        gm, gc = gpu_masks(eb, w.offsets, w.col_ids, chosen)
+        assert (gm == wm).all() and (gc == wc).all()
+
+
+def test_probe_read_bandwidth(B):
+    """Measurement utility: an L2-resident buffer streams faster than HBM; bad arguments are refused."""
+    l2 = B.ebic_probe_read_bandwidth(64 << 20, 20)
+    hbm = B.ebic_probe_read_bandwidth(2 << 30, 2)
+    assert 2_000 < hbm < 9_000 and l2 > hbm
+    with pytest.raises(B.EbicError):
+        B.ebic_probe_read_bandwidth(1024, 1)
+
+
 def test_empty_calls(B):
     import torch
     m = np.zeros((10, 3), dtype=np.float32)
