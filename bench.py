@@ -149,7 +149,7 @@ def pair_stats(w):
 
 
 def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None, l2_gbs=None,
-             pairs=None, ld=None):
+             pairs=None, ld=None, cols=None):
     """each kernel against the memory its operands have to come through."""
     f_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
     pipe_gbs = sm_count * 128 * f_hz / 1e9                 # 128 B / clk / SM: shared memory and L1 share this pipe
@@ -159,8 +159,20 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
     bound, peak, basis = "alu", pipe_gbs, pipe_basis
     resource = "shared-memory data pipe (128 B/clk/SM)"
     extra = {}
-    if kernel_name == "rank8":
-        resource += " == INT ALU pipe at 0.5 op/visit"
+    if kernel_name in ("rank8", "tiled_f32"):
+        if kernel_name == "rank8":
+            resource += " == INT ALU pipe at 0.5 op/visit"
+        # second floor: the tiles are staged from HBM once per evaluation (tiny populations are bound by that)
+        if ld and cols:
+            hbm_peak = float(peaks["hbm_gbs"])
+            stage_bytes = ld * cols * (1 if kernel_name == "rank8" else 4)
+            t_pipe, t_hbm = visits_executed * bytes_per_visit / (pipe_gbs * 1e9), stage_bytes / (hbm_peak * 1e9)
+            extra = {"pipe_floor_ms": t_pipe * 1e3, "hbm_floor_ms": t_hbm * 1e3}
+            if t_hbm > t_pipe:
+                bound, peak, achieved = "hbm", hbm_peak, stage_bytes / kernel_s / 1e9
+                resource = "HBM read of the matrix tiles (staged once per evaluation; population too small to hide it)"
+                basis = f"{peaks_kind} hbm_gbs"
+                bytes_per_visit = stage_bytes / max(visits_executed, 1)
     elif kernel_name == "direct":
         resource = "L1/LSU data pipe (128 B/clk/SM)"
     elif kernel_name == "pairbits":
@@ -331,7 +343,7 @@ def run_gpu(args):
         if traffic is None and args.rows is None and args.n_ind is None:
             traffic = NCU_TRAFFIC_BYTES.get((args.workload, kernel_name))
         roof = roofline(kernel_name, visits_exec, kernel_ns * 1e-9, peaks, peaks_kind, sm_count,
-                        traffic=traffic, l2_gbs=l2_gbs, pairs=pair_stats(w), ld=eb.ld)
+                        traffic=traffic, l2_gbs=l2_gbs, pairs=pair_stats(w), ld=eb.ld, cols=w.cols)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -499,7 +511,7 @@ def run_table(args):
                 log("graph replay unavailable:", ex)
                 torch.cuda.synchronize()
             roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7), l2_gbs=l2_gbs,
-                            pairs=pstats, ld=eb.ld)
+                            pairs=pstats, ld=eb.ld, cols=w.cols)
             rows_out.append({"workload": w.cfg.name, "kernel": kname, "early_exit": ee,
                              "executed_over_nominal_visits": visits / nominal,
                              "call_ms_median": statistics.median(call_ms),

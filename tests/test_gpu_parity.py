@@ -285,6 +285,39 @@ def test_file_to_counts(B, oracle_mod, tmp_path):
         assert (gm == wm).all() and (gc == wc).all()
 
 
+@pytest.mark.parametrize("env", [
+    {"EBIC_PB_SMEM": "0"},                                       # register-only landing
+    {"EBIC_PB_WARPS": "8", "EBIC_PB_TASKS_PER_SLOT": "2"},       # 8-warp CTAs, large chunks
+    {"EBIC_PB_WARPS": "1", "EBIC_PB_PREFETCH": "0"},             # 1-warp CTAs, no L2 prefetch
+    {"EBIC_PB_WARM": "3", "EBIC_PB_PREFETCH": "2"},              # warm prefetch from ingest, distance 2
+])
+def test_experiment_knobs_keep_parity(env):
+    """The PAIRBITS experiment knobs (environment variables read once per process) select other
+    template instantiations of the kernel; each must still reproduce the oracle bit for bit.  Runs in a child
+    process because the knobs are latched at first use."""
+    import os
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    code = (
+        "import numpy as np, torch, oracle\n"
+        "from paper_1807_09932_b200 import binding as B, workloads as W\n"
+        "w = W.make_workload(3, rows=70_001, n_ind=700)\n"
+        "st, want = oracle.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)\n"
+        "with B.Ebic(w.matrix, w.missing_mode) as eb:\n"
+        "    eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)\n"
+        "    for ee in (False, True):\n"
+        "        eb.set_early_exit(ee)\n"
+        "        got = eb.eval_fitness(torch.from_numpy(w.offsets).cuda(), torch.from_numpy(w.col_ids).cuda())\n"
+        "        torch.cuda.synchronize()\n"
+        "        assert (got.cpu().numpy().view(np.uint64) == want).all(), ee\n"
+        "print('ok')\n")
+    res = subprocess.run([sys.executable, "-c", code], cwd=root, env={**os.environ, **env}, capture_output=True,
+                         text=True, timeout=600)
+    assert res.returncode == 0 and res.stdout.strip().endswith("ok"), res.stderr[-2000:]
+
+
 def test_probe_read_bandwidth(B):
     """Measurement utility: an L2-resident buffer streams faster than HBM; bad arguments are refused."""
     l2 = B.ebic_probe_read_bandwidth(64 << 20, 20)
