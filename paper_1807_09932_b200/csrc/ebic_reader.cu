@@ -9,7 +9,10 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <algorithm>
+#include <atomic>
 #include <new>
+#include <thread>
 #include <vector>
 
 namespace {
@@ -85,15 +88,18 @@ int ebic_read_delimited(const char* path, char delimiter, float** matrix, int64_
     if (!f) return EBIC_ERR_IO;
     std::vector<char> buf;
     {
-        char chunk[1 << 16];
-        size_t got;
-        try {
-            while ((got = fread(chunk, 1, sizeof(chunk), f)) > 0) buf.insert(buf.end(), chunk, chunk + got);
-        } catch (const std::bad_alloc&) {
-            fclose(f);
-            return EBIC_ERR_OOM;
+        bool bad = fseek(f, 0, SEEK_END) != 0;
+        const long size = bad ? -1 : ftell(f);
+        bad = bad || size < 0 || fseek(f, 0, SEEK_SET) != 0;
+        if (!bad) {
+            try {
+                buf.resize(static_cast<size_t>(size));
+            } catch (const std::bad_alloc&) {
+                fclose(f);
+                return EBIC_ERR_OOM;
+            }
+            bad = size > 0 && fread(buf.data(), 1, buf.size(), f) != buf.size();
         }
-        const bool bad = ferror(f) != 0;
         fclose(f);
         if (bad) return EBIC_ERR_IO;
     }
@@ -114,25 +120,42 @@ int ebic_read_delimited(const char* path, char delimiter, float** matrix, int64_
     if (C < 1 || C > 2147483647ll || R > 2147483647ll) return EBIC_ERR_IO;
     float* M = static_cast<float*>(malloc(static_cast<size_t>(R) * static_cast<size_t>(C) * sizeof(float)));
     if (!M) return EBIC_ERR_OOM;
-    for (int64_t r = 0; r < R; ++r) {
-        const Line& l = lines[static_cast<size_t>(r) + 1];
-        const char* p = static_cast<const char*>(memchr(l.begin, d, static_cast<size_t>(l.end - l.begin)));   // skip the row name
-        int64_t c = 0;
-        while (p) {
-            const char* b = p + 1;
-            const char* nx = static_cast<const char*>(memchr(b, d, static_cast<size_t>(l.end - b)));
-            const char* e = nx ? nx : l.end;
-            if (c >= C || !parse_value(b, e, &M[r * C + c])) {
-                free(M);
-                return EBIC_ERR_IO;
+    // rows are independent: contiguous row ranges are parsed by up to 16 host threads
+    std::atomic<bool> failed(false);
+    auto parse_rows = [&](int64_t r_begin, int64_t r_end) {
+        for (int64_t r = r_begin; r < r_end && !failed.load(std::memory_order_relaxed); ++r) {
+            const Line& l = lines[static_cast<size_t>(r) + 1];
+            const char* p = static_cast<const char*>(memchr(l.begin, d, static_cast<size_t>(l.end - l.begin)));   // skip the row name
+            int64_t c = 0;
+            bool ok = true;
+            while (p && ok) {
+                const char* b = p + 1;
+                const char* nx = static_cast<const char*>(memchr(b, d, static_cast<size_t>(l.end - b)));
+                const char* e = nx ? nx : l.end;
+                ok = c < C && parse_value(b, e, &M[r * C + c]);
+                ++c;
+                p = nx;
             }
-            ++c;
-            p = nx;
+            if (!ok || c != C) failed.store(true, std::memory_order_relaxed);   // not a number, or a ragged line
         }
-        if (c != C) {                                  // ragged line
-            free(M);
-            return EBIC_ERR_IO;
+    };
+    const unsigned hw = std::thread::hardware_concurrency();
+    const int64_t n_threads = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(hw ? hw : 1, 16), R * C / 65536));
+    if (n_threads == 1) {
+        parse_rows(0, R);
+    } else {
+        std::vector<std::thread> pool;
+        try {
+            for (int64_t t = 0; t < n_threads; ++t) pool.emplace_back(parse_rows, R * t / n_threads, R * (t + 1) / n_threads);
+        } catch (...) {                                // could not start a thread: finish what is left here
+            const int64_t started = static_cast<int64_t>(pool.size());
+            parse_rows(R * started / n_threads, R);
         }
+        for (auto& th : pool) th.join();
+    }
+    if (failed.load()) {
+        free(M);
+        return EBIC_ERR_IO;
     }
     *matrix = M;
     *rows = R;
