@@ -35,6 +35,8 @@ struct ebic_ctx {
     int64_t pb_bytes = 0;
     int32_t* d_err = nullptr;               // sticky device error
     unsigned long long* d_visits = nullptr; // executed-visit counter (instrumentation)
+    unsigned long long* d_task = nullptr;   // task counter of the persistent PAIRBITS kernel (zeroed by every ingest)
+    int32_t pb_persist_ctas = 0;            // resident CTAs of that kernel on this GPU (0 = not yet queried)
     int32_t count_visits = 0;
 
     // scratch, grown on demand
@@ -233,6 +235,21 @@ int launch_pairbits(ebic_ctx* ctx, int32_t n_ind, int64_t n_ids, unsigned long l
         else fitness_pairbits_kernel<false, NW><<<g, NW * 32, 0, stream>>>(p);                 \
     } while (0)
     static const int use_smem = env_int("EBIC_PB_SMEM", 1);
+    static const int persist = env_int("EBIC_PB_PERSIST", 0);
+    p.task_counter = ctx->d_task;
+    if (persist && use_smem && nw == 2) {
+        if (ctx->pb_persist_ctas == 0) {
+            int per_sm = 0;
+            EBIC_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fitness_pairbits_persistent_kernel<false, 2, true>, 64, 8192));
+            ctx->pb_persist_ctas = std::max(1, per_sm) * ctx->sm_count;
+        }
+        const unsigned pg = static_cast<unsigned>(std::min<int64_t>(ctx->pb_persist_ctas, grid));
+        ctx->last_grid = static_cast<int32_t>(pg);
+        if (ctx->early_exit) fitness_pairbits_persistent_kernel<true, 2, true><<<pg, 64, 8192, stream>>>(p);
+        else fitness_pairbits_persistent_kernel<false, 2, true><<<pg, 64, 8192, stream>>>(p);
+        ctx->launches++;
+        return cuda_status(cudaGetLastError());
+    }
     if (use_smem && nw == 2) {
         if (ctx->early_exit) fitness_pairbits_kernel<true, 2, true><<<g, 64, 8192, stream>>>(p);
         else fitness_pairbits_kernel<false, 2, true><<<g, 64, 8192, stream>>>(p);
@@ -310,7 +327,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         offsets, col_ids, n_ind, n_ids, ctx->cols, ctx->rows, ctx->missing_mode == EBIC_MISSING_ON,
         ctx->nonmissing, ctx->meta, ctx->pids, ctx->cols <= 256 ? ctx->pids8 : nullptr,
         ctx->PB ? ctx->ppair : nullptr, ctx->PB ? ctx->prec : nullptr, static_cast<uint32_t>(ctx->ld / 128), counts,
-        ctx->d_err, ctx->PB, ctx->cols * ctx->cols, warm_bytes);
+        ctx->d_err, ctx->PB, ctx->cols * ctx->cols, warm_bytes, ctx->d_task);
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());
 
@@ -422,9 +439,10 @@ static int create_impl(const float* matrix, int64_t rows, int32_t cols, int32_t 
         if ((st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->Mc), n * 4))) break;
         if ((st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->nanmask), n / 8))) break;
         if ((st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->nonmissing), static_cast<int64_t>(cols) * 8))) break;
-        if ((st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->d_err), 16))) break;
+        if ((st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->d_err), 32))) break;
         ctx->d_visits = reinterpret_cast<unsigned long long*>(ctx->d_err + 2);
-        if ((st = cuda_status(cudaMemset(ctx->d_err, 0, 16)))) break;
+        ctx->d_task = reinterpret_cast<unsigned long long*>(ctx->d_err + 4);
+        if ((st = cuda_status(cudaMemset(ctx->d_err, 0, 32)))) break;
         if ((st = cuda_status(cudaMemset(ctx->nonmissing, 0, static_cast<size_t>(cols) * 8)))) break;
 
         // a1: transpose (device input: in one go; host input: through a bounded staging buffer)

@@ -38,8 +38,10 @@ ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __r
                          int32_t* __restrict__ pids, uint8_t* __restrict__ pids8, int32_t* __restrict__ ppair,
                          int32_t* __restrict__ prec, uint32_t pair_stride16,
                          unsigned long long* __restrict__ counts, int32_t* __restrict__ err,
-                         const uint32_t* __restrict__ warm_PB, int32_t warm_pairs, uint32_t warm_bytes)
+                         const uint32_t* __restrict__ warm_PB, int32_t warm_pairs, uint32_t warm_bytes,
+                         unsigned long long* __restrict__ task_counter)
 {
+    if (blockIdx.x == 0 && threadIdx.x == 0 && task_counter != nullptr) *task_counter = 0;   // for the persistent PAIRBITS kernel
     // one warp per individual, lane i takes ids i, i + 32, ...: the id loads and the slot stores run in parallel
     const int lane = threadIdx.x & 31;
     const int32_t k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);

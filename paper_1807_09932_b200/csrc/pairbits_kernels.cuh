@@ -32,7 +32,8 @@ struct PairbitsParams {
     unsigned long long* counts;
     unsigned long long* visits;      // executed (row, pair) visits (instrumented) or nullptr
     int32_t n_pairs;                 // cols * cols bit columns in PB
-    int32_t prefetch_dist;           // CTAs of chunk g prefetch a slice of the bit columns of chunk g + dist into L2 (0 = off)
+    int32_t prefetch_dist;           // tasks of chunk g prefetch a slice of the bit columns of chunk g + dist into L2 (0 = off)
+    unsigned long long* task_counter; // persistent kernel: next task index (zeroed by the ingest kernel)
 };
 
 __device__ __forceinline__ void and4(uint4& a, const uint4& v) {
@@ -128,36 +129,30 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
     return done;
 }
 
-template <bool EARLY_EXIT, int NW, bool SMEM = false>
-__global__ void __launch_bounds__(NW * 32)
-fitness_pairbits_kernel(const PairbitsParams p)
+// One warp task: individual k = task % n_ind on row chunk g = task / n_ind.  `rec` = lane's word of k's record.
+template <bool EARLY_EXIT, bool SMEM>
+__device__ __forceinline__ void pairbits_task(const PairbitsParams& p, int64_t task, uint32_t rec, int lane, uint32_t ring,
+                                              unsigned long long& executed)
 {
-    extern __shared__ __align__(16) unsigned char pb_ring[];     // SMEM: NW x 4 KB landing ring
-    constexpr int kPairbitsWarps = NW;   // warps (= tasks) per CTA: a CTA's slot is held until its longest chromosome ends
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t task = static_cast<int64_t>(blockIdx.x) * kPairbitsWarps + warp;
     const int64_t g = task / p.n_ind;
     const int32_t k = static_cast<int32_t>(task - g * p.n_ind);
     const int64_t w_begin = g * p.chunk_words;
     if (w_begin >= p.ldw) return;                                // warp-uniform
-    if (p.prefetch_dist > 0 && warp == 0) {
-        // Every bit column of a later chunk is requested from HBM exactly once, by one lane of one CTA of
-        // this chunk, `prefetch_dist` chunks before the demand loads arrive: those then hit L2.
-        const int64_t ctas_per_chunk = (static_cast<int64_t>(p.n_ind) + kPairbitsWarps - 1) / kPairbitsWarps;
-        const int64_t j = blockIdx.x - g * p.n_ind / kPairbitsWarps; // position of this CTA inside its chunk (approx.)
-        const int32_t per_cta = static_cast<int32_t>((p.n_pairs + ctas_per_chunk - 1) / ctas_per_chunk);
+    if (p.prefetch_dist > 0) {
+        // Every bit column of a later chunk is requested from HBM exactly once, by one lane of one task of this
+        // chunk, `prefetch_dist` chunks before the demand loads arrive: those then hit L2.
+        const int32_t per = (p.n_pairs + p.n_ind - 1) / p.n_ind;     // columns per task
         const int64_t first = (g == 0) ? 1 : p.prefetch_dist;        // chunk 0 also covers the cold start
         for (int64_t d = first; d <= p.prefetch_dist; ++d) {
             const int64_t pw = (g + d) * p.chunk_words;
             if (pw >= p.ldw) break;
             const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.chunk_words), p.ldw - pw)) * 4u;
-            for (int32_t q = lane; q < per_cta; q += 32) {
-                const int64_t pair = j * per_cta + q;
-                if (pair >= 0 && pair < p.n_pairs) bulk_prefetch_l2(p.PB + pair * p.ldw + pw, bytes);
+            for (int32_t q = lane; q < per; q += 32) {
+                const int64_t pair = static_cast<int64_t>(k) * per + q;
+                if (pair < p.n_pairs) bulk_prefetch_l2(p.PB + pair * p.ldw + pw, bytes);
             }
         }
     }
-    const uint32_t rec = static_cast<uint32_t>(__ldg(p.prec + 32ll * k + lane));   // the individual: one coalesced 128 B load
     const int32_t L = static_cast<int32_t>(__shfl_sync(0xffffffffu, rec, 0));
     if (L < 2) return;
     const int32_t npr = L - 1;
@@ -167,15 +162,13 @@ fitness_pairbits_kernel(const PairbitsParams p)
     const uint4* PB4 = reinterpret_cast<const uint4*>(p.PB);
 
     unsigned int cnt = 0;
-    unsigned long long executed = 0;
     // Lane l holds words 4l .. 4l+3 of the step's first 128 words (acc_a) and the same words of its second 128
     // (acc_b).  Record / ppair entries are the bit columns' offsets into PB in uint4 units (< 2^32, host-checked).
     const int64_t n_full = (w_end - w_begin) / kPairbitsStepWords;
     const uint4* base = PB4 + (w_begin >> 2) + lane;
     for (int64_t s = 0; s < n_full; ++s, base += kPairbitsStepWords / 4) {
         uint4 acc_a = make_uint4(~0u, ~0u, ~0u, ~0u), acc_b = acc_a;
-        const int32_t done = pairbits_step<EARLY_EXIT, true, SMEM>(base, base, rec, n0, npr, pp, lane, acc_a, acc_b,
-                                                                   SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u);
+        const int32_t done = pairbits_step<EARLY_EXIT, true, SMEM>(base, base, rec, n0, npr, pp, lane, acc_a, acc_b, ring);
         cnt += __popc(acc_a.x) + __popc(acc_a.y) + __popc(acc_a.z) + __popc(acc_a.w);
         cnt += __popc(acc_b.x) + __popc(acc_b.y) + __popc(acc_b.z) + __popc(acc_b.w);
         executed += static_cast<unsigned long long>(done) * (kPairbitsStepWords * 32);
@@ -194,10 +187,56 @@ fitness_pairbits_kernel(const PairbitsParams p)
         executed += static_cast<unsigned long long>(done) * ((w_end - w0) * 32);
     }
     cnt = __reduce_add_sync(0xffffffffu, cnt);
-    if (lane == 0) {
-        if (cnt) atomicAdd(&p.counts[k], static_cast<unsigned long long>(cnt));
-        if (p.visits != nullptr) atomicAdd(p.visits, executed);
+    if (lane == 0 && cnt) atomicAdd(&p.counts[k], static_cast<unsigned long long>(cnt));
+}
+
+// One task per warp, a CTA of NW warps per NW consecutive tasks: the hardware block scheduler balances the load.
+template <bool EARLY_EXIT, int NW, bool SMEM = false>
+__global__ void __launch_bounds__(NW * 32)
+fitness_pairbits_kernel(const PairbitsParams p)
+{
+    extern __shared__ __align__(16) unsigned char pb_ring[];     // SMEM: NW x 4 KB landing ring
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t task = static_cast<int64_t>(blockIdx.x) * NW + warp;
+    if (task >= static_cast<int64_t>(p.n_chunks) * p.n_ind) return;
+    const uint32_t rec = static_cast<uint32_t>(__ldg(p.prec + 32ll * (task % p.n_ind) + lane));   // one coalesced 128 B load
+    unsigned long long executed = 0;
+    pairbits_task<EARLY_EXIT, SMEM>(p, task, rec, lane, SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u, executed);
+    if (lane == 0 && p.visits != nullptr && executed) atomicAdd(p.visits, executed);
+}
+
+// Persistent variant: as many CTAs as fit the GPU; every warp draws task indices from a global counter (zeroed by the
+// ingest kernel) and fetches the NEXT task's index and record while it works on the current one, so neither the
+// counter's nor the record's latency sits on a task's critical path, and a warp never idles behind a longer
+// neighbour of its CTA.
+#ifndef EBIC_PB_PERSIST_MIN_BLOCKS          /* -DEBIC_PB_PERSIST_MIN_BLOCKS=1 lifts the 64-register cap (diagnostic build) */
+#define EBIC_PB_PERSIST_MIN_BLOCKS (32 / NW)
+#endif
+template <bool EARLY_EXIT, int NW, bool SMEM>
+__global__ void __launch_bounds__(NW * 32, EBIC_PB_PERSIST_MIN_BLOCKS)
+fitness_pairbits_persistent_kernel(const PairbitsParams p)
+{
+    extern __shared__ __align__(16) unsigned char pb_ring[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const uint32_t ring = SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u;
+    const int64_t total = static_cast<int64_t>(p.n_chunks) * p.n_ind;
+    auto grab = [&]() {
+        unsigned long long t = 0;
+        if (lane == 0) t = atomicAdd(p.task_counter, 1ull);
+        return static_cast<int64_t>(__shfl_sync(0xffffffffu, t, 0));
+    };
+    int64_t next = grab();
+    uint32_t rec_next = 0;
+    if (next < total) rec_next = static_cast<uint32_t>(__ldg(p.prec + 32ll * (next % p.n_ind) + lane));
+    unsigned long long executed = 0;
+    while (next < total) {
+        const int64_t cur = next;
+        const uint32_t rec = rec_next;
+        next = grab();
+        if (next < total) rec_next = static_cast<uint32_t>(__ldg(p.prec + 32ll * (next % p.n_ind) + lane));
+        pairbits_task<EARLY_EXIT, SMEM>(p, cur, rec, lane, ring, executed);
     }
+    if (lane == 0 && p.visits != nullptr && executed) atomicAdd(p.visits, executed);
 }
 
 }  // namespace ebic

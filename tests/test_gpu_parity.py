@@ -290,6 +290,7 @@ def test_file_to_counts(B, oracle_mod, tmp_path):
     {"EBIC_PB_WARPS": "8", "EBIC_PB_TASKS_PER_SLOT": "2"},       # 8-warp CTAs, large chunks
     {"EBIC_PB_WARPS": "1", "EBIC_PB_PREFETCH": "0"},             # 1-warp CTAs, no L2 prefetch
     {"EBIC_PB_WARM": "3", "EBIC_PB_PREFETCH": "2"},              # warm prefetch from ingest, distance 2
+    {"EBIC_PB_PERSIST": "1"},                                    # persistent warps drawing tasks from a counter
 ])
 def test_experiment_knobs_keep_parity(env):
     """The PAIRBITS experiment knobs (environment variables read once per process) select other
