@@ -133,7 +133,7 @@ def measure_l2_gbs(B):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the fitness kernel, from the committed ncu --set full
 # captures (profiles/r01_fitness_<kernel>_<workload>_ncu_full.txt), full-size workloads only.
-NCU_TRAFFIC_BYTES = {("c4", "pairbits"): 224.25e6 + 4.37e6, ("c5", "pairbits"): 2151.88e6 + 4.86e6,
+NCU_TRAFFIC_BYTES = {("c4", "pairbits"): 224.23e6 + 4.39e6, ("c5", "pairbits"): 2152.17e6 + 4.21e6,
                      ("c4", "rank8"): 28.03e6, ("c4", "tiled_f32"): 125.01e6 + 6.72e6}
 
 
