@@ -1,26 +1,34 @@
 #!/usr/bin/env python
 """bench.py -- row-pair comparisons/s of EBIC population fitness evaluation on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c1..c5] [--kernel auto|rank8|tiled_f32|direct]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c1..c5|p1..p3] [--kernel auto|...]
     python bench.py --impl reference ...      # the CPU oracle as it stands, on the host cores
     python bench.py --table                   # every workload x every kernel -> gpurun_out/table.json
 
-A step = one pass of the hot path over one population: population ingest
-+ validation, tile staging, trend predicate, count accumulation (`ebic_eval_fitness`) and the
-matched-row bitmasks of 8 chosen individuals (`ebic_extract_rows`).  The loader (a1/a2: transpose,
-NaN mask, rank tiles) runs once per dataset in `ebic_create`; its time is reported as `create_ms`.
+A step = one pass of the hot path over one population: population ingest +
+validation, trend predicate, count accumulation and the matched-row bitmasks of 8 chosen individuals -- one
+`ebic_eval_extract` call (N > 1: the rank's row slice, then the all-reduce of the counts).  The loader (a1/a2:
+transpose, NaN mask, pair table / rank tiles) runs once per dataset in `ebic_create`; its time is reported as
+`create_ms` with a per-phase breakdown.
 
-`value`  = nominal row-pair comparisons of the fitness evaluation (rows * sum(max(L-1,0))) per second of
-           step time, population and matrix resident in HBM, CUDA events on the launch stream, L2
-           flushed between steps, max over ranks.
-`e2e`    = same, through the C-ABI with HOST buffers: pinned population in, counts and masks out,
-           copies inside the timed region.
-`roofline` is for the dominant kernel (the fitness kernel), timed live with CUDA events recorded by
-the library around that kernel on its stream (DESIGN.md section 6 derives the peak).
+Default workload: C5 (16,777,216 x 32, population 4,096), the largest single-GPU configuration of BASELINE.json
+(its `metric` names none).  The other configurations and the paper-shaped stand-ins are measured in the same run
+and printed in the `per_workload` block of the same JSON line.
+
+`value`  = nominal row-pair comparisons of the fitness evaluation (rows * sum(max(L-1,0))) per second of step
+           time, population and matrix resident in HBM, CUDA events on the launch stream, L2 flushed between
+           steps, max over ranks.
+`e2e`    = same, through the C ABI with HOST buffers: pinned population in, counts and masks out, copies inside
+           the timed region.
+`roofline` is for the dominant kernel (the fitness kernel), timed live with CUDA events recorded by the library
+around that kernel on its stream (DESIGN.md section 6 derives the peaks; the probes of include/ebic_debug.h
+measure them in the same process).
 """
 from __future__ import annotations
 
 import argparse
+import csv
+import hashlib
 import json
 import os
 import statistics
@@ -41,7 +49,9 @@ METRIC = "row_pair_comparisons_per_s"
 UNIT = "comparisons/s"
 N_CHOSEN = 8
 WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4, "p1": 5, "p2": 6, "p3": 7}
-KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4}
+KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "union_f32": 5}
+TRAFFIC_CSV = ROOT / "profiles" / "r02_dram_traffic.csv"
+KERNEL_SOURCES = ["pairbits_kernels.cuh", "fitness_kernels.cuh", "union_kernels.cuh", "ebic_device.cuh"]
 
 
 def log(*a):
@@ -70,7 +80,7 @@ class ClockSampler:
     def __enter__(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
                  "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -117,6 +127,33 @@ def pick_chosen(w):
     return np.array(ch, dtype=np.int32)
 
 
+def kernel_source_sha() -> str:
+    """Identifies the fitness kernels a committed ncu capture was taken on (profiles/r02_dram_traffic.csv)."""
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        p = ROOT / "paper_1807_09932_b200" / "csrc" / name
+        if p.exists():
+            h.update(p.read_bytes())
+    return h.hexdigest()[:12]
+
+
+def ncu_traffic(workload_key: str, kernel_name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the fitness kernel from the committed
+    `ncu --set full` captures (profiles/r02_dram_traffic.csv, written by hand from the .txt summaries it names).
+    None -- with the reason -- when there is no capture for this workload / kernel or when the kernels have
+    changed since the capture was taken."""
+    if not TRAFFIC_CSV.exists():
+        return None, "no profiles/r02_dram_traffic.csv"
+    sha = kernel_source_sha()
+    with TRAFFIC_CSV.open() as f:
+        for row in csv.DictReader(f):
+            if row["workload"] == workload_key and row["kernel"] == kernel_name:
+                if row["kernel_sha"] != sha:
+                    return None, f"capture {row['capture']} is older than the kernel sources ({row['kernel_sha']} != {sha})"
+                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), f"profiles/{row['capture']}"
+    return None, "no capture for this workload and kernel"
+
+
 # ----------------------------------------------------------------------------------------------------
 # roofline of the fitness kernel (DESIGN.md section 6)
 # ----------------------------------------------------------------------------------------------------
@@ -125,16 +162,18 @@ def pick_chosen(w):
 L2_XBAR_BYTES_PER_CLK = 184 * 64
 
 
-def measure_l2_gbs(B):
-    """What a plain streaming read of an L2-resident buffer reaches on this GPU (64 MiB, L1 bypassed):
-    ebic_probe_read_bandwidth.  Context for the L2 roofline, not its denominator."""
-    return B.ebic_probe_read_bandwidth(64 << 20, 40)
+class Probes:
+    """The ceilings measured in this process by the probes of include/ebic_debug.h (once per run)."""
 
+    def __init__(self, B):
+        self.l2_gbs = B.ebic_probe_read_bandwidth(48 << 20, 40)      # L2-resident streaming read, L1 bypassed
+        self.hbm_read_gbs = B.ebic_probe_read_bandwidth(4 << 30, 2)  # far larger than the 126 MB L2
+        self.smem_gbs = B.ebic_probe_smem_bandwidth()                # conflict-free LDS.128, all SMs
+        self.fsetp_gcmp = B.ebic_probe_fsetp_rate()                  # 1e9 ordered float compares / s, all SMs
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the fitness kernel, from the committed ncu --set full
-# captures (profiles/r01_fitness_<kernel>_<workload>_ncu_full.txt), full-size workloads only.
-NCU_TRAFFIC_BYTES = {("c4", "pairbits"): 224.23e6 + 4.39e6, ("c5", "pairbits"): 2152.17e6 + 4.21e6,
-                     ("c4", "rank8"): 28.03e6, ("c4", "tiled_f32"): 125.01e6 + 6.72e6}
+    def as_dict(self):
+        return {"l2_read_gbs": self.l2_gbs, "hbm_read_gbs": self.hbm_read_gbs, "smem_lds128_gbs": self.smem_gbs,
+                "fsetp_gcompares_per_s": self.fsetp_gcmp}
 
 
 def pair_stats(w):
@@ -148,13 +187,19 @@ def pair_stats(w):
     return {"uses": int(keys.size), "unique": int(np.unique(keys).size)}
 
 
-def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, traffic=None, l2_gbs=None,
-             pairs=None, ld=None, cols=None):
-    """each kernel against the memory its operands have to come through."""
+def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count, probes=None, traffic=None,
+             traffic_source=None, pairs=None, ld=None, cols=None):
+    """each kernel against the memory its operands have to come through.  `frac` uses the
+    STRICTER of the stated and the probed ceiling for the on-chip pipes (the larger number), and says which."""
     f_hz = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
-    pipe_gbs = sm_count * 128 * f_hz / 1e9                 # 128 B / clk / SM: shared memory and L1 share this pipe
-    pipe_basis = f"{sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz ({peaks_kind} sm_max_mhz)"
-    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "direct": 4, "pairbits": 0.125}[kernel_name]
+    hbm_peak = float(peaks["hbm_gbs"])
+    pipe_stated = sm_count * 128 * f_hz / 1e9              # 128 B / clk / SM: shared memory and L1 share this pipe
+    pipe_probe = probes.smem_gbs if probes else None
+    pipe_gbs = max(pipe_stated, pipe_probe or 0.0)
+    pipe_basis = (f"max(stated {sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz = {pipe_stated:.0f} GB/s, "
+                  f"LDS.128 probe {pipe_probe:.0f} GB/s)" if pipe_probe else
+                  f"{sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz ({peaks_kind} sm_max_mhz)")
+    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "union_f32": 4, "direct": 4, "pairbits": 0.125}[kernel_name]
     achieved = visits_executed * bytes_per_visit / kernel_s / 1e9
     bound, peak, basis = "alu", pipe_gbs, pipe_basis
     resource = "shared-memory data pipe (128 B/clk/SM)"
@@ -164,7 +209,6 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
             resource += " == INT ALU pipe at 0.5 op/visit"
         # second floor: the tiles are staged from HBM once per evaluation (tiny populations are bound by that)
         if ld and cols:
-            hbm_peak = float(peaks["hbm_gbs"])
             stage_bytes = ld * cols * (1 if kernel_name == "rank8" else 4)
             t_pipe, t_hbm = visits_executed * bytes_per_visit / (pipe_gbs * 1e9), stage_bytes / (hbm_peak * 1e9)
             extra = {"pipe_floor_ms": t_pipe * 1e3, "hbm_floor_ms": t_hbm * 1e3}
@@ -177,8 +221,9 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
         resource = "L1/LSU data pipe (128 B/clk/SM)"
     elif kernel_name == "pairbits":
         # two floors: the gathered bits through L2 -> SM, and the distinct bit columns once from HBM
-        l2_peak = L2_XBAR_BYTES_PER_CLK * f_hz / 1e9
-        hbm_peak = float(peaks["hbm_gbs"])
+        l2_stated = L2_XBAR_BYTES_PER_CLK * f_hz / 1e9
+        l2_probe = probes.l2_gbs if probes else None
+        l2_peak = max(l2_stated, l2_probe or 0.0)
         t_l2 = visits_executed * bytes_per_visit / (l2_peak * 1e9)
         unique_bytes = pairs["unique"] * (ld // 8) if pairs and ld else 0
         if pairs and ld and pairs["uses"]:
@@ -187,7 +232,8 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
             unique_bytes *= min(1.0, visits_executed / (pairs["uses"] * ld))
         t_hbm = unique_bytes / (hbm_peak * 1e9)
         extra = {"l2_floor_ms": t_l2 * 1e3, "hbm_floor_ms": t_hbm * 1e3, "pair_uses": pairs["uses"] if pairs else None,
-                 "distinct_pairs": pairs["unique"] if pairs else None, "l2_probe_gbs": l2_gbs}
+                 "distinct_pairs": pairs["unique"] if pairs else None, "l2_peak_stated_gbs": l2_stated,
+                 "l2_peak_probe_gbs": l2_probe}
         if t_hbm > t_l2:
             bound, peak, achieved = "hbm", hbm_peak, unique_bytes / kernel_s / 1e9
             resource = "HBM read of the distinct bit columns the population uses (each once; little re-use)"
@@ -196,11 +242,11 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
         else:
             bound, peak = "l2", l2_peak
             resource = "L2 -> SM read bandwidth (bit columns gathered from L2 with 128-bit loads)"
-            basis = (f"184 L2 slices x 64 B/clk x {f_hz/1e6:.0f} MHz (ncu lts2xbar peak_sustained; a plain L2-resident "
-                     f"streaming read reaches {l2_gbs:.0f} GB/s in this run)" if l2_gbs else
+            basis = (f"max(ncu-stated lts2xbar peak 184 slices x 64 B/clk x {f_hz/1e6:.0f} MHz = {l2_stated:.0f} GB/s, "
+                     f"L2-resident read probe {l2_probe:.0f} GB/s)" if l2_probe else
                      f"184 L2 slices x 64 B/clk x {f_hz/1e6:.0f} MHz (ncu lts2xbar peak_sustained)")
     out = {"bound": bound, "resource": resource, "kernel": "fitness_" + kernel_name, "achieved": achieved,
-           "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+           "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source,
            "bytes_per_visit": bytes_per_visit, "visits_per_launch": visits_executed,
            "kernel_ms": kernel_s * 1e3, "peak_basis": basis}
     out.update(extra)
@@ -208,12 +254,133 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
 
 
 # ----------------------------------------------------------------------------------------------------
+# one workload on one GPU: create (with breakdown), production step, event-bracketed kernel, roofline, break-even
+# ----------------------------------------------------------------------------------------------------
+def timed_ms(fn, reps, flush):
+    """Median / all of `reps` calls of fn(), each bracketed by CUDA events on the current stream, L2 flushed before."""
+    import torch
+    out = []
+    for _ in range(reps):
+        flush.zero_()
+        s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s.record()
+        fn()
+        e.record()
+        torch.cuda.synchronize()
+        out.append(s.elapsed_time(e))
+    return statistics.median(out), out
+
+
+def best_kernel_without_table(B, eb):
+    """The fastest kernel that needs no pair table for this shape (what AUTO falls to when the table is refused)."""
+    for k in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_UNION_F32, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_DIRECT):
+        try:
+            eb.set_kernel(k)
+            eb.set_kernel(B.EBIC_KERNEL_AUTO)
+            return k
+        except B.EbicError:
+            continue
+    return B.EBIC_KERNEL_DIRECT
+
+
+def measure_workload(B, key, w, peaks, peaks_kind, probes, flush, reps, early_exit=0, with_alt=True):
+    """One `per_workload` entry: everything measured in this process on the workload `w`."""
+    import torch
+    t0 = time.time()
+    eb = B.Ebic(w.matrix, w.missing_mode)                      # host matrix -> H2D + loader kernels
+    torch.cuda.synchronize()
+    create_ms = (time.time() - t0) * 1e3
+    breakdown = eb.create_breakdown_ms()
+    eb.set_early_exit(bool(early_exit))
+    chosen = pick_chosen(w)
+    d_off, d_ids, d_chosen = (torch.from_numpy(a).cuda() for a in (w.offsets, w.col_ids, chosen))
+    d_counts = torch.empty(w.n_ind, dtype=torch.int64, device="cuda")
+    d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
+    d_mcnt = torch.empty(len(chosen), dtype=torch.int64, device="cuda")
+
+    def step():
+        eb.eval_extract(d_off, d_ids, d_chosen, counts=d_counts, masks=d_masks, mask_counts=d_mcnt)
+
+    def eval_only():
+        eb.eval_fitness(d_off, d_ids, counts=d_counts)
+
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    kernel_name = B.KERNEL_NAMES[eb.last_kernel]
+    step_ms, _ = timed_ms(step, reps, flush)                    # production configuration: no instrumentation
+    eb.set_instrumentation(1)
+    eval_only()
+    visits = eb.info(10)
+    if kernel_name == "direct":
+        visits = eb.ld * int(w.lengths.sum())
+    eb.set_instrumentation(2)                                   # event pair around the fitness kernel
+    timed_ms(eval_only, reps, flush)
+    kernel_ms = eb.info(11) / 1e6
+    eb.set_instrumentation(0)
+    traffic, traffic_src = ncu_traffic(key, kernel_name)
+    roof = roofline(kernel_name, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7), probes=probes,
+                    traffic=traffic, traffic_source=traffic_src, pairs=pair_stats(w), ld=eb.ld, cols=w.cols)
+    entry = {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind, "kernel": kernel_name,
+             "step_ms": step_ms, "kernel_ms": kernel_ms, "comparisons_per_s": w.comparisons / (step_ms * 1e-3),
+             "bound": roof["bound"], "frac": roof["frac"], "achieved_gbs": roof["achieved"], "peak_gbs": roof["peak"],
+             "create_ms": create_ms, "create_breakdown_ms": breakdown, "device_bytes": eb.info(9),
+             "pair_table_bytes": eb.info(14)}
+    # the pair table's builder against its own HBM floor: read the float32 matrix once, write the table once
+    if eb.info(14):
+        floor_ms = (eb.ld * w.cols * 4 + eb.info(14)) / (float(peaks["hbm_gbs"]) * 1e9) * 1e3
+        entry["pair_table_build"] = {"ms": breakdown["pair_table"], "hbm_floor_ms": floor_ms,
+                                     "frac_of_hbm_floor": floor_ms / max(breakdown["pair_table"], 1e-9)}
+    # break-even: evaluations after which building the table has paid for itself against the best kernel that
+    # needs no table (its own derived data -- the rank tiles -- is credited to it)
+    if with_alt and eb.info(14):
+        alt = best_kernel_without_table(B, eb)
+        eb.set_kernel(alt)
+        for _ in range(2):
+            eval_only()
+        eb.set_instrumentation(2)
+        timed_ms(eval_only, max(3, reps // 2), flush)
+        alt_ms = eb.info(11) / 1e6
+        eb.set_instrumentation(0)
+        alt_build = eb.info(23) / 1e6 if alt == B.EBIC_KERNEL_RANK8 else 0.0
+        gain = alt_ms - kernel_ms
+        entry["break_even"] = {"against": B.KERNEL_NAMES[alt], "its_kernel_ms": alt_ms, "its_build_ms": alt_build,
+                               "pair_table_build_ms": breakdown["pair_table"],
+                               "evals": (breakdown["pair_table"] - alt_build) / gain if gain > 0 else None}
+        eb.set_kernel(B.EBIC_KERNEL_AUTO)
+    eb.close()
+    return entry, roof
+
+
+# ----------------------------------------------------------------------------------------------------
 # GPU arm
 # ----------------------------------------------------------------------------------------------------
+def rank_matrix(w, idx, rank, world, scaling):
+    """The rows this rank holds.  strong: its row_partition slice of the one dataset (Fig. 1 / line 77:
+    a fixed dataset over 1..8 GPUs).  weak: every rank holds `rows` rows of its own -- rank 0 the workload's
+    matrix, the others a fresh draw of the same distribution and NaN rate (not a permutation of rank 0's)."""
+    from paper_1807_09932_b200.sharded import row_partition
+    if world == 1:
+        return w.matrix, w.rows
+    if scaling == "strong":
+        b, e = row_partition(w.rows, world)[rank]
+        return np.ascontiguousarray(w.matrix[b:e]), w.rows
+    if rank > 0:
+        rng = np.random.default_rng([5, idx, rank])
+        m = W._draw_matrix(rng, w.cfg.dist, w.rows, w.cols)
+        if w.cfg.nan_rate > 0:
+            for r0 in range(0, w.rows, 1 << 20):
+                blk = m[r0:r0 + (1 << 20)]
+                blk[rng.random(blk.shape, dtype=np.float32) < np.float32(w.cfg.nan_rate)] = np.float32(np.nan)
+        return m, w.rows * world
+    return w.matrix, w.rows * world
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
     from paper_1807_09932_b200 import binding as B
+    from paper_1807_09932_b200.sharded import ShardedEbic, row_partition
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -225,54 +392,55 @@ def run_gpu(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     peaks, peaks_kind = measured_peaks()
+    scaling = args.scaling if world > 1 else "weak"            # one GPU: fixed per-GPU work by definition
 
     idx = WORKLOADS[args.workload]
     t0 = time.time()
-    # weak scaling: every rank holds its own `rows`-row slice of an (N x rows)-row dataset
     w = W.make_workload(idx, rows=args.rows, n_ind=args.n_ind)
-    if world > 1 and rank > 0:
-        rng = np.random.default_rng([2, idx, rank])
-        w.matrix = w.matrix[rng.permutation(w.rows)]           # a different slice per rank, same recipe
     gen_s = time.time() - t0
     chosen = pick_chosen(w)
+    local, rows_total = rank_matrix(w, idx, rank, world, scaling)
 
     torch.cuda.synchronize()
     t0 = time.time()
-    eb = B.Ebic(w.matrix, w.missing_mode)                      # host matrix -> H2D + loader kernels
+    if world > 1 and scaling == "strong":
+        sh = ShardedEbic.from_matrix(local, w.missing_mode, rank, world, rows_total=rows_total)
+    else:                                                      # weak: every rank is a whole context of `rows` rows
+        sh = ShardedEbic.from_matrix(local, w.missing_mode, 0, 1)
+        sh.world_size = world                                  # ... that still all-reduces its counts
+    eb = sh.ebic
     torch.cuda.synchronize()
     create_ms = (time.time() - t0) * 1e3
+    if eb is None:
+        raise SystemExit(f"rank {rank} holds no rows: {w.rows} rows over {world} ranks")
     eb.set_kernel(KERNELS[args.kernel])
     eb.set_early_exit(args.early_exit)
 
     d_off = torch.from_numpy(w.offsets).cuda()
     d_ids = torch.from_numpy(w.col_ids).cuda()
     d_chosen = torch.from_numpy(chosen).cuda()
-    d_counts = torch.empty(w.n_ind, dtype=torch.int64, device="cuda")
-    eb.eval_fitness(d_off, d_ids, counts=d_counts)             # AUTO picks by shape and population size
-    torch.cuda.synchronize()
-    kernel_name = B.KERNEL_NAMES[eb.last_kernel]
-    d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
-    d_mcnt = torch.empty(len(chosen), dtype=torch.int64, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
 
     def step():
-        eb.eval_fitness(d_off, d_ids, counts=d_counts)
-        if world > 1:
-            dist.all_reduce(d_counts)                          # the path's one exchange step (8(e))
-        eb.extract_rows(d_off, d_ids, d_chosen, masks=d_masks, counts=d_mcnt)
+        return sh.step(d_off, d_ids, d_chosen)                 # ebic_eval_extract (+ the all-reduce when N > 1)
 
     launches0 = eb.info(8)
+    d_counts, _ = step()
+    torch.cuda.synchronize()
+    launches_per_step = eb.info(8) - launches0
+    kernel_name = B.KERNEL_NAMES[eb.last_kernel]
     for _ in range(max(args.warmup, 0)):
         flush.zero_()
         step()
     torch.cuda.synchronize()
-    launches_per_step = (eb.info(8) - launches0) // max(args.warmup, 1) if args.warmup else None
 
     # executed visits of one evaluation (instrumented, outside the timed region)
     eb.set_instrumentation(1)
-    eb.eval_fitness(d_off, d_ids, counts=d_counts)
+    step()
     visits_exec = eb.info(10)
-    eb.set_instrumentation(2)                                   # event pairs around the fitness kernel
+    if kernel_name == "direct":
+        visits_exec = eb.ld * int(w.lengths.sum())
+    eb.set_instrumentation(2)                                   # event pairs around the fitness kernel, timed region included
 
     if world > 1:
         dist.barrier()
@@ -294,17 +462,17 @@ def run_gpu(args):
     total_ms = float(sum(step_ms))
     kernel_ns = eb.info(11)
     eb.set_instrumentation(0)
-    if launches_per_step is None:
-        launches_per_step = 3
+    # the same step without the library's kernel events (they keep the ingest and the fitness kernel from overlapping)
+    plain_ms, _ = timed_ms(step, args.steps, flush)
     if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        t = torch.tensor([total_ms, plain_ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+        total_ms, plain_ms = float(t[0].item()), float(t[1].item())
     ms_per_step = total_ms / args.steps
-    comparisons = w.comparisons * world
+    comparisons = w.comparisons if scaling == "strong" else w.comparisons * world
     value = comparisons / (ms_per_step * 1e-3)
 
-    # ---- e2e: host buffers through the C ABI, copies inside the timed region
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region: ONE ebic_eval_extract call
     p_off = torch.from_numpy(w.offsets).pin_memory()
     p_ids = torch.from_numpy(w.col_ids).pin_memory()
     p_chosen = torch.from_numpy(chosen).pin_memory()
@@ -313,8 +481,11 @@ def run_gpu(args):
     h_mcnt = torch.empty(len(chosen), dtype=torch.int64).pin_memory()
 
     def e2e_step():
-        eb.eval_fitness(p_off, p_ids, counts=h_counts)          # H2D population, kernels, D2H counts, sync
-        eb.extract_rows(p_off, p_ids, p_chosen, masks=h_masks, counts=h_mcnt)
+        eb.eval_extract(p_off, p_ids, p_chosen, counts=h_counts, masks=h_masks, mask_counts=h_mcnt)
+        if world > 1:                                           # the exchange step on the host-resident result
+            d = h_counts.cuda(non_blocking=True)
+            dist.all_reduce(d)
+            h_counts.copy_(d)
 
     for _ in range(3):
         e2e_step()
@@ -331,41 +502,95 @@ def run_gpu(args):
         t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
-    h2d = int(p_off.numel() * 4 * 2 + p_ids.numel() * 4 * 2 + p_chosen.numel() * 4)
+    h2d = int(p_off.numel() * 4 + p_ids.numel() * 4 + p_chosen.numel() * 4)
     d2h = int(h_counts.numel() * 8 + h_masks.numel() * 8 + h_mcnt.numel() * 8)
-    assert (h_counts.numpy() == d_counts.cpu().numpy()).all() or world > 1
+    if world == 1:
+        assert (h_counts.numpy() == d_counts.cpu().numpy()).all()
+
+    # ---- PAPER.md Fig. 1 shapes (12,483 / 54,675 / 436,444 rows) on this many GPUs, strong split (N > 1 only;
+    #      at N = 1 the per_workload block holds them)
+    fig1 = None
+    if world > 1 and not args.no_per_workload:
+        fig1 = []
+        for key in ("p1", "p2", "p3"):
+            wp = W.make_workload(WORKLOADS[key])
+            b, e = row_partition(wp.rows, world)[rank]
+            shp = ShardedEbic.from_matrix(np.ascontiguousarray(wp.matrix[b:e]), wp.missing_mode, rank, world, rows_total=wp.rows)
+            if shp.ebic is not None:
+                shp.ebic.set_early_exit(args.early_exit)
+            po, pi = torch.from_numpy(wp.offsets).cuda(), torch.from_numpy(wp.col_ids).cuda()
+            pc = torch.from_numpy(pick_chosen(wp)).cuda()
+            for _ in range(3):
+                shp.step(po, pi, pc)
+            ms, _ = timed_ms(lambda: shp.step(po, pi, pc), 20, flush)
+            t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            fig1.append({"workload": wp.cfg.name, "rows": wp.rows, "cols": wp.cols, "n_gpus": world,
+                         "step_ms": float(t.item()), "comparisons_per_s": wp.comparisons / (float(t.item()) * 1e-3)})
+            shp.close()
+            del wp
 
     out = None
     if rank == 0:
         sm_count = eb.info(7)
-        l2_gbs = measure_l2_gbs(B) if kernel_name == "pairbits" else None
-        traffic = args.traffic
-        if traffic is None and args.rows is None and args.n_ind is None:
-            traffic = NCU_TRAFFIC_BYTES.get((args.workload, kernel_name))
-        roof = roofline(kernel_name, visits_exec, kernel_ns * 1e-9, peaks, peaks_kind, sm_count,
-                        traffic=traffic, l2_gbs=l2_gbs, pairs=pair_stats(w), ld=eb.ld, cols=w.cols)
+        probes = Probes(B)
+        traffic, traffic_src = (args.traffic, "--traffic") if args.traffic is not None else (None, None)
+        if traffic is None and args.rows is None and args.n_ind is None and world == 1:
+            traffic, traffic_src = ncu_traffic(args.workload, kernel_name)
+        local_w = w
+        roof = roofline(kernel_name, visits_exec, kernel_ns * 1e-9, peaks, peaks_kind, sm_count, probes=probes,
+                        traffic=traffic, traffic_source=traffic_src, pairs=pair_stats(local_w), ld=eb.ld, cols=w.cols)
+        breakdown = eb.create_breakdown_ms()
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": scaling,
             "vs_baseline": None, "dtype": {"rank8": "u8", "pairbits": "u32"}.get(kernel_name, "f32"), "data": "synthetic",
             "config": {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind,
                        "sum_L": int(w.lengths.sum()), "missing_mode": w.missing_mode, "kernel": kernel_name,
-                       "tile_rows": eb.info(5), "ctas": eb.info(6), "n_chosen": int(len(chosen)),
-                       "early_exit": bool(args.early_exit),
+                       "rows_per_task_or_tile": eb.info(5), "ctas": eb.info(6), "n_chosen": int(len(chosen)),
+                       "early_exit": bool(args.early_exit), "rows_this_rank": int(local.shape[0]),
                        "l2": "flushed between steps (256 MiB write)",
-                       "parallelism": f"row-sharded x{world}, 1 all-reduce(int64[n_ind]) per step" if world > 1 else "1 GPU"},
-            "individuals_rows_per_s": w.n_ind * w.rows * world / (ms_per_step * 1e-3),
+                       "parallelism": (f"rows sharded x{world} ({scaling}), 1 all-reduce(int64[n_ind]) per step"
+                                       if world > 1 else "1 GPU")},
+            "individuals_rows_per_s": w.n_ind * (w.rows if scaling == "strong" else w.rows * world) / (ms_per_step * 1e-3),
             "clocks": clk.summary(),
             "e2e": {"value": comparisons / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3},
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
+                    "how": "one ebic_eval_extract call with pinned host buffers: population in, counts + masks out"},
             "gpu_launches": int(launches_per_step * args.steps),
+            "gpu_launches_per_step": int(launches_per_step),
             "roofline": roof,
-            "create_ms": create_ms, "generate_s": gen_s, "wall_s_timed_region": wall_s,
+            "probes": probes.as_dict(),
+            "ms_per_step_without_kernel_events": plain_ms,
+            "create_ms": create_ms, "create_breakdown_ms": breakdown,
+            "pair_table_bytes": eb.info(14), "device_bytes": eb.info(9),
+            "generate_s": gen_s, "wall_s_timed_region": wall_s,
             "step_ms_min_max": [min(step_ms), max(step_ms)],
         }
-        if not args.no_cpu_baseline and world == 1:
+        if fig1 is not None:
+            out["fig1_shapes"] = fig1
+    sh.close()
+    if rank == 0 and world == 1:
+        if not args.no_per_workload:
+            flushed = flush
+            per, keys = [], [k for k in args.per_workload.split(",") if k]
+            for key in keys:
+                t0 = time.time()
+                wk = w if key == args.workload and args.rows is None and args.n_ind is None else W.make_workload(WORKLOADS[key])
+                reps = 5 if wk.comparisons > 1e11 else 20
+                entry, _ = measure_workload(B, key, wk, peaks, peaks_kind, probes, flushed, reps,
+                                            early_exit=args.early_exit)
+                entry["wall_s"] = time.time() - t0
+                per.append(entry)
+                log(json.dumps(entry))
+                if wk is not w:
+                    del wk
+            out["per_workload"] = per
+            out["fig1_shapes"] = [{"workload": e["workload"], "rows": e["rows"], "cols": e["cols"], "n_gpus": 1,
+                                   "step_ms": e["step_ms"], "comparisons_per_s": e["comparisons_per_s"]}
+                                  for e in per if e["workload"].startswith("P")]
+        if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(w, budget_s=args.cpu_budget)
-    eb.close()
     if world > 1:
         dist.destroy_process_group()
     return out
@@ -390,7 +615,7 @@ def oracle_sample(w, n_sample, seed=0):
 def cpu_baseline(w, budget_s=15.0):
     import oracle
     cores = oracle.max_threads()
-    # calibrate on 8 individuals, then size the sample to ~budget_s of CPU work
+    # calibrate on a few individuals, then size the sample to ~budget_s of CPU work
     off, ids, comps = oracle_sample(w, max(8, cores), seed=1)
     t0 = time.perf_counter()
     oracle.eval_fitness(w.matrix, w.missing_mode, off, ids)
@@ -431,9 +656,11 @@ def run_reference(args):
     sample = f"each step: {n} of {w.n_ind} individuals x all {w.rows} rows (fresh sample per step)"
     return {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_t / len(times) * 1e3,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "higher_is_better": True, "scaling": "weak" if args.gpus == 1 else args.scaling, "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind,
-                       "missing_mode": w.missing_mode, "kernel": "cpu oracle (oracle/ebic_oracle.c)"},
+                       "sum_L": int(w.lengths.sum()), "missing_mode": w.missing_mode,
+                       "kernel": "cpu oracle (oracle/ebic_oracle.c)"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -448,21 +675,25 @@ def run_table(args):
     peaks, peaks_kind = measured_peaks()
     torch.cuda.set_device(0)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    l2_gbs = measure_l2_gbs(B)
-    log(f"L2 -> SM read bandwidth (probe): {l2_gbs:.0f} GB/s")
-    rows_out = []
+    probes = Probes(B)
+    log("probes:", json.dumps(probes.as_dict()))
+    rows_out = [{"workload": "-", "kernel": "probes", **probes.as_dict()}]
     names = args.table_workloads.split(",")
     for name in names:
         w = W.make_workload(WORKLOADS[name], rows=args.rows, n_ind=args.n_ind)
         eb = B.Ebic(w.matrix, w.missing_mode)
+        rows_out.append({"workload": w.cfg.name, "kernel": "ebic_create", "create_breakdown_ms": eb.create_breakdown_ms(),
+                         "pair_table_bytes": eb.info(14), "device_bytes": eb.info(9)})
+        log(json.dumps(rows_out[-1]))
         d_off, d_ids = torch.from_numpy(w.offsets).cuda(), torch.from_numpy(w.col_ids).cuda()
         d_counts = torch.empty(w.n_ind, dtype=torch.int64, device="cuda")
         chosen = pick_chosen(w)
         d_chosen = torch.from_numpy(chosen).cuda()
         d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
+        d_mcnt = torch.empty(len(chosen), dtype=torch.int64, device="cuda")
         pstats = pair_stats(w)
-        for kname, ee in (("pairbits", 0), ("pairbits", 1), ("rank8", 0), ("rank8", 1),
-                          ("tiled_f32", 0), ("tiled_f32", 1), ("direct", 0)):
+        for kname, ee in (("pairbits", 0), ("pairbits", 1), ("rank8", 0), ("rank8", 1), ("tiled_f32", 0),
+                          ("tiled_f32", 1), ("union_f32", 0), ("union_f32", 1), ("direct", 0)):
             if kname == "direct" and w.comparisons > 2e10:
                 continue
             try:
@@ -471,34 +702,36 @@ def run_table(args):
             except B.EbicError:
                 continue
             reps = 5 if w.comparisons > 1e11 else 20
-            for _ in range(3):
+
+            def call():
                 eb.eval_fitness(d_off, d_ids, counts=d_counts)
+
+            def step():
+                eb.eval_extract(d_off, d_ids, d_chosen, counts=d_counts, masks=d_masks, mask_counts=d_mcnt)
+
+            for _ in range(3):
+                step()
             eb.set_instrumentation(1)
-            eb.eval_fitness(d_off, d_ids, counts=d_counts)
+            call()
             visits = eb.info(10) if kname != "direct" else eb.ld * int(w.lengths.sum())
             nominal = eb.ld * int((w.lengths - 1).sum() if kname.startswith("pair") else w.lengths.sum())
+            eb.set_instrumentation(0)
+            call_ms, _ = timed_ms(call, reps, flush)            # production: ingest + fitness, chained
+            step_ms, _ = timed_ms(step, reps, flush)            # + extraction of 8 individuals
             eb.set_instrumentation(2)
-            call_ms = []
-            for _ in range(reps):
-                flush.zero_()
-                s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                s.record()
-                eb.eval_fitness(d_off, d_ids, counts=d_counts)
-                e.record()
-                torch.cuda.synchronize()
-                call_ms.append(s.elapsed_time(e))
+            timed_ms(call, reps, flush)
             kernel_ms = eb.info(11) / 1e6
             eb.set_instrumentation(0)
-            # CUDA-graph replay of the whole call (ingest + fitness): separates launch latency
+            # CUDA-graph replay of the whole step: separates launch latency
             graph_ms = None
             try:
                 g = torch.cuda.CUDAGraph()
                 side = torch.cuda.Stream()
                 with torch.cuda.stream(side):
-                    eb.eval_fitness(d_off, d_ids, counts=d_counts, stream=side)
+                    eb.eval_extract(d_off, d_ids, d_chosen, counts=d_counts, masks=d_masks, mask_counts=d_mcnt, stream=side)
                     torch.cuda.synchronize()
                     with torch.cuda.graph(g, stream=side):
-                        eb.eval_fitness(d_off, d_ids, counts=d_counts, stream=side)
+                        eb.eval_extract(d_off, d_ids, d_chosen, counts=d_counts, masks=d_masks, mask_counts=d_mcnt, stream=side)
                 torch.cuda.synchronize()
                 s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 s.record()
@@ -510,18 +743,17 @@ def run_table(args):
             except Exception as ex:                              # noqa: BLE001
                 log("graph replay unavailable:", ex)
                 torch.cuda.synchronize()
-            roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7), l2_gbs=l2_gbs,
+            roof = roofline(kname, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7), probes=probes,
                             pairs=pstats, ld=eb.ld, cols=w.cols)
             rows_out.append({"workload": w.cfg.name, "kernel": kname, "early_exit": ee,
                              "executed_over_nominal_visits": visits / nominal,
-                             "call_ms_median": statistics.median(call_ms),
-                             "kernel_ms": kernel_ms, "graph_replay_ms": graph_ms,
-                             "comparisons_per_s": w.comparisons / (statistics.median(call_ms) * 1e-3),
+                             "call_ms_median": call_ms, "step_ms_median": step_ms,
+                             "kernel_ms": kernel_ms, "graph_replay_step_ms": graph_ms,
+                             "comparisons_per_s": w.comparisons / (step_ms * 1e-3),
                              "comparisons_per_s_kernel": w.comparisons / (kernel_ms * 1e-3),
-                             "individuals_rows_per_s": w.n_ind * w.rows / (statistics.median(call_ms) * 1e-3),
+                             "individuals_rows_per_s": w.n_ind * w.rows / (step_ms * 1e-3),
                              "roofline_bound": roof["bound"], "roofline_frac": roof["frac"], "achieved_gbs": roof["achieved"],
-                             "tile_rows": eb.info(5),
-                             "ctas": eb.info(6)})
+                             "peak_gbs": roof["peak"], "rows_per_task_or_tile": eb.info(5), "ctas": eb.info(6)})
             log(json.dumps(rows_out[-1]))
         # extraction (a7): HBM-bound.  Two sources: the pair table's bit columns (default when it exists;
         # (L-1) * ld/8 bytes read per individual) and the float32 columns (4 * L * ld bytes read).
@@ -532,21 +764,12 @@ def run_table(args):
             if source == "pairbits" and eb.info(14) == 0:
                 continue
             eb.set_extract_source(source == "pairbits")
-            ex_ms = []
-            for _ in range(10):
-                flush.zero_()
-                s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                s.record()
-                eb.extract_rows(d_off, d_ids, d_chosen, masks=d_masks, want_counts=False)
-                e.record()
-                torch.cuda.synchronize()
-                ex_ms.append(s.elapsed_time(e))
+            ex_ms, _ = timed_ms(lambda: eb.extract_rows(d_off, d_ids, d_chosen, masks=d_masks, want_counts=False), 10, flush)
             read_bytes = eb.ld // 8 * Psum if source == "pairbits" else eb.ld * 4 * Lsum
             ex_bytes = read_bytes + len(chosen) * eb.mask_words * 8
             rows_out.append({"workload": w.cfg.name, "kernel": "extract_rows", "source": source,
-                             "call_ms_median": statistics.median(ex_ms),
-                             "hbm_gbs": ex_bytes / (statistics.median(ex_ms) * 1e-3) / 1e9,
-                             "hbm_frac": ex_bytes / (statistics.median(ex_ms) * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                             "call_ms_median": ex_ms, "hbm_gbs": ex_bytes / (ex_ms * 1e-3) / 1e9,
+                             "hbm_frac": ex_bytes / (ex_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                              "n_chosen": int(len(chosen)), "bytes": ex_bytes})
             log(json.dumps(rows_out[-1]))
         eb.set_extract_source(True)
@@ -557,29 +780,36 @@ def run_table(args):
         del w
     out_dir = ROOT / "gpurun_out"
     out_dir.mkdir(exist_ok=True)
-    (out_dir / "table.json").write_text(json.dumps(rows_out, indent=1))
+    (out_dir / args.table_out).write_text(json.dumps(rows_out, indent=1))
     return {"table": rows_out}
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ebic", choices=["ebic", "reference"])
-    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS),
+                    help="default c5: the largest single-GPU configuration of BASELINE.json")
     ap.add_argument("--kernel", default="auto", choices=sorted(KERNELS))
     ap.add_argument("--rows", type=int, default=None, help="override the workload's row count")
     ap.add_argument("--n-ind", type=int, default=None, dest="n_ind")
+    ap.add_argument("--scaling", default="strong", choices=["strong", "weak"],
+                    help="N > 1: strong = one dataset split over the ranks by rows (PAPER.md Fig. 1), weak = every "
+                         "rank holds its own `rows` rows")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-workload", action="store_true", help="skip the per_workload block (N = 1) / fig1_shapes")
+    ap.add_argument("--per-workload", default="c1,c2,c3,c4,c5,p1,p2,p3", help="workloads of the per_workload block")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of CPU work for cpu_baseline")
     ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per launch of the fitness kernel from an ncu --set full capture")
+                    help="dram bytes per launch of the fitness kernel from an ncu --set full capture (overrides the csv)")
     ap.add_argument("--early-exit", type=int, default=0, dest="early_exit",
                     help="1: let warps stop a chromosome once no row can match (fewer executed visits); "
                          "0 (default for the headline): plain work, every column of every chromosome visited")
     ap.add_argument("--table", action="store_true")
     ap.add_argument("--table-workloads", default="c1,c2,c3,c4,c5")
+    ap.add_argument("--table-out", default="table.json")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ebic" and not args.table:
         log("note: fewer than 3 warm-up steps requested; using 3 (timing rules)")

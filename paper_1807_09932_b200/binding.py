@@ -31,32 +31,43 @@ EBIC_KERNEL_DIRECT = 1
 EBIC_KERNEL_TILED_F32 = 2
 EBIC_KERNEL_RANK8 = 3
 EBIC_KERNEL_PAIRBITS = 4
-KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits"}
+EBIC_KERNEL_UNION_F32 = 5
+KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits", 5: "union_f32"}
+# ebic_set_tuning knobs (include/ebic_debug.h)
+TUNE_PB_TASKS_PER_SLOT, TUNE_PB_PREFETCH, TUNE_PB_SMEM_RING, TUNE_SORT, TUNE_PDL, TUNE_UNION_BATCH = range(6)
 
 LIB_PATH = Path(__file__).resolve().parent / "libebic.so"
 
-# every symbol include/ebic.h declares: (restype, argtypes)
+# every symbol include/ebic.h (the boundary) declares: (restype, argtypes)
 _vp, _i32, _i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+_f64p = ctypes.POINTER(ctypes.c_double)
 SYMBOLS = {
     "ebic_create": (ctypes.c_int, [_vp, _i64, _i32, _i32, ctypes.POINTER(_vp)]),
     "ebic_create_sentinel": (ctypes.c_int, [_vp, _i64, _i32, _i32, ctypes.c_float, ctypes.POINTER(_vp)]),
     "ebic_destroy": (ctypes.c_int, [_vp]),
     "ebic_eval_fitness": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _vp]),
     "ebic_extract_rows": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _i32, _vp, _vp, _vp]),
+    "ebic_eval_extract": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _vp, _i32, _vp, _vp, _vp]),
     "ebic_mask_words": (_i64, [_vp]),
     "ebic_status": (ctypes.c_int, [_vp, _vp]),
+    "ebic_read_delimited": (ctypes.c_int, [ctypes.c_char_p, ctypes.c_char, ctypes.POINTER(ctypes.POINTER(ctypes.c_float)),
+                                           ctypes.POINTER(_i64), ctypes.POINTER(_i32)]),
+    "ebic_free_host": (None, [_vp]),
+    "ebic_strerror": (ctypes.c_char_p, [ctypes.c_int]),
+}
+# every symbol include/ebic_debug.h declares (knobs, read-backs, probes for tests and bench.py)
+DEBUG_SYMBOLS = {
     "ebic_set_kernel": (ctypes.c_int, [_vp, _i32]),
     "ebic_set_pairbits": (ctypes.c_int, [_vp, _i32]),
     "ebic_set_extract_source": (ctypes.c_int, [_vp, _i32]),
     "ebic_set_early_exit": (ctypes.c_int, [_vp, _i32]),
+    "ebic_set_tuning": (ctypes.c_int, [_vp, _i32, _i32]),
     "ebic_set_instrumentation": (ctypes.c_int, [_vp, _i32]),
     "ebic_get_info": (_i64, [_vp, _i32]),
     "ebic_debug_read": (ctypes.c_int, [_vp, _i32, _vp, _i64]),
-    "ebic_read_delimited": (ctypes.c_int, [ctypes.c_char_p, ctypes.c_char, ctypes.POINTER(ctypes.POINTER(ctypes.c_float)),
-                                           ctypes.POINTER(_i64), ctypes.POINTER(_i32)]),
-    "ebic_free_host": (None, [_vp]),
-    "ebic_probe_read_bandwidth": (ctypes.c_int, [_i64, _i32, ctypes.POINTER(ctypes.c_double)]),
-    "ebic_strerror": (ctypes.c_char_p, [ctypes.c_int]),
+    "ebic_probe_read_bandwidth": (ctypes.c_int, [_i64, _i32, _f64p]),
+    "ebic_probe_smem_bandwidth": (ctypes.c_int, [_f64p]),
+    "ebic_probe_fsetp_rate": (ctypes.c_int, [_f64p]),
 }
 
 _lib = None
@@ -77,7 +88,7 @@ def load_library() -> ctypes.CDLL:
                 f"{LIB_PATH} is missing: build it with `python -m paper_1807_09932_b200.csrc.build` "
                 "(there is no CPU fallback)")
         lib = ctypes.CDLL(str(LIB_PATH))
-        for name, (res, args) in SYMBOLS.items():
+        for name, (res, args) in {**SYMBOLS, **DEBUG_SYMBOLS}.items():
             fn = getattr(lib, name)
             fn.restype, fn.argtypes = res, args
         _lib = lib
@@ -126,6 +137,14 @@ def ebic_extract_rows(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, chosen_ptr, n
         raise EbicError(st, "ebic_extract_rows")
 
 
+def ebic_eval_extract(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, counts_ptr, chosen_ptr, n_chosen, masks_ptr,
+                      mask_counts_ptr, stream=0) -> None:
+    st = load_library().ebic_eval_extract(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, counts_ptr, chosen_ptr, n_chosen,
+                                          masks_ptr, mask_counts_ptr, stream)
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_eval_extract")
+
+
 def ebic_mask_words(ctx) -> int:
     return int(load_library().ebic_mask_words(ctx))
 
@@ -152,6 +171,12 @@ def ebic_set_extract_source(ctx, use_pairbits: bool) -> None:
 
 def ebic_set_early_exit(ctx, on: bool) -> None:
     load_library().ebic_set_early_exit(ctx, 1 if on else 0)
+
+
+def ebic_set_tuning(ctx, knob: int, value: int) -> None:
+    st = load_library().ebic_set_tuning(ctx, int(knob), int(value))
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_set_tuning")
 
 
 def ebic_set_instrumentation(ctx, on: int) -> None:
@@ -192,6 +217,22 @@ def ebic_probe_read_bandwidth(buffer_bytes: int, reps: int) -> float:
     return out.value
 
 
+def ebic_probe_smem_bandwidth() -> float:
+    out = ctypes.c_double(0.0)
+    st = load_library().ebic_probe_smem_bandwidth(ctypes.byref(out))
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_probe_smem_bandwidth")
+    return out.value
+
+
+def ebic_probe_fsetp_rate() -> float:
+    out = ctypes.c_double(0.0)
+    st = load_library().ebic_probe_fsetp_rate(ctypes.byref(out))
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_probe_fsetp_rate")
+    return out.value
+
+
 def _require_cuda():
     import torch
     if not torch.cuda.is_available():
@@ -214,6 +255,37 @@ def _ptr(a) -> int:
 
 def _is_cuda(a) -> bool:
     return (not isinstance(a, np.ndarray)) and a.is_cuda
+
+
+def _itemsize_kind(a):
+    """(itemsize, kind) of a numpy array or torch tensor; kind 'i' / 'u' / 'f' / '?'."""
+    if isinstance(a, np.ndarray):
+        return a.dtype.itemsize, a.dtype.kind
+    name = str(a.dtype)
+    kind = "f" if ("float" in name or "bfloat" in name) else "u" if "uint" in name else "i" if "int" in name else "?"
+    return a.element_size(), kind
+
+
+def _check_args(where: str, device_index: int, int32_args, int64_args):
+    """The C ABI takes raw addresses, so a wrong dtype or device would be read as garbage: refuse it here.
+    int32_args: offsets / col_ids / chosen (int32); int64_args: counts / masks (int64 or uint64).  All arguments
+    must be of one kind (all CUDA tensors on the context's device, or all host arrays)."""
+    kinds = set()
+    for name, a in list(int32_args.items()) + list(int64_args.items()):
+        if a is None:
+            continue
+        size, kind = _itemsize_kind(a)
+        want = 4 if name in int32_args else 8
+        if kind not in ("i", "u") or size != want or (want == 4 and kind != "i"):
+            raise ValueError(f"{where}: `{name}` must be {'int32' if want == 4 else 'int64 / uint64'}, got {a.dtype}")
+        if _is_cuda(a):
+            if a.device.index != device_index:
+                raise ValueError(f"{where}: `{name}` is on cuda:{a.device.index}, the context on cuda:{device_index}")
+            kinds.add("cuda")
+        else:
+            kinds.add("host")
+    if len(kinds) > 1:
+        raise ValueError(f"{where}: arguments must be all CUDA tensors or all host arrays, not a mix")
 
 
 def _stream_handle(stream) -> int:
@@ -242,6 +314,9 @@ class Ebic:
                 torch.cuda.current_stream().synchronize()      # ebic_create runs on the legacy stream
         self.rows, self.cols = int(matrix.shape[0]), int(matrix.shape[1])
         self.missing_mode = int(missing_mode)
+        self.device_index = int(torch.cuda.current_device())
+        if _is_cuda(matrix) and matrix.device.index != self.device_index:
+            raise ValueError(f"matrix is on cuda:{matrix.device.index}, the current device is cuda:{self.device_index}")
         if sentinel is None:
             self._ctx = ebic_create(_ptr(matrix), self.rows, self.cols, self.missing_mode)
         else:
@@ -275,6 +350,7 @@ class Ebic:
         happen inside the call).
         """
         torch = _require_cuda()
+        _check_args("eval_fitness", self.device_index, {"offsets": offsets, "col_ids": col_ids}, {"counts": counts})
         n_ind = int(offsets.shape[0]) - 1
         n_ids = int(col_ids.shape[0])
         if _is_cuda(offsets):
@@ -288,9 +364,15 @@ class Ebic:
 
     def extract_rows(self, offsets, col_ids, chosen, masks=None, counts=None, want_counts=True, stream=None):
         """(masks [n_chosen][mask_words], counts [n_chosen] or None) for the chosen individuals."""
+        masks, counts = self._extract_outputs("extract_rows", offsets, col_ids, chosen, masks, counts, want_counts)
+        ebic_extract_rows(self._ctx, _ptr(offsets), _ptr(col_ids), int(offsets.shape[0]) - 1, int(col_ids.shape[0]),
+                          _ptr(chosen), int(chosen.shape[0]), _ptr(masks), _ptr(counts), _stream_handle(stream))
+        return masks, counts
+
+    def _extract_outputs(self, where, offsets, col_ids, chosen, masks, counts, want_counts):
         torch = _require_cuda()
-        n_ind = int(offsets.shape[0]) - 1
-        n_ids = int(col_ids.shape[0])
+        _check_args(where, self.device_index, {"offsets": offsets, "col_ids": col_ids, "chosen": chosen},
+                    {"masks": masks, "mask_counts": counts})
         n_chosen = int(chosen.shape[0])
         if _is_cuda(offsets):
             if masks is None:
@@ -302,9 +384,21 @@ class Ebic:
                 masks = np.empty((n_chosen, self.mask_words), dtype=np.uint64)
             if counts is None and want_counts:
                 counts = np.empty(n_chosen, dtype=np.uint64)
-        ebic_extract_rows(self._ctx, _ptr(offsets), _ptr(col_ids), n_ind, n_ids, _ptr(chosen), n_chosen,
-                          _ptr(masks), _ptr(counts), _stream_handle(stream))
         return masks, counts
+
+    def eval_extract(self, offsets, col_ids, chosen, counts=None, masks=None, mask_counts=None, want_counts=True,
+                     stream=None):
+        """ebic_eval_extract: one GA generation -> (counts [n_ind], masks [n_chosen][mask_words], mask_counts)."""
+        torch = _require_cuda()
+        _check_args("eval_extract", self.device_index, {"offsets": offsets, "col_ids": col_ids}, {"counts": counts})
+        n_ind = int(offsets.shape[0]) - 1
+        if counts is None:
+            counts = (torch.empty(n_ind, dtype=torch.int64, device=offsets.device) if _is_cuda(offsets)
+                      else np.empty(n_ind, dtype=np.uint64))
+        masks, mask_counts = self._extract_outputs("eval_extract", offsets, col_ids, chosen, masks, mask_counts, want_counts)
+        ebic_eval_extract(self._ctx, _ptr(offsets), _ptr(col_ids), n_ind, int(col_ids.shape[0]), _ptr(counts),
+                          _ptr(chosen), int(chosen.shape[0]), _ptr(masks), _ptr(mask_counts), _stream_handle(stream))
+        return counts, masks, mask_counts
 
     # -- status / knobs / introspection
     def status(self, stream=None) -> int:
@@ -324,6 +418,14 @@ class Ebic:
 
     def set_instrumentation(self, on: int) -> None:
         ebic_set_instrumentation(self._ctx, on)
+
+    def set_tuning(self, knob: int, value: int) -> None:
+        ebic_set_tuning(self._ctx, knob, value)
+
+    def create_breakdown_ms(self) -> dict:
+        """ebic_create's time by phase (CUDA events inside the library)."""
+        names = ["h2d_transpose_pad", "nan_mask", "pair_table", "rank_tiles", "total"]
+        return {n: self.info(20 + i) / 1e6 for i, n in enumerate(names)}
 
     def info(self, what: int) -> int:
         return ebic_get_info(self._ctx, what)

@@ -15,8 +15,9 @@ from pathlib import Path
 CSRC = Path(__file__).resolve().parent
 PKG = CSRC.parent
 LIB = PKG / "libebic.so"
-SOURCES = [CSRC / "ebic_api.cu", CSRC / "ebic_reader.cu"]
-HEADERS = sorted(CSRC.glob("*.cuh")) + [PKG.parent / "include" / "ebic.h"]
+SOURCES = [CSRC / "ebic_api.cu", CSRC / "ebic_debug.cu", CSRC / "ebic_reader.cu"]
+HEADERS = (sorted(CSRC.glob("*.cuh")) + sorted(CSRC.glob("*.hpp")) +
+           [PKG.parent / "include" / "ebic.h", PKG.parent / "include" / "ebic_debug.h"])
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

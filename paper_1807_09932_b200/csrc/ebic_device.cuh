@@ -93,6 +93,13 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
     return v;
 }
 
+// ---- programmatic dependent launch (sm_90+): a kernel launched with the programmatic-stream-serialization
+// attribute may start while its predecessor on the stream is still running.  griddep_wait() blocks until every
+// prerequisite grid has completed and its memory is visible; griddep_launch_dependents() lets the NEXT kernel's
+// CTAs be scheduled once every CTA of this grid has called it (or exited).  Both are no-ops for plain launches.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ bool is_nan_bits(float v) {
     return (__float_as_uint(v) & 0x7fffffffu) > 0x7f800000u;
 }

@@ -1,4 +1,8 @@
 // extract_kernels.cuh -- SURVEY.md 8(a) row a7: matched-row bitmask (and count) of chosen individuals.
+// Both kernels are launched with programmatic dependent launch.  `overlap` = 0 (ebic_extract_rows): wait for the
+// stream's earlier work before touching anything, so only the launch latency is hidden.  `overlap` = 1
+// (ebic_eval_extract, where the library knows the predecessor is its own fitness kernel and that this kernel
+// reads nothing it writes): run alongside the fitness kernel's last wave and wait for it only before exiting.
 // results are biclusters = rows + columns; the rows of an individual are the rows
 // for which ok(k,r) of include/ebic.h holds.  HBM-bound: reads 4*L bytes per row, writes 1/8 byte.
 //
@@ -21,8 +25,10 @@ extract_rows_kernel(const float* __restrict__ Mc, int64_t ld, int64_t rows, int3
                     const uint32_t* __restrict__ nanmask, const int32_t* __restrict__ offsets,
                     const int32_t* __restrict__ col_ids, int32_t n_ind, int64_t n_ids,
                     const int32_t* __restrict__ chosen, int32_t n_chosen, uint32_t* __restrict__ masks32,
-                    int64_t words32, unsigned long long* __restrict__ counts, int32_t* __restrict__ err)
+                    int64_t words32, unsigned long long* __restrict__ counts, int32_t* __restrict__ err,
+                    int32_t overlap)
 {
+    if (!overlap) griddep_wait();                                  // stream order: everything before this launch is done
     __shared__ int32_t s_ids[kExtractMaxSmemIds];
     __shared__ int32_t s_bad;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -106,6 +112,7 @@ extract_rows_kernel(const float* __restrict__ Mc, int64_t ld, int64_t rows, int3
         }
         __syncthreads();                                           // s_ids / s_bad are reused for the next j
     }
+    if (overlap) griddep_wait();                                   // this grid must not complete before its predecessor
 }
 
 // Extraction from the pair-relation bit columns (loader_kernels.cuh): for L >= 2 the mask IS the AND of
@@ -119,8 +126,9 @@ extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_
                              const int32_t* __restrict__ offsets, const int32_t* __restrict__ col_ids,
                              int32_t n_ind, int64_t n_ids, const int32_t* __restrict__ chosen, int32_t n_chosen,
                              uint32_t* __restrict__ masks32, int64_t words32,
-                             unsigned long long* __restrict__ counts, int32_t* __restrict__ err)
+                             unsigned long long* __restrict__ counts, int32_t* __restrict__ err, int32_t overlap)
 {
+    if (!overlap) griddep_wait();                                  // stream order: everything before this launch is done
     __shared__ int32_t s_pair[kExtractMaxSmemIds];
     __shared__ int32_t s_bad;
     __shared__ unsigned int s_cnt;
@@ -197,6 +205,7 @@ extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_
         }
         __syncthreads();
     }
+    if (overlap) griddep_wait();                                   // this grid must not complete before its predecessor
 }
 
 }  // namespace ebic

@@ -1,5 +1,5 @@
-// fitness_kernels.cuh -- SURVEY.md 8(a) rows a3 (population ingest), a4 (tile staging),
-// a5 (trend predicate) and a6 (count accumulation).
+// fitness_kernels.cuh -- SURVEY.md 8(a) rows a4 (tile staging), a5 (trend predicate) and a6 (count
+// accumulation) on the float32 columns / the 8-bit rank tiles.  (a3, the ingest, is ingest_kernels.cuh.)
 //
 // Definition (include/ebic.h): count[k] = #{ r : AND_i M[r][c_{i+1}] >= M[r][c_i]
 // and, in missing mode, no M[r][c_i] is NaN }.  For L >= 2 an ordered >= is already false on NaN, so
@@ -10,114 +10,6 @@
 
 namespace ebic {
 
-constexpr int kRecPairs = 30;        // pair indices held in an individual's 128-byte record
-
-// ------------------------------------------------------------------------------------------------
-// a3  Population ingest + validation.  One warp per individual.
-//   meta[k] = { slot4, L }   slot4 = index, in 4-entry groups, of the individual's id slot; L = chromosome
-//                            length, or -1 if the individual is invalid.
-//   pids    = int32 ids copied to the slot (entries 4*slot4 ..), padded to a multiple of 4 with the last id
-//             (read by the DIRECT kernel);
-//   pids8   = the same ids as bytes (bytes 4*slot4 ..), written when cols <= 256: the tiled kernels fetch
-//             four ids with one warp-uniform 32-bit load.
-//   The slot of individual k starts at entry (offsets[k] + 3k) & ~3: 4-aligned and disjoint from its
-//   neighbours without a prefix sum.
-//   ppair   = (pair-bit kernels) for each of the L-1 pairs (id_i, id_{i+1}) the offset of its bit column in
-//             the pair table in 16-byte units, (id_i * cols + id_{i+1}) * pair_stride16 as uint32, in the same
-//             slot (entries 4*slot4 ..), padded to a multiple of 4 with the last pair (AND is idempotent).
-//   prec    = (pair-bit kernels) one 128-byte record per individual, read by a warp with ONE coalesced
-//             load: [0] = L (-1 = invalid), [1] = slot4, [2..31] = the first 30 pair offsets, padded with
-//             the last pair.
-//   counts[k] is initialised: rows (L = 0, or L = 1 in mode OFF), non-missing rows of the column
-//             (L = 1, mode ON), else 0 -- the chain kernels then add to it.
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __restrict__ col_ids,
-                         int32_t n_ind, int64_t n_ids, int32_t cols, int64_t rows, int32_t missing_on,
-                         const unsigned long long* __restrict__ nonmissing, int2* __restrict__ meta,
-                         int32_t* __restrict__ pids, uint8_t* __restrict__ pids8, int32_t* __restrict__ ppair,
-                         int32_t* __restrict__ prec, uint32_t pair_stride16,
-                         unsigned long long* __restrict__ counts, int32_t* __restrict__ err,
-                         const uint32_t* __restrict__ warm_PB, int32_t warm_pairs, uint32_t warm_bytes,
-                         unsigned long long* __restrict__ task_counter)
-{
-    if (blockIdx.x == 0 && threadIdx.x == 0 && task_counter != nullptr) *task_counter = 0;   // for the persistent PAIRBITS kernel
-    // one warp per individual, lane i takes ids i, i + 32, ...: the id loads and the slot stores run in parallel
-    const int lane = threadIdx.x & 31;
-    const int32_t k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (k >= n_ind) return;                                      // warp-uniform
-    if (warm_bytes != 0) {
-        // Cold start of the PAIRBITS kernel that follows on the stream: the first rows of every bit column (the
-        // chunks its first wave of CTAs will gather) are requested from HBM now, one slice of columns per warp.
-        const int32_t per = (warm_pairs + n_ind - 1) / n_ind;
-        for (int32_t q = lane; q < per; q += 32) {
-            const int64_t pair = static_cast<int64_t>(k) * per + q;
-            if (pair < warm_pairs)
-                bulk_prefetch_l2(reinterpret_cast<const uint4*>(warm_PB) + pair * pair_stride16, warm_bytes);
-        }
-    }
-    const int32_t b = offsets[k], e = offsets[k + 1];
-    if (b < 0 || e < b || static_cast<int64_t>(e) > n_ids) {
-        if (lane == 0) {
-            meta[k] = make_int2(0, -1);
-            if (prec != nullptr) prec[32ll * k] = -1;
-            counts[k] = 0;
-            atomicMax(err, 5 /* EBIC_ERR_BAD_OFFSETS */);
-        }
-        return;
-    }
-    const int32_t L = e - b;
-    const int32_t npr = max(L - 1, 0);
-    const int64_t slot = (static_cast<int64_t>(b) + 3ll * k) & ~3ll;
-    const bool bytes = pids8 != nullptr;
-    bool bad = false;
-    auto clean = [&](int32_t id) {                               // an id outside [0, cols) becomes 0 in the slots
-        const bool out = id < 0 || id >= cols;
-        bad |= out;
-        return out ? 0 : id;
-    };
-    auto pair_offset = [&](int32_t a, int32_t c) {
-        return static_cast<int32_t>(static_cast<uint32_t>(a * cols + c) * pair_stride16);
-    };
-    for (int32_t i = lane; i < L; i += 32) {
-        const int32_t id = clean(col_ids[b + i]);
-        pids[slot + i] = id;
-        if (bytes) pids8[slot + i] = static_cast<uint8_t>(id);
-        if (ppair != nullptr && i > 0) {
-            const int32_t po = pair_offset(clean(col_ids[b + i - 1]), id);
-            ppair[slot + i - 1] = po;
-            if (i <= kRecPairs) prec[32ll * k + 1 + i] = po;
-        }
-    }
-    bad = __any_sync(0xffffffffu, bad);
-    const int32_t last = (L > 0) ? clean(col_ids[b + L - 1]) : 0;
-    for (int32_t i = L + lane; i < ((L + 3) & ~3); i += 32) {
-        pids[slot + i] = last;
-        if (bytes) pids8[slot + i] = static_cast<uint8_t>(last);
-    }
-    if (ppair != nullptr) {
-        const int32_t last_pair = (L > 1) ? pair_offset(clean(col_ids[b + L - 2]), last) : 0;
-        for (int32_t i = npr + lane; i < ((npr + 3) & ~3); i += 32) ppair[slot + i] = last_pair;
-        for (int32_t i = npr + lane; i < kRecPairs; i += 32) prec[32ll * k + 2 + i] = last_pair;
-        if (lane == 0) {
-            prec[32ll * k] = bad ? -1 : L;
-            prec[32ll * k + 1] = static_cast<int32_t>(slot >> 2);
-        }
-    }
-    if (lane != 0) return;
-    if (bad) {
-        meta[k] = make_int2(static_cast<int32_t>(slot >> 2), -1);
-        counts[k] = 0;
-        atomicMax(err, 4 /* EBIC_ERR_BAD_COLUMN */);
-        return;
-    }
-    meta[k] = make_int2(static_cast<int32_t>(slot >> 2), L);
-    unsigned long long c = 0;
-    if (L == 0) c = static_cast<unsigned long long>(rows);
-    else if (L == 1) c = missing_on ? nonmissing[last] : static_cast<unsigned long long>(rows);
-    counts[k] = c;
-}
-
 // ------------------------------------------------------------------------------------------------
 // DIRECT kernel: one thread per row, column-major global loads, ballot + popc, one global atomic
 // per warp and individual.  Any shape; the simple GPU witness the tiled kernels are diffed against.
@@ -125,9 +17,10 @@ ingest_population_kernel(const int32_t* __restrict__ offsets, const int32_t* __r
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 fitness_direct_kernel(const float* __restrict__ Mc, int64_t ld, const int2* __restrict__ meta,
-                      const int32_t* __restrict__ pids, int32_t n_ind,
+                      const int32_t* __restrict__ col_ids, int32_t n_ind,
                       unsigned long long* __restrict__ counts)
 {
+    griddep_wait();                                              // meta / counts come from the ingest kernel
     const int64_t r = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;   // < ld; padding is NaN
     const int lane = threadIdx.x & 31;
     const int32_t per = (n_ind + gridDim.y - 1) / gridDim.y;
@@ -136,7 +29,7 @@ fitness_direct_kernel(const float* __restrict__ Mc, int64_t ld, const int2* __re
     for (int32_t k = k_begin; k < k_end; ++k) {
         const int2 m = __ldg(&meta[k]);
         if (m.y < 2) continue;
-        const int32_t* ids = pids + 4ll * m.x;
+        const int32_t* ids = col_ids + m.x;                      // validated by the ingest: every id inside [0, cols)
         float prev = Mc[static_cast<int64_t>(__ldg(&ids[0])) * ld + r];
         bool ok = true;
         for (int32_t i = 1; i < m.y; ++i) {
@@ -170,7 +63,8 @@ struct TiledParams {
     int32_t T;                       // rows per tile (multiple of the slab size)
     int64_t n_tiles;                 // ceil(ld / T)
     const int2* meta;                // [n_ind] of this launch's population chunk
-    const uint32_t* idw;             // packed ids, four uint8 per word (pids8 viewed as words)
+    const uint32_t* idrec;           // [n_ind][8]: the first 32 ids of each individual as bytes (ingest_kernels.cuh)
+    const int32_t* col_ids;          // the caller's ids: chromosomes with more than 32 columns continue from them
     int32_t n_ind;                   // individuals in this launch (<= kMaxIndPerLaunch)
     int32_t early_exit;              // stop a chain once no row of the warp's slab group is alive
     unsigned long long* counts;      // [n_ind]
@@ -269,15 +163,29 @@ struct ChainR8 {
     }
 };
 
-// One chromosome on one slab group.  ids arrive four per word; w0 = first word (already loaded),
-// idw points at it.  Full words run branch-free; the (at most two) ragged words go byte by byte.
+// The ids of one individual, four per 32-bit word: words 0..7 come from its id record (one warp-uniform load
+// each), later words are packed on the fly from the caller's int32 ids (valid individual: every id < cols <= 256).
+struct IdWords {
+    const uint32_t* rec;             // idrec + 8 * k
+    const int32_t* ids;              // col_ids + b
+    int32_t L;
+    __device__ __forceinline__ uint32_t word(int32_t j) const {
+        if (j < 8) return __ldg(rec + j);
+        const int32_t i = 4 * j, last = L - 1;
+        return static_cast<uint32_t>(__ldg(ids + min(i, last))) | (static_cast<uint32_t>(__ldg(ids + min(i + 1, last))) << 8) |
+               (static_cast<uint32_t>(__ldg(ids + min(i + 2, last))) << 16) | (static_cast<uint32_t>(__ldg(ids + min(i + 3, last))) << 24);
+    }
+};
+
+// One chromosome on one slab group.  ids arrive four per word; w0 = first word (already loaded).
+// Full words run branch-free; the (at most two) ragged words go byte by byte.
 // Returns the number of matching rows; adds the number of columns actually visited to `steps`.
 template <class C>
-__device__ __forceinline__ int run_chain(C& c, const uint32_t* __restrict__ idw, uint32_t w0, int32_t L,
+__device__ __forceinline__ int run_chain(C& c, const IdWords& iw, uint32_t w0, int32_t L,
                                          bool early_exit, int32_t& steps)
 {
     uint32_t w = w0;
-    uint32_t wn = (L > 4) ? __ldg(idw + 1) : 0u;
+    uint32_t wn = (L > 4) ? iw.word(1) : 0u;
     c.init(id_byte(w, 0));
     int32_t rem = L - 1;                                  // steps still to do; L >= 2
     int32_t done = 1;
@@ -293,7 +201,7 @@ __device__ __forceinline__ int run_chain(C& c, const uint32_t* __restrict__ idw,
     while (rem > 0) {
         if (early_exit && !__any_sync(0xffffffffu, c.alive())) break;
         w = wn;
-        if (rem > 4) wn = __ldg(idw + j + 1);
+        if (rem > 4) wn = iw.word(j + 1);
         ++j;
         if (rem >= 4) {
             c.step(id_byte(w, 0));
@@ -326,12 +234,12 @@ struct ElemR8 {
 // All slabs of the tile for one individual.  Returns matches; `visited` += rows * columns actually visited.
 template <class E>
 __device__ __forceinline__ int eval_individual_on_tile(const typename E::type* tile, int32_t T, int32_t nslabs, int lane,
-                                                        const uint32_t* idw, uint32_t w0, int32_t L, bool early_exit,
+                                                        const IdWords& iw, uint32_t w0, int32_t L, bool early_exit,
                                                         unsigned long long& visited);
 
 template <>
 __device__ __forceinline__ int eval_individual_on_tile<ElemF32>(const float* tile, int32_t T, int32_t nslabs, int lane,
-                                                                const uint32_t* idw, uint32_t w0, int32_t L,
+                                                                const IdWords& iw, uint32_t w0, int32_t L,
                                                                 bool early_exit, unsigned long long& visited)
 {
     int cnt = 0;
@@ -340,7 +248,7 @@ __device__ __forceinline__ int eval_individual_on_tile<ElemF32>(const float* til
         ChainF32 c;
         c.base = smem_u32(tile) + (s * kRowsPerSlabF32 + lane * 4) * 4;
         c.stride = static_cast<uint32_t>(T) * 4;
-        cnt += run_chain(c, idw, w0, L, early_exit, steps);
+        cnt += run_chain(c, iw, w0, L, early_exit, steps);
     }
     visited += static_cast<unsigned long long>(steps) * kRowsPerSlabF32;
     return cnt;
@@ -348,7 +256,7 @@ __device__ __forceinline__ int eval_individual_on_tile<ElemF32>(const float* til
 
 template <>
 __device__ __forceinline__ int eval_individual_on_tile<ElemR8>(const uint8_t* tile, int32_t T, int32_t nslabs, int lane,
-                                                               const uint32_t* idw, uint32_t w0, int32_t L,
+                                                               const IdWords& iw, uint32_t w0, int32_t L,
                                                                bool early_exit, unsigned long long& visited)
 {
     int cnt = 0;
@@ -358,19 +266,19 @@ __device__ __forceinline__ int eval_individual_on_tile<ElemR8>(const uint8_t* ti
         ChainR8<4> c;
         c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
         c.stride = static_cast<uint32_t>(T);
-        cnt += run_chain(c, idw, w0, L, early_exit, steps4);
+        cnt += run_chain(c, iw, w0, L, early_exit, steps4);
     }
     for (; s + 2 <= nslabs; s += 2) {
         ChainR8<2> c;
         c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
         c.stride = static_cast<uint32_t>(T);
-        cnt += run_chain(c, idw, w0, L, early_exit, steps2);
+        cnt += run_chain(c, iw, w0, L, early_exit, steps2);
     }
     for (; s < nslabs; ++s) {
         ChainR8<1> c;
         c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
         c.stride = static_cast<uint32_t>(T);
-        cnt += run_chain(c, idw, w0, L, early_exit, steps1);
+        cnt += run_chain(c, iw, w0, L, early_exit, steps1);
     }
     visited += static_cast<unsigned long long>(4 * steps4 + 2 * steps2 + steps1) * kRowsPerSlabR8;
     return cnt;
@@ -423,8 +331,11 @@ fitness_tiled_kernel(const TiledParams p)
                 bulk_copy_g2s(dst + static_cast<size_t>(c) * p.T, M + static_cast<int64_t>(c) * p.ld + r0, col_bytes,
                               &full[buf]);
         }
+        griddep_wait();                                          // before the count flush below
     } else {
         // ---------------- consumer warps (a5, a6) ----------------
+        griddep_wait();                                          // meta / idrec / counts come from the ingest kernel;
+                                                                 // the producer warp is already staging tiles
         unsigned long long visited = 0;
         const bool early_exit = p.early_exit != 0;
         for (int32_t j = 0; j < ntl; ++j) {
@@ -435,24 +346,25 @@ fitness_tiled_kernel(const TiledParams p)
             const int32_t ka = (j == 0) ? static_cast<int32_t>(pb - t0 * p.n_ind) : 0;
             const int32_t kb = (j == ntl - 1) ? static_cast<int32_t>(pe - t1 * p.n_ind) : p.n_ind;
             const elem_t* tile = tiles + buf * tile_elems;
-            // software pipeline over this warp's individuals: meta two ahead, first id word one ahead
+            // software pipeline over this warp's individuals: meta and first id word one ahead
             int32_t k = ka + warp;
-            int2 m_cur = make_int2(0, 0), m_next = make_int2(0, 0);
+            int2 m_cur = make_int2(0, 0);
             uint32_t w_cur = 0;
             if (k < kb) {
                 m_cur = __ldg(&p.meta[k]);
-                w_cur = __ldg(p.idw + m_cur.x);
+                w_cur = __ldg(p.idrec + 8ll * k);
             }
-            if (k + NCONS < kb) m_next = __ldg(&p.meta[k + NCONS]);
             mbar_wait(&full[buf], (j >> 1) & 1);
             for (; k < kb; k += NCONS) {
                 const int2 m = m_cur;
                 const uint32_t w0 = w_cur;
-                m_cur = m_next;
-                if (k + NCONS < kb) w_cur = __ldg(p.idw + m_cur.x);
-                if (k + 2 * NCONS < kb) m_next = __ldg(&p.meta[k + 2 * NCONS]);
+                if (k + NCONS < kb) {
+                    m_cur = __ldg(&p.meta[k + NCONS]);
+                    w_cur = __ldg(p.idrec + 8ll * (k + NCONS));
+                }
                 if (m.y < 2) continue;
-                int cnt = eval_individual_on_tile<E>(tile, p.T, nslabs, lane, p.idw + m.x, w0, m.y, early_exit, visited);
+                const IdWords iw{p.idrec + 8ll * k, p.col_ids + m.x, m.y};
+                int cnt = eval_individual_on_tile<E>(tile, p.T, nslabs, lane, iw, w0, m.y, early_exit, visited);
                 cnt = __reduce_add_sync(0xffffffffu, cnt);
                 if (lane == 0 && cnt) atomicAdd(&s_cnt[k], static_cast<unsigned int>(cnt));
             }

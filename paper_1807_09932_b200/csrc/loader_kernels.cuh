@@ -111,34 +111,86 @@ rank8_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint8_t* __
     }
 }
 
-// Pair bit columns.  Block = 8 warps; warp w of block (t, y) owns column a = 8*y + w on the 1024-row
-// tile t: it keeps the tile's 1024 values of column a in registers (32 per lane, lane = row % 32) and
-// walks every column b (coalesced 128 B loads, served by L1 for the other 7 warps of the block), turning
-// each 32-row comparison into one ballot word; lane j keeps word j and the 32 words go out as one 128 B
-// store into the bit column of pair (a, b).  grid = (ld / 1024, ceil(cols / 8)).
-__global__ void __launch_bounds__(256)
+// Pair bit columns (a2").  A lane OWNS one output word: lane l of a warp produces the word of rows
+// [1024 t + 32 l, + 32) of the bit column of pair (a, b), so a warp's 32 words are one coalesced 128-byte store
+// and a bit costs one FSETP + one predicated LOP3 -- no ballots.  A warp keeps its two `a` columns in registers
+// (32 consecutive rows per lane each) and walks every column b; the b columns of the tile are staged through
+// shared memory in groups of kPairCB with cp.async, double-buffered, in a padded layout (a lane's 128 bytes start
+// every 144 bytes) that makes the lanes' 16-byte reads conflict-free.
+// Block = 8 warps = 16 `a` columns on one 1,024-row tile; grid = (ld / 1024) * ceil(cols / 16) blocks, the `a`
+// group fastest, so the blocks that share a tile's b columns run together and HBM sees the matrix about once.
+constexpr int kPairCB = 8;                       // b columns per stage
+constexpr int kPairLaneStride = 144;             // bytes between two lanes' 32-row runs in the staged copy
+constexpr int kPairColBytes = 32 * kPairLaneStride;          // 4,608
+constexpr int kPairStageBytes = kPairCB * kPairColBytes;     // 36,864; two stages
+
+__device__ __forceinline__ uint32_t pair_word(const float (&va)[32], const float (&vb)[32]) {
+    uint32_t w = 0;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) w |= (vb[j] >= va[j]) ? (1u << j) : 0u;      // ordered >=: false on NaN
+    return w;
+}
+
+__global__ void __launch_bounds__(256, 2)
 pairbits_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint32_t* __restrict__ PB)
 {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int32_t a = blockIdx.y * 8 + warp;
-    if (a >= cols) return;
-    const int64_t t = blockIdx.x;
-    const float* tile = Mc + t * kPairTileRows + lane;
-    float va[32];
-    const float* ca = tile + static_cast<int64_t>(a) * ld;
-#pragma unroll
-    for (int j = 0; j < 32; ++j) va[j] = ca[32 * j];
+    extern __shared__ __align__(16) unsigned char pb_stage[];   // 2 x kPairStageBytes
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int32_t n_groups = (cols + 15) / 16;
+    const int64_t t = blockIdx.x / n_groups;
+    const int32_t a0 = static_cast<int32_t>(blockIdx.x % n_groups) * 16 + 2 * warp, a1 = a0 + 1;
+    const float* tile = Mc + t * kPairTileRows;
     const int64_t ldw = ld / 32;
-    uint32_t* out = PB + static_cast<int64_t>(a) * cols * ldw + t * 32 + lane;
-    for (int32_t b = 0; b < cols; ++b) {
-        const float* cb = tile + static_cast<int64_t>(b) * ld;
-        unsigned int mine = 0;
+
+    float va0[32], va1[32];
+    {
+        const float4* c0 = reinterpret_cast<const float4*>(tile + static_cast<int64_t>(min(a0, cols - 1)) * ld) + 8 * lane;
+        const float4* c1 = reinterpret_cast<const float4*>(tile + static_cast<int64_t>(min(a1, cols - 1)) * ld) + 8 * lane;
 #pragma unroll
-        for (int j = 0; j < 32; ++j) {
-            const unsigned int w = __ballot_sync(0xffffffffu, cb[32 * j] >= va[j]);
-            if (lane == j) mine = w;
+        for (int q = 0; q < 8; ++q) {
+            const float4 x = __ldg(c0 + q), y = __ldg(c1 + q);
+            va0[4 * q] = x.x; va0[4 * q + 1] = x.y; va0[4 * q + 2] = x.z; va0[4 * q + 3] = x.w;
+            va1[4 * q] = y.x; va1[4 * q + 1] = y.y; va1[4 * q + 2] = y.z; va1[4 * q + 3] = y.w;
         }
-        out[static_cast<int64_t>(b) * ldw] = mine;
+    }
+    const uint32_t stage0 = smem_u32(pb_stage);
+    // thread `tid` copies 16-byte unit `tid` (rows 4 tid .. 4 tid + 3) of each staged column
+    const uint32_t my_dst = (tid >> 3) * kPairLaneStride + (tid & 7) * 16;
+    auto stage = [&](int32_t b0, int buf) {
+#pragma unroll
+        for (int c = 0; c < kPairCB; ++c)
+            if (b0 + c < cols)
+                cp_async16(stage0 + buf * kPairStageBytes + c * kPairColBytes + my_dst,
+                           tile + static_cast<int64_t>(b0 + c) * ld + 4 * tid);
+        cp_async_commit();
+    };
+    uint32_t* out0 = PB + static_cast<int64_t>(a0) * cols * ldw + t * 32 + lane;
+    uint32_t* out1 = PB + static_cast<int64_t>(a1) * cols * ldw + t * 32 + lane;
+    const int32_t n_stage = (cols + kPairCB - 1) / kPairCB;
+    stage(0, 0);
+    for (int32_t s = 0; s < n_stage; ++s) {
+        if (s + 1 < n_stage) {
+            stage((s + 1) * kPairCB, (s + 1) & 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            cp_async_wait_all();
+        }
+        __syncthreads();                                         // every thread's share of stage s has landed
+        const uint32_t src = stage0 + (s & 1) * kPairStageBytes + lane * kPairLaneStride;
+        const int32_t b_end = min(kPairCB, cols - s * kPairCB);
+        for (int32_t c = 0; c < b_end; ++c) {
+            float vb[32];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const uint4 x = lds128(src + c * kPairColBytes + q * 16);
+                vb[4 * q] = __uint_as_float(x.x); vb[4 * q + 1] = __uint_as_float(x.y);
+                vb[4 * q + 2] = __uint_as_float(x.z); vb[4 * q + 3] = __uint_as_float(x.w);
+            }
+            const int64_t b = s * kPairCB + c;
+            if (a0 < cols) out0[b * ldw] = pair_word(va0, vb);
+            if (a1 < cols) out1[b * ldw] = pair_word(va1, vb);
+        }
+        __syncthreads();                                         // stage s may be overwritten by stage s + 2
     }
 }
 

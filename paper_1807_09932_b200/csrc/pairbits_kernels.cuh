@@ -18,22 +18,26 @@
 
 namespace ebic {
 
-constexpr int kRecPairsPb = 30;      // pair indices held in an individual's 128-byte record (see ingest)
+constexpr int kRecPairsPb = 30;      // pair offsets held in an individual's 128-byte record (ingest_kernels.cuh)
 constexpr int kPairbitsStepWords = 256;   // words (x32 rows) a warp covers per step: 2 x LDG.128 per lane and pair
+constexpr int kPairbitsWarps = 2;    // warps per CTA: neighbours in the length-sorted record order
 
 struct PairbitsParams {
     const uint32_t* PB;              // [npairs][ldw]
     int64_t ldw;                     // words per bit column = ld / 32
     int32_t chunk_words;             // words per warp task, multiple of kPairbitsStepWords
     int32_t n_chunks;                // ceil(ldw / chunk_words)
-    const int32_t* prec;             // [n_ind][32] records: L, slot4, 30 pair offsets (pair * ldw / 4, uint32)
-    const int32_t* ppair;            // padded pair-offset slots (chromosomes with more than 31 columns)
+    const uint32_t* prec;            // [n_ind][32] records: L, k, 30 pair offsets (pair * ldw / 4, uint32)
+    const int2* meta;                // [n_ind] {b, L}: only read for chromosomes with more than 31 columns
+    const int32_t* col_ids;          // the caller's ids: pairs beyond the record are formed from them
+    int32_t cols;
+    uint32_t pair_stride16;          // 16-byte units per bit column = ldw / 4
     int32_t n_ind;
     unsigned long long* counts;
     unsigned long long* visits;      // executed (row, pair) visits (instrumented) or nullptr
     int32_t n_pairs;                 // cols * cols bit columns in PB
-    int32_t prefetch_dist;           // tasks of chunk g prefetch a slice of the bit columns of chunk g + dist into L2 (0 = off)
-    unsigned long long* task_counter; // persistent kernel: next task index (zeroed by the ingest kernel)
+    int32_t prefetch_dist;           // tasks of chunk g prefetch a slice of the bit columns of chunk g + dist into L2 (0 = off);
+                                     // chunks 0 .. dist-1 are requested by the kernel's prologue, before it waits for the ingest
 };
 
 __device__ __forceinline__ void and4(uint4& a, const uint4& v) {
@@ -46,7 +50,7 @@ __device__ __forceinline__ bool any4(const uint4& a) { return (a.x | a.y | a.z |
 // first one's address + 512 bytes (an immediate).  Returns the number of pairs visited.
 template <bool EARLY_EXIT, bool FULL, bool SMEM = false>
 __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_a, const uint4* __restrict__ base_b,
-                                                 uint32_t rec, int32_t n0, int32_t npr, const uint32_t* __restrict__ pp,
+                                                 uint32_t rec, int32_t n0, int32_t npr, const PairbitsParams& p, int32_t k,
                                                  int lane, uint4& acc_a, uint4& acc_b, uint32_t ring = 0)
 {
     int32_t done = 0;
@@ -117,8 +121,12 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
     }
     for (int32_t seg = kRecPairsPb; seg < npr; seg += 32) {      // chromosomes with more than 31 columns
         if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) break;
+        // pair offsets beyond the 30 a record holds are formed from the caller's ids (a VALID individual: every
+        // id is inside [0, cols)); pair q = (id_q, id_{q+1}), q + 1 <= L - 1
         const int32_t n = min(32, npr - seg);
-        const uint32_t mine = __ldg(pp + seg + min(lane, n - 1));
+        const int32_t* ids = p.col_ids + __ldg(&p.meta[k]).x + seg + min(lane, n - 1);
+        const uint32_t mine = (static_cast<uint32_t>(__ldg(ids)) * static_cast<uint32_t>(p.cols) +
+                               static_cast<uint32_t>(__ldg(ids + 1))) * p.pair_stride16;
         for (int32_t j = 0; j < n; ++j) {
             const uint4* q0 = base_a + __shfl_sync(0xffffffffu, mine, j);
             const uint4 a0 = __ldg(q0), b0 = __ldg(FULL ? q0 + 32 : base_b + __shfl_sync(0xffffffffu, mine, j));
@@ -129,46 +137,45 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
     return done;
 }
 
-// One warp task: individual k = task % n_ind on row chunk g = task / n_ind.  `rec` = lane's word of k's record.
+// One warp task: record j = task % n_ind (individual k = its word 1) on row chunk g = task / n_ind.
+// `rec` = this lane's word of the record.
 template <bool EARLY_EXIT, bool SMEM>
 __device__ __forceinline__ void pairbits_task(const PairbitsParams& p, int64_t task, uint32_t rec, int lane, uint32_t ring,
                                               unsigned long long& executed)
 {
     const int64_t g = task / p.n_ind;
-    const int32_t k = static_cast<int32_t>(task - g * p.n_ind);
+    const int32_t j = static_cast<int32_t>(task - g * p.n_ind);
     const int64_t w_begin = g * p.chunk_words;
     if (w_begin >= p.ldw) return;                                // warp-uniform
     if (p.prefetch_dist > 0) {
-        // Every bit column of a later chunk is requested from HBM exactly once, by one lane of one task of this
-        // chunk, `prefetch_dist` chunks before the demand loads arrive: those then hit L2.
+        // Every bit column of chunk g + dist is requested from HBM exactly once, by one lane of one task of chunk g:
+        // the demand loads that arrive `dist` chunks later then hit L2.  (Chunks 0 .. dist-1: the kernel's prologue.)
         const int32_t per = (p.n_pairs + p.n_ind - 1) / p.n_ind;     // columns per task
-        const int64_t first = (g == 0) ? 1 : p.prefetch_dist;        // chunk 0 also covers the cold start
-        for (int64_t d = first; d <= p.prefetch_dist; ++d) {
-            const int64_t pw = (g + d) * p.chunk_words;
-            if (pw >= p.ldw) break;
+        const int64_t pw = (g + p.prefetch_dist) * p.chunk_words;
+        if (pw < p.ldw) {
             const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.chunk_words), p.ldw - pw)) * 4u;
             for (int32_t q = lane; q < per; q += 32) {
-                const int64_t pair = static_cast<int64_t>(k) * per + q;
+                const int64_t pair = static_cast<int64_t>(j) * per + q;
                 if (pair < p.n_pairs) bulk_prefetch_l2(p.PB + pair * p.ldw + pw, bytes);
             }
         }
     }
     const int32_t L = static_cast<int32_t>(__shfl_sync(0xffffffffu, rec, 0));
-    if (L < 2) return;
+    if (L < 2) return;                                           // L <= 1: closed form (ingest); -1: invalid
+    const int32_t k = static_cast<int32_t>(__shfl_sync(0xffffffffu, rec, 1));
     const int32_t npr = L - 1;
     const int32_t n0 = min(npr, kRecPairsPb);
-    const uint32_t* pp = reinterpret_cast<const uint32_t*>(p.ppair) + 4ll * __shfl_sync(0xffffffffu, rec, 1);
     const int64_t w_end = min(p.ldw, w_begin + p.chunk_words);
     const uint4* PB4 = reinterpret_cast<const uint4*>(p.PB);
 
     unsigned int cnt = 0;
     // Lane l holds words 4l .. 4l+3 of the step's first 128 words (acc_a) and the same words of its second 128
-    // (acc_b).  Record / ppair entries are the bit columns' offsets into PB in uint4 units (< 2^32, host-checked).
+    // (acc_b).  Record entries are the bit columns' offsets into PB in uint4 units (< 2^32, host-checked).
     const int64_t n_full = (w_end - w_begin) / kPairbitsStepWords;
     const uint4* base = PB4 + (w_begin >> 2) + lane;
     for (int64_t s = 0; s < n_full; ++s, base += kPairbitsStepWords / 4) {
         uint4 acc_a = make_uint4(~0u, ~0u, ~0u, ~0u), acc_b = acc_a;
-        const int32_t done = pairbits_step<EARLY_EXIT, true, SMEM>(base, base, rec, n0, npr, pp, lane, acc_a, acc_b, ring);
+        const int32_t done = pairbits_step<EARLY_EXIT, true, SMEM>(base, base, rec, n0, npr, p, k, lane, acc_a, acc_b, ring);
         cnt += __popc(acc_a.x) + __popc(acc_a.y) + __popc(acc_a.z) + __popc(acc_a.w);
         cnt += __popc(acc_b.x) + __popc(acc_b.y) + __popc(acc_b.z) + __popc(acc_b.w);
         executed += static_cast<unsigned long long>(done) * (kPairbitsStepWords * 32);
@@ -181,7 +188,7 @@ __device__ __forceinline__ void pairbits_task(const PairbitsParams& p, int64_t t
         const uint4* base_b = PB4 + ((vb ? wb : w0) >> 2);
         uint4 acc_a = va ? make_uint4(~0u, ~0u, ~0u, ~0u) : make_uint4(0u, 0u, 0u, 0u);
         uint4 acc_b = vb ? make_uint4(~0u, ~0u, ~0u, ~0u) : make_uint4(0u, 0u, 0u, 0u);
-        const int32_t done = pairbits_step<EARLY_EXIT, false>(base_a, base_b, rec, n0, npr, pp, lane, acc_a, acc_b);
+        const int32_t done = pairbits_step<EARLY_EXIT, false>(base_a, base_b, rec, n0, npr, p, k, lane, acc_a, acc_b);
         cnt += __popc(acc_a.x) + __popc(acc_a.y) + __popc(acc_a.z) + __popc(acc_a.w);
         cnt += __popc(acc_b.x) + __popc(acc_b.y) + __popc(acc_b.z) + __popc(acc_b.w);
         executed += static_cast<unsigned long long>(done) * ((w_end - w0) * 32);
@@ -190,52 +197,32 @@ __device__ __forceinline__ void pairbits_task(const PairbitsParams& p, int64_t t
     if (lane == 0 && cnt) atomicAdd(&p.counts[k], static_cast<unsigned long long>(cnt));
 }
 
-// One task per warp, a CTA of NW warps per NW consecutive tasks: the hardware block scheduler balances the load.
-template <bool EARLY_EXIT, int NW, bool SMEM = false>
-__global__ void __launch_bounds__(NW * 32)
+// One task per warp, a CTA of kPairbitsWarps warps per consecutive tasks: the hardware block scheduler balances
+// the load.  Launched with programmatic dependent launch right behind the ingest kernel: the prologue (the HBM ->
+// L2 requests for the first chunks of every bit column, which depend on the matrix only) overlaps the ingest;
+// griddep_wait() then orders the record loads and the count atomics behind it.
+template <bool EARLY_EXIT, bool SMEM>
+__global__ void __launch_bounds__(kPairbitsWarps * 32)
 fitness_pairbits_kernel(const PairbitsParams p)
 {
-    extern __shared__ __align__(16) unsigned char pb_ring[];     // SMEM: NW x 4 KB landing ring
+    extern __shared__ __align__(16) unsigned char pb_ring[];     // SMEM: one 4 KB landing ring per warp
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int64_t task = static_cast<int64_t>(blockIdx.x) * NW + warp;
+    griddep_launch_dependents();                                 // a dependent extraction launch may be scheduled
+    if (p.prefetch_dist > 0) {
+        // chunks 0 .. dist-1 of every bit column, each requested exactly once, spread over the first CTAs
+        const int64_t n_pro = min(static_cast<int64_t>(gridDim.x), static_cast<int64_t>(p.n_pairs + 63) / 64);
+        if (blockIdx.x < n_pro) {
+            const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.prefetch_dist) * p.chunk_words, p.ldw)) * 4u;
+            for (int64_t pair = static_cast<int64_t>(blockIdx.x) * 64 + threadIdx.x; pair < p.n_pairs; pair += n_pro * 64)
+                bulk_prefetch_l2(p.PB + pair * p.ldw, bytes);
+        }
+    }
+    griddep_wait();
+    const int64_t task = static_cast<int64_t>(blockIdx.x) * kPairbitsWarps + warp;
     if (task >= static_cast<int64_t>(p.n_chunks) * p.n_ind) return;
-    const uint32_t rec = static_cast<uint32_t>(__ldg(p.prec + 32ll * (task % p.n_ind) + lane));   // one coalesced 128 B load
+    const uint32_t rec = __ldg(p.prec + 32ll * (task % p.n_ind) + lane);   // one coalesced 128 B load
     unsigned long long executed = 0;
     pairbits_task<EARLY_EXIT, SMEM>(p, task, rec, lane, SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u, executed);
-    if (lane == 0 && p.visits != nullptr && executed) atomicAdd(p.visits, executed);
-}
-
-// Persistent variant: as many CTAs as fit the GPU; every warp draws task indices from a global counter (zeroed by the
-// ingest kernel) and fetches the NEXT task's index and record while it works on the current one, so neither the
-// counter's nor the record's latency sits on a task's critical path, and a warp never idles behind a longer
-// neighbour of its CTA.
-#ifndef EBIC_PB_PERSIST_MIN_BLOCKS          /* -DEBIC_PB_PERSIST_MIN_BLOCKS=1 lifts the 64-register cap (diagnostic build) */
-#define EBIC_PB_PERSIST_MIN_BLOCKS (32 / NW)
-#endif
-template <bool EARLY_EXIT, int NW, bool SMEM>
-__global__ void __launch_bounds__(NW * 32, EBIC_PB_PERSIST_MIN_BLOCKS)
-fitness_pairbits_persistent_kernel(const PairbitsParams p)
-{
-    extern __shared__ __align__(16) unsigned char pb_ring[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const uint32_t ring = SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u;
-    const int64_t total = static_cast<int64_t>(p.n_chunks) * p.n_ind;
-    auto grab = [&]() {
-        unsigned long long t = 0;
-        if (lane == 0) t = atomicAdd(p.task_counter, 1ull);
-        return static_cast<int64_t>(__shfl_sync(0xffffffffu, t, 0));
-    };
-    int64_t next = grab();
-    uint32_t rec_next = 0;
-    if (next < total) rec_next = static_cast<uint32_t>(__ldg(p.prec + 32ll * (next % p.n_ind) + lane));
-    unsigned long long executed = 0;
-    while (next < total) {
-        const int64_t cur = next;
-        const uint32_t rec = rec_next;
-        next = grab();
-        if (next < total) rec_next = static_cast<uint32_t>(__ldg(p.prec + 32ll * (next % p.n_ind) + lane));
-        pairbits_task<EARLY_EXIT, SMEM>(p, cur, rec, lane, ring, executed);
-    }
     if (lane == 0 && p.visits != nullptr && executed) atomicAdd(p.visits, executed);
 }
 

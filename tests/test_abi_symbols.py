@@ -19,30 +19,43 @@ def lib():
     return binding.load_library()
 
 
-def _declared_functions():
-    text = (ROOT / "include" / "ebic.h").read_text()
+def _declared_functions(header="ebic.h"):
+    text = (ROOT / "include" / header).read_text()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(ebic_[a-z_]+)\s*\(", text)))
 
 
 def test_header_declares_the_boundary():
+    """include/ebic.h is the boundary of SURVEY.md 8(b) plus the ingest side and the one-generation call -- and
+    nothing else: knobs, read-backs and probes live in include/ebic_debug.h."""
     names = _declared_functions()
-    for must in ("ebic_create", "ebic_destroy", "ebic_eval_fitness", "ebic_extract_rows",
-                 "ebic_mask_words", "ebic_status", "ebic_strerror"):
-        assert must in names
+    assert names == sorted(["ebic_create", "ebic_create_sentinel", "ebic_destroy", "ebic_eval_fitness",
+                            "ebic_extract_rows", "ebic_eval_extract", "ebic_mask_words", "ebic_status",
+                            "ebic_strerror", "ebic_read_delimited", "ebic_free_host"])
+    debug = _declared_functions("ebic_debug.h")
+    assert not set(names) & set(debug)
+    assert all(n.startswith(("ebic_set_", "ebic_get_", "ebic_debug_", "ebic_probe_")) for n in debug)
 
 
 def test_library_exports_every_declared_symbol(lib):
     from paper_1807_09932_b200 import binding
-    names = _declared_functions()
-    assert sorted(binding.SYMBOLS) == names          # binding and header list the same calls
-    for name in names:
-        assert hasattr(lib, name), name
+    for header, table in (("ebic.h", binding.SYMBOLS), ("ebic_debug.h", binding.DEBUG_SYMBOLS)):
+        names = _declared_functions(header)
+        assert sorted(table) == names                # binding and header list the same calls
+        for name in names:
+            assert hasattr(lib, name), name
+
+
+def test_library_reads_no_environment_variable():
+    """The configuration is the defaults in csrc/ebic_ctx.hpp, changed only through include/ebic_debug.h."""
+    for path in (ROOT / "paper_1807_09932_b200" / "csrc").glob("*.cu*"):
+        assert "getenv" not in path.read_text(), path
 
 
 def test_no_torch_types_or_oracle_in_the_product():
-    header = (ROOT / "include" / "ebic.h").read_text()
-    assert "torch" not in header and "at::" not in header
+    for name in ("ebic.h", "ebic_debug.h"):
+        header = (ROOT / "include" / name).read_text()
+        assert "torch" not in header and "at::" not in header
     pkg = ROOT / "paper_1807_09932_b200"
     for path in list(pkg.rglob("*.py")) + list(pkg.rglob("*.cu")) + list(pkg.rglob("*.cuh")):
         src = path.read_text()

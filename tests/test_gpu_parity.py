@@ -99,9 +99,17 @@ def test_loader_products(B, rows, cols, nan_rate):
     m = rng.standard_normal((rows, cols), dtype=np.float32)
     m[rng.random((rows, cols)) < nan_rate] = np.nan
     m[0, 0] = np.float32(-0.0) if nan_rate == 0 else m[0, 0]
+    if rows >= 200:                                            # values an inexact compare would get wrong
+        specials = np.array([0.0, -0.0, np.inf, -np.inf, 1e-45, -1e-45, 1.1754942e-38, 1.1754944e-38, 3.4028235e38,
+                             -3.4028235e38, 1.0, np.nextafter(np.float32(1.0), np.float32(2.0))], dtype=np.float32)
+        m[5:5 + 64] = rng.choice(specials, size=(64, cols))
+        m[70:70 + 32, ::3] = np.nan
     for src in (m, dev(m)):                                    # host pointer and device pointer
         with B.Ebic(src, ON) as eb:
             ld = eb.ld
+            assert eb.info(16) == 0                            # no rank tiles while the pair table serves
+            eb.set_kernel(B.EBIC_KERNEL_RANK8)                 # builds them on demand
+            eb.set_kernel(B.EBIC_KERNEL_AUTO)
             assert ld % 1024 == 0 and ld >= rows and ld - rows < 1024
             mc = eb.debug_read(0)
             assert (mc[:, :rows].view(np.uint32) == m.T.view(np.uint32)).all()   # bit-exact transpose
@@ -157,11 +165,12 @@ def test_workload_c5_scaled(B, oracle_mod):
     check_all(B, oracle_mod, w.matrix, w.missing_mode, w.offsets, w.col_ids, np.array(chosen, np.int32))
 
 
-@pytest.mark.parametrize("index,rows,n_ind", [(5, None, 1_600), (6, None, 400), (7, 40_001, 300)])
+@pytest.mark.parametrize("index,rows,n_ind", [(5, None, 1_600), (7, 40_001, 300)])
 def test_paper_shaped_workloads(B, oracle_mod, index, rows, n_ind):
-    """150 / 178 / 310 columns (Table 1 shapes): no rank tiles, at 310 columns
-    no float tile either; every kernel that applies, and both extraction sources, against the oracle.  P1 at
-    full size; P2 with a quarter of the population and P3 at 40,001 rows to keep the oracle to seconds."""
+    """150 / 310 columns (Table 1 shapes): no rank tiles, at 310 columns no
+    float tile of all columns either; every kernel that applies in both early-exit modes, and both extraction
+    sources, against the oracle.  P1 at full size, P3 at 40,001 rows (test_paper_shapes_full_size runs P2 and
+    P3 at full size)."""
     w = W.make_workload(index, rows=rows, n_ind=n_ind)
     chosen = [k for k, _ in w.planted_individuals][:6] + [w.n_ind - 1]
     check_all(B, oracle_mod, w.matrix, w.missing_mode, w.offsets, w.col_ids, np.array(chosen, np.int32))
@@ -285,47 +294,52 @@ def test_file_to_counts(B, oracle_mod, tmp_path):
         assert (gm == wm).all() and (gc == wc).all()
 
 
-@pytest.mark.parametrize("env", [
-    {"EBIC_PB_SMEM": "0"},                                       # register-only landing
-    {"EBIC_PB_WARPS": "8", "EBIC_PB_TASKS_PER_SLOT": "2"},       # 8-warp CTAs, large chunks
-    {"EBIC_PB_WARPS": "1", "EBIC_PB_PREFETCH": "0"},             # 1-warp CTAs, no L2 prefetch
-    {"EBIC_PB_WARM": "3", "EBIC_PB_PREFETCH": "2"},              # warm prefetch from ingest, distance 2
-    {"EBIC_PB_PERSIST": "1"},                                    # persistent warps drawing tasks from a counter
+@pytest.mark.parametrize("knobs", [
+    {"TUNE_PB_SMEM_RING": 0},                                    # register-only landing
+    {"TUNE_PB_TASKS_PER_SLOT": 2, "TUNE_SORT": 0},               # large chunks, population order
+    {"TUNE_PB_TASKS_PER_SLOT": 32, "TUNE_PB_PREFETCH": 0},       # smallest chunks, no L2 prefetch
+    {"TUNE_PB_PREFETCH": 3, "TUNE_PDL": 0},                      # distance 3, plain launches
+    {"TUNE_PDL": 0, "TUNE_SORT": 0, "TUNE_PB_SMEM_RING": 0, "TUNE_PB_PREFETCH": 0},
 ])
-def test_experiment_knobs_keep_parity(env):
-    """The PAIRBITS experiment knobs (environment variables read once per process) select other
-    template instantiations of the kernel; each must still reproduce the oracle bit for bit.  Runs in a child
-    process because the knobs are latched at first use."""
-    import os
-    import subprocess
-    import sys
-    from pathlib import Path
-    root = Path(__file__).resolve().parent.parent
-    code = (
-        "import numpy as np, torch, oracle\n"
-        "from paper_1807_09932_b200 import binding as B, workloads as W\n"
-        "w = W.make_workload(3, rows=70_001, n_ind=700)\n"
-        "st, want = oracle.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)\n"
-        "with B.Ebic(w.matrix, w.missing_mode) as eb:\n"
-        "    eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)\n"
-        "    for ee in (False, True):\n"
-        "        eb.set_early_exit(ee)\n"
-        "        got = eb.eval_fitness(torch.from_numpy(w.offsets).cuda(), torch.from_numpy(w.col_ids).cuda())\n"
-        "        torch.cuda.synchronize()\n"
-        "        assert (got.cpu().numpy().view(np.uint64) == want).all(), ee\n"
-        "print('ok')\n")
-    res = subprocess.run([sys.executable, "-c", code], cwd=root, env={**os.environ, **env}, capture_output=True,
-                         text=True, timeout=600)
-    assert res.returncode == 0 and res.stdout.strip().endswith("ok"), res.stderr[-2000:]
+def test_tuning_knobs_keep_parity(B, oracle_mod, knobs):
+    """ebic_set_tuning (include/ebic_debug.h) selects other launch configurations / template instantiations of the
+    PAIRBITS kernel; each must still reproduce the oracle bit for bit, masks included (the extraction launch is
+    chained to the fitness kernel with and without programmatic dependent launch)."""
+    import torch
+    w = W.make_workload(3, rows=70_001, n_ind=700)
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    chosen = np.array([0, 5, 699], dtype=np.int32)
+    _, wm, wc = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
+    d_off, d_ids, d_ch = dev(w.offsets), dev(w.col_ids), dev(chosen)
+    with B.Ebic(w.matrix, w.missing_mode) as eb:
+        eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)
+        for name, value in knobs.items():
+            eb.set_tuning(getattr(B, name), value)
+        for ee in (False, True):
+            eb.set_early_exit(ee)
+            for _ in range(3):                                   # back to back: exercises the launch chaining
+                c, m, mc = eb.eval_extract(d_off, d_ids, d_ch)
+            torch.cuda.synchronize()
+            assert (c.cpu().numpy().view(np.uint64) == want).all(), ee
+            assert (m.cpu().numpy().view(np.uint64) == wm).all() and (mc.cpu().numpy().view(np.uint64) == wc).all()
+        with pytest.raises(B.EbicError):
+            eb.set_tuning(99, 0)
+        with pytest.raises(B.EbicError):
+            eb.set_tuning(B.TUNE_PB_TASKS_PER_SLOT, 0)
 
 
 def test_probe_read_bandwidth(B):
     """Measurement utility: an L2-resident buffer streams faster than HBM; bad arguments are refused."""
-    l2 = B.ebic_probe_read_bandwidth(64 << 20, 20)
+    l2 = B.ebic_probe_read_bandwidth(48 << 20, 40)
     hbm = B.ebic_probe_read_bandwidth(2 << 30, 2)
     assert 2_000 < hbm < 9_000 and l2 > hbm
     with pytest.raises(B.EbicError):
         B.ebic_probe_read_bandwidth(1024, 1)
+    # the on-chip ceilings of the tiled kernels (SURVEY.md section 7 step 6): 128 B/clk/SM would be ~37 TB/s
+    smem = B.ebic_probe_smem_bandwidth()
+    fsetp = B.ebic_probe_fsetp_rate()
+    assert 10_000 < smem < 60_000, smem
+    assert 2_000 < fsetp < 80_000, fsetp
 
 
 def test_empty_calls(B):
@@ -349,6 +363,19 @@ def test_invalid_population_sticky_error(B, oracle_mod):
     off = np.array([0, 2, 1, 3, 9], dtype=np.int32)
     ids = np.array([0, 1, 2, 3], dtype=np.int32)
     check_all(B, oracle_mod, m, ON, off, ids, expect_status=B.EBIC_ERR_BAD_OFFSETS)
+    # offsets that jump BACKWARDS after an invalid individual (round-1 advisor finding): individuals 0, 2 and 3 are
+    # valid and overlap in col_ids; nothing the ingest writes may depend on the contents of `offsets`
+    off = np.array([0, 10, 5, 8, 12], dtype=np.int32)
+    ids = np.array([0, 1, 2, 3, 4, 3, 2, 1, 0, 4, 2, 3], dtype=np.int32)
+    check_all(B, oracle_mod, m, ON, off, ids, expect_status=B.EBIC_ERR_BAD_OFFSETS)
+    # the same at random: every adjacent pair of random offsets is an individual (half of them invalid), lengths
+    # up to 90 ids (beyond the 32-id / 30-pair records), ranges overlapping freely
+    rng = np.random.default_rng(11)
+    ids = rng.integers(0, 5, 90).astype(np.int32)
+    off = rng.integers(0, 91, 301).astype(np.int32)
+    for mode in (ON, OFF):
+        check_all(B, oracle_mod, m, mode, off, ids, chosen=np.arange(0, 300, 7, dtype=np.int32),
+                  expect_status=B.EBIC_ERR_BAD_OFFSETS)
     # chosen index out of range
     off, ids = csr(good)
     with B.Ebic(m, ON) as eb:
@@ -417,57 +444,139 @@ def test_instrumentation_counts_executed_visits(B):
                     assert seen == nominal_pairs, B.KERNEL_NAMES[kern]
 
 
-# ------------------------------------------------------------------------- full-size C5 (bench config)
-def test_c5_full_size_sampled(B, oracle_mod):
-    """BASELINE.json configs[4] at full size, in the launch configuration bench.py times: a sample of
-    individuals against the oracle one by one, plus properties that hold at any size."""
-    w = W.make_workload(4)
-    d_off, d_ids = dev(w.offsets), dev(w.col_ids)
-    rng = np.random.default_rng(99)
-    sample = np.unique(np.concatenate([[k for k, _ in w.planted_individuals][:16],
-                                       rng.choice(w.n_ind, 32, replace=False)])).astype(np.int32)
-    sub_off, sub_ids = csr([w.col_ids[w.offsets[k]:w.offsets[k + 1]].tolist() for k in sample])
-    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, sub_off, sub_ids)
+def test_eval_extract_one_call(B, oracle_mod):
+    """ebic_eval_extract = ebic_eval_fitness + ebic_extract_rows on one population: device pointers (extraction
+    chained behind the fitness kernel) and host pointers (one upload, one synchronisation); halves skipped when
+    n_ind or n_chosen is 0."""
+    import torch
+    w = W.make_workload(1, rows=9_001, n_ind=500)
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    chosen = np.array([0, 3, 499, 7], dtype=np.int32)
+    _, wm, wc = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
     with B.Ebic(w.matrix, w.missing_mode) as eb:
-        import torch
-        results = {}
-        eb.eval_fitness(d_off, d_ids)
-        assert eb.last_kernel == B.EBIC_KERNEL_PAIRBITS          # what AUTO (and bench.py --workload c5) runs
-        for kern in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_PAIRBITS):
+        for kern in kernels_for(eb, B):
             eb.set_kernel(kern)
-            for early_exit in (False, True):
+            for use_pairbits in (True, False):
+                eb.set_extract_source(use_pairbits)
+                c, m, mc = eb.eval_extract(dev(w.offsets), dev(w.col_ids), dev(chosen))
+                torch.cuda.synchronize()
+                assert (c.cpu().numpy().view(np.uint64) == want).all(), B.KERNEL_NAMES[kern]
+                assert (m.cpu().numpy().view(np.uint64) == wm).all() and (mc.cpu().numpy().view(np.uint64) == wc).all()
+        eb.set_kernel(B.EBIC_KERNEL_AUTO)
+        c, m, mc = eb.eval_extract(w.offsets, w.col_ids, chosen)                 # host buffers
+        assert (c == want).all() and (m == wm).all() and (mc == wc).all()
+        c, m, mc = eb.eval_extract(w.offsets, w.col_ids, chosen, want_counts=False)
+        assert (c == want).all() and (m == wm).all() and mc is None
+        c, m, mc = eb.eval_extract(w.offsets, w.col_ids, chosen[:0])             # no extraction
+        assert (c == want).all() and m.shape == (0, eb.mask_words)
+        assert eb.status() == 0
+
+
+def test_binding_refuses_wrong_dtypes(B):
+    """The C ABI takes raw addresses: the binding must refuse what would be read as garbage (advisor finding)."""
+    w = W.make_workload(0)
+    with B.Ebic(w.matrix, w.missing_mode) as eb:
+        with pytest.raises(ValueError, match="int32"):
+            eb.eval_fitness(w.offsets.astype(np.int64), w.col_ids)
+        with pytest.raises(ValueError, match="int32"):
+            eb.eval_fitness(dev(w.offsets), dev(w.col_ids.astype(np.int64)))
+        with pytest.raises(ValueError, match="int64"):
+            eb.eval_fitness(w.offsets, w.col_ids, counts=np.zeros(w.n_ind, dtype=np.int32))
+        with pytest.raises(ValueError, match="mix"):
+            eb.eval_fitness(dev(w.offsets), w.col_ids)
+        with pytest.raises(ValueError, match="int32"):
+            eb.extract_rows(w.offsets, w.col_ids, np.array([0], dtype=np.int64))
+
+
+# ------------------------------------------------------------------------- row shards on one GPU (SURVEY.md 8(e))
+@pytest.mark.parametrize("world", [2, 3])
+def test_row_shards_through_the_cuda_evaluator(B, oracle_mod, world):
+    """The N-GPU path on one GPU, shard by shard: a ragged matrix cut by `row_partition` (64-row seams, which fall
+    inside the loader's 1,024-row padding), one ebic context per shard, counts summed and mask shards
+    concatenated -- against the UNSHARDED oracle.  What differs from N ranks is only the all-reduce, which the gloo
+    tests cover."""
+    from paper_1807_09932_b200.sharded import row_partition
+    w = W.make_workload(3, rows=5_003, n_ind=300)                # 5,003 = 78 * 64 + 11: ragged last word
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    chosen = np.array([k for k, _ in w.planted_individuals][:4] + [299], dtype=np.int32)
+    _, wm, wc = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
+    total = np.zeros(w.n_ind, dtype=np.uint64)
+    shards, shard_counts = [], np.zeros(len(chosen), dtype=np.uint64)
+    for b, e in row_partition(w.rows, world):
+        assert b % 64 == 0
+        with B.Ebic(np.ascontiguousarray(w.matrix[b:e]), w.missing_mode) as eb:
+            c, m, mc = eb.eval_extract(w.offsets, w.col_ids, chosen)
+            total += c
+            shards.append(m)
+            shard_counts += mc
+    assert (total == want).all()
+    assert (np.concatenate(shards, axis=1) == wm).all() and (shard_counts == wc).all()
+
+
+# ------------------------------------------------------------------------- full sizes against the oracle
+@pytest.mark.parametrize("index", [6, 7])
+def test_paper_shapes_full_size(B, oracle_mod, index):
+    """P2 (54,675 x 178, 1,600 individuals) and P3 (436,444 x 310, 1,600 individuals) at FULL size: every count of
+    the kernel AUTO picks and of the float32 kernels that apply, and the masks of 9 individuals from both
+    extraction sources, word for word against the oracle."""
+    import torch
+    w = W.make_workload(index)
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    chosen = np.array([k for k, _ in w.planted_individuals][:8] + [w.n_ind - 1], dtype=np.int32)
+    _, wm, wc = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
+    d_off, d_ids = dev(w.offsets), dev(w.col_ids)
+    with B.Ebic(w.matrix, w.missing_mode) as eb:
+        assert eb.kernel == B.EBIC_KERNEL_PAIRBITS
+        for kern in kernels_for(eb, B):
+            eb.set_kernel(kern)
+            got = eb.eval_fitness(d_off, d_ids)
+            torch.cuda.synchronize()
+            assert (got.cpu().numpy().view(np.uint64) == want).all(), B.KERNEL_NAMES[kern]
+        eb.set_kernel(B.EBIC_KERNEL_AUTO)
+        for use_pairbits in (True, False):
+            eb.set_extract_source(use_pairbits)
+            gm, gc = gpu_masks(eb, w.offsets, w.col_ids, chosen)
+            assert (gm == wm).all() and (gc == wc).all(), use_pairbits
+        assert eb.status() == 0
+
+
+def test_c5_full_size(B, oracle_mod):
+    """BASELINE.json configs[4] at FULL size (16,777,216 rows x 32 columns, 4,096 individuals), in the launch
+    configuration bench.py times: the oracle evaluates ALL 4,096 individuals (about 5.5e11 comparisons, 1-2
+    minutes on the box's host cores) and every GPU kernel's counts are compared with it element by element; the
+    masks of 8 planted individuals from both extraction sources are compared with oracle.extract_rows word for
+    word (BASELINE.json north_star: "bit-exact fitness counts and row bitmasks vs the oracle on all five configs")."""
+    import torch
+    w = W.make_workload(4)
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    assert st == 0
+    chosen = np.array([k for k, _ in w.planted_individuals][:8], dtype=np.int32)
+    _, wm, wc = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
+    assert (wc == want[chosen]).all()
+    d_off, d_ids = dev(w.offsets), dev(w.col_ids)
+    with B.Ebic(w.matrix, w.missing_mode) as eb:
+        eb.set_early_exit(False)                                 # bench.py's headline configuration
+        got = eb.eval_fitness(d_off, d_ids)
+        torch.cuda.synchronize()
+        assert eb.last_kernel == B.EBIC_KERNEL_PAIRBITS          # what AUTO (and bench.py) runs on C5
+        assert (got.cpu().numpy().view(np.uint64) == want).all()
+        for kern in (B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_DIRECT):
+            eb.set_kernel(kern)
+            for early_exit in ((True,) if kern == B.EBIC_KERNEL_DIRECT else (True, False)):
                 eb.set_early_exit(early_exit)
                 c = eb.eval_fitness(d_off, d_ids)
                 torch.cuda.synchronize()
-                results[kern] = c.cpu().numpy().view(np.uint64)
-                assert (results[kern][sample] == want).all(), (B.KERNEL_NAMES[kern], early_exit)
-        for kern in results:
-            assert (results[kern] == results[B.EBIC_KERNEL_RANK8]).all(), B.KERNEL_NAMES[kern]
-        counts = results[B.EBIC_KERNEL_RANK8]
-        # properties: planted rows are a subset; popcount(mask) == count; tail bits zero
-        chosen = np.array([k for k, _ in w.planted_individuals][:4], dtype=np.int32)
-        gm, gc = gpu_masks(eb, w.offsets, w.col_ids, chosen)
-        for slot, (k, b) in enumerate(w.planted_individuals[:4]):
-            bits = mask_to_bits(gm[slot], w.rows)
-            assert bits[w.planted[b].clean_rows].all()
-            assert int(bits.sum()) == int(gc[slot]) == int(counts[k])
-        # closed form on uniformly random individuals: count ~ Binomial(rows, (1-p)^L / L!) on the rows
-        # that are iid; planted rows (sorted in some column order) can shift it either way, by at most
-        # the number of planted rows in biclusters sharing a column with the individual.
-        import math
-        p = w.cfg.nan_rate
-        first_random = 4 * len(w.planted)
-        for k in range(first_random, first_random + 200):
-            L = int(w.lengths[k])
-            if L > 5:
-                continue
-            chrom = set(w.col_ids[w.offsets[k]:w.offsets[k + 1]].tolist())
-            affected = sum(b.rows.size for b in w.planted if chrom & set(b.order.tolist()))
-            q = (1 - p) ** L / math.factorial(L)
-            sigma = math.sqrt(w.rows * q * (1 - q))
-            assert abs(int(counts[k]) - w.rows * q) <= 6 * sigma + affected, (k, L, int(counts[k]), w.rows * q)
-        # third witness on the whole population: the simple DIRECT kernel
-        eb.set_kernel(B.EBIC_KERNEL_DIRECT)
-        c = eb.eval_fitness(d_off, d_ids)
+                got = c.cpu().numpy().view(np.uint64)
+                assert (got == want).all(), (B.KERNEL_NAMES[kern], early_exit, np.flatnonzero(got != want)[:10])
+        eb.set_kernel(B.EBIC_KERNEL_AUTO)
+        for use_pairbits in (True, False):
+            eb.set_extract_source(use_pairbits)
+            gm, gc = gpu_masks(eb, w.offsets, w.col_ids, chosen)
+            assert (gm == wm).all() and (gc == wc).all(), use_pairbits
+        # the fused call, as bench.py's step issues it
+        c, m, mc = eb.eval_extract(d_off, d_ids, dev(chosen))
         torch.cuda.synchronize()
-        assert (c.cpu().numpy().view(np.uint64) == counts).all()
+        assert (c.cpu().numpy().view(np.uint64) == want).all() and (m.cpu().numpy().view(np.uint64) == wm).all()
+        for slot, (k, b) in enumerate(w.planted_individuals[:8]):
+            assert mask_to_bits(wm[slot], w.rows)[w.planted[b].clean_rows].all()      # planted rows are matched
+        assert eb.status() == 0

@@ -35,14 +35,14 @@ def _free_port() -> int:
         return s.getsockname()[1]
 
 
-def _worker(rank: int, world: int, port: int, out_dir: str):
+def _worker(rank: int, world: int, port: int, out_dir: str, rows: int = 3001):
     import torch
     import torch.distributed as dist
     import oracle
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
-        w = W.make_workload(1, rows=3001, n_ind=120)             # ragged: 3001 = 46*64 + 57
+        w = W.make_workload(1, rows=rows, n_ind=120)             # ragged: 3001 = 46*64 + 57
         chosen = np.array([0, 4, 7, 119], dtype=np.int32)
         b, e = row_partition(w.rows, world)[rank]
         local = np.ascontiguousarray(w.matrix[b:e])
@@ -54,19 +54,20 @@ def _worker(rank: int, world: int, port: int, out_dir: str):
             return oracle.extract_rows(local, w.missing_mode, off, ids, ch)[1]
 
         sh = ShardedEbic(w.rows, rank, world, local_eval, local_extract)
-        counts = sh.eval_fitness(w.offsets, w.col_ids)
-        masks = sh.gather_masks(sh.extract_rows(w.offsets, w.col_ids, chosen))
+        counts, shard = sh.step(w.offsets, w.col_ids, chosen)
+        assert shard.shape == (len(chosen), sh.local_words)
+        masks = sh.gather_masks(shard)
         np.save(os.path.join(out_dir, f"counts{rank}.npy"), counts.numpy())
         np.save(os.path.join(out_dir, f"masks{rank}.npy"), masks.numpy())
     finally:
         dist.destroy_process_group()
 
 
-def test_world_size_2_gloo_matches_unsharded_oracle(tmp_path, oracle_mod):
+@pytest.mark.parametrize("world,rows", [(2, 3001), (3, 100)])    # (3, 100): two 64-row words, rank 2 holds no rows
+def test_gloo_matches_unsharded_oracle(tmp_path, oracle_mod, world, rows):
     import torch.multiprocessing as mp
-    world = 2
-    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
-    w = W.make_workload(1, rows=3001, n_ind=120)
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path), rows), nprocs=world, join=True)
+    w = W.make_workload(1, rows=rows, n_ind=120)
     chosen = np.array([0, 4, 7, 119], dtype=np.int32)
     _, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
     _, want_masks, _ = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
