@@ -84,7 +84,8 @@ int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
  *   on/off, 14 bytes of the pair table (0 = absent), 15 kernel of the last fitness launch (0 = none yet),
  *   16 bytes of the rank tiles (0 = absent),
  *   20..24 ebic_create's time in ns, CUDA events on the legacy stream: 20 host-to-device copy + transpose +
- *   padding, 21 NaN bitmask, 22 pair table (allocation + kernel), 23 rank tiles, 24 all of it.
+ *   padding, 21 NaN bitmask, 22 pair-table kernel, 23 rank-tile kernel (22 / 23 also when built later on demand;
+ *   allocations excluded), 24 all of ebic_create including the allocations.
  * Returns -1 for NULL / unknown `what`.
  */
 int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);

@@ -6,6 +6,7 @@
 
 #include <cuda_runtime.h>
 #include <algorithm>
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -17,6 +18,7 @@
 #include "ingest_kernels.cuh"
 #include "loader_kernels.cuh"
 #include "pairbits_kernels.cuh"
+#include "union_kernels.cuh"
 
 using namespace ebic;
 
@@ -119,6 +121,23 @@ int32_t tile_rows_r8(const ebic_ctx* ctx, int32_t n_ind_launch) {
     if (T == 0) T = pick_tile_rows(ctx, 1, kRowsPerSlabR8, 4096, n_ind_launch);
     return T;
 }
+// UNION_F32: columns a staged 128-row tile can hold, double-buffered.
+int32_t union_cap(const ebic_ctx* ctx) {
+    if (ctx->cols > kUnionMaxCols) return 0;
+    const int64_t avail = static_cast<int64_t>(ctx->smem_optin) - kSmemHeader;
+    return static_cast<int32_t>(std::min<int64_t>(std::min<int64_t>(avail / (2ll * kUnionTileRows * 4), 256), ctx->cols));
+}
+// Individuals per batch: the largest batch whose expected union, cols * (1 - exp(-batch * mean_L / cols)), still
+// fits 85 % of the tile (the plan kernel evaluates whatever does not fit from global memory).
+int32_t union_batch(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
+    if (ctx->union_batch > 0) return ctx->union_batch;
+    const double cap = 0.85 * union_cap(ctx), cols = ctx->cols;
+    const double mean_l = std::max(2.0, static_cast<double>(n_ids) / std::max(n_ind, 1));
+    double b = 128.0;
+    if (cap < cols) b = -cols / mean_l * std::log(1.0 - cap / cols);
+    return static_cast<int32_t>(std::max(4.0, std::min(128.0, b)));
+}
+
 int32_t tile_rows(const ebic_ctx* ctx, int32_t kernel, int32_t n_ind_launch) {
     return kernel == EBIC_KERNEL_RANK8 ? tile_rows_r8(ctx, n_ind_launch) : tile_rows_f32(ctx, n_ind_launch);
 }
@@ -164,6 +183,7 @@ bool kernel_applies(const ebic_ctx* ctx, int32_t kernel) {
         case EBIC_KERNEL_TILED_F32: return tile_rows_f32(ctx, 64) > 0;
         case EBIC_KERNEL_RANK8: return tile_rows_r8(ctx, 64) > 0;
         case EBIC_KERNEL_PAIRBITS: return ctx->PB != nullptr;
+        case EBIC_KERNEL_UNION_F32: return union_cap(ctx) >= 2;
         default: return false;
     }
 }
@@ -172,7 +192,8 @@ int32_t resolve_kernel(const ebic_ctx* ctx, int32_t /*n_ind_launch*/) {
     if (ctx->kernel_request != EBIC_KERNEL_AUTO) return ctx->kernel_request;
     if (ctx->PB) return EBIC_KERNEL_PAIRBITS;
     if (ctx->Rk && kernel_applies(ctx, EBIC_KERNEL_RANK8)) return EBIC_KERNEL_RANK8;
-    if (kernel_applies(ctx, EBIC_KERNEL_TILED_F32)) return EBIC_KERNEL_TILED_F32;
+    if (kernel_applies(ctx, EBIC_KERNEL_TILED_F32)) return EBIC_KERNEL_TILED_F32;   // every column fits a tile
+    if (kernel_applies(ctx, EBIC_KERNEL_UNION_F32)) return EBIC_KERNEL_UNION_F32;   // wider: a batch's column union
     return EBIC_KERNEL_DIRECT;
 }
 
@@ -180,9 +201,9 @@ int32_t resolve_kernel(const ebic_ctx* ctx, int32_t /*n_ind_launch*/) {
 int build_rank_tiles(ebic_ctx* ctx) {
     if (ctx->Rk) return EBIC_OK;
     if (ctx->cols > kMaxColsRank8) return EBIC_ERR_ARG;
-    BuildTimer timer(&ctx->create_ms[3]);
     int st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->Rk), ctx->ld * ctx->cols);
     if (st) return st;
+    BuildTimer timer(&ctx->create_ms[3]);                        // the kernel, not the allocation
     const size_t smem = static_cast<size_t>(ctx->cols) * 256 * 5;
     EBIC_TRY(cudaFuncSetAttribute(rank8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
     rank8_kernel<<<static_cast<unsigned>(ctx->ld / 256), 256, smem>>>(ctx->Mc, ctx->ld, ctx->cols, ctx->Rk);
@@ -201,12 +222,12 @@ int build_pairbits(ebic_ctx* ctx) {
     const int64_t blocks = (ctx->ld / kPairTileRows) * ((ctx->cols + 15) / 16);
     if (blocks > 0x7fffffffll) return EBIC_ERR_ARG;
     const dim3 grid(static_cast<unsigned>(blocks));
-    BuildTimer timer(&ctx->create_ms[2]);
     int st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->PB), bytes);
     if (st) return st;
     ctx->pb_bytes = bytes;
+    BuildTimer timer(&ctx->create_ms[2]);                        // the kernel, not the allocation
     EBIC_TRY(cudaFuncSetAttribute(pairbits_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * kPairStageBytes));
-    pairbits_kernel<<<grid, 256, 2 * kPairStageBytes>>>(ctx->Mc, ctx->ld, ctx->cols, ctx->PB);
+    pairbits_kernel<<<grid, 256, 2 * kPairStageBytes>>>(ctx->Mc, ctx->nanmask, ctx->ld, ctx->cols, ctx->PB);
     ctx->launches++;
     st = cuda_status(cudaGetLastError());
     if (!st) st = cuda_status(cudaDeviceSynchronize());
@@ -316,8 +337,17 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     }
     int st = grow(ctx, reinterpret_cast<void**>(&ctx->meta), &ctx->meta_cap, static_cast<int64_t>(n_ind) * 8);
     if (st) return st;
-    if (tiled) {
+    const bool by_union = kernel0 == EBIC_KERNEL_UNION_F32;
+    UnionParams up;
+    if (tiled || by_union) {
         st = grow(ctx, reinterpret_cast<void**>(&ctx->idrec), &ctx->idrec_cap, 32ll * n_ind);
+        if (st) return st;
+    }
+    if (by_union) {
+        up.batch = union_batch(ctx, n_ind, n_ids);
+        up.n_batches = (n_ind + up.batch - 1) / up.batch;
+        up.u_cap = union_cap(ctx);
+        st = grow(ctx, reinterpret_cast<void**>(&ctx->ubatch), &ctx->ubatch_cap, 4ll * up.n_batches * (up.u_cap + 1));
         if (st) return st;
     }
     if (kernel0 == EBIC_KERNEL_PAIRBITS) {
@@ -344,6 +374,25 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     ingest_population_kernel<<<(n_ind + kIngestBlock - 1) / kIngestBlock, 256, 0, stream>>>(ip);
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());
+
+    if (by_union) {                                         // a3, second half: the batches' column unions and local ids
+        up.Mc = ctx->Mc;
+        up.ld = ctx->ld;
+        up.cols = ctx->cols;
+        up.n_ind = n_ind;
+        up.meta = ctx->meta;
+        up.col_ids = col_ids;
+        up.ucount = ctx->ubatch;
+        up.ucols = ctx->ubatch + up.n_batches;
+        up.urec = ctx->idrec;
+        up.early_exit = ctx->early_exit;
+        up.counts = counts;
+        up.visits = ctx->count_visits ? ctx->d_visits : nullptr;
+        const size_t plan_smem = 8ull * ((ctx->cols + 31) / 32);
+        ctx->launches++;
+        EBIC_TRY(launch_pdl(union_plan_kernel, dim3(static_cast<unsigned>(up.n_batches)), dim3(256), plan_smem, stream,
+                            ctx->pdl != 0, up));
+    }
 
     // With kernel timing on, an event sits between the ingest and the fitness kernel, so the two cannot overlap:
     // the timed kernel then includes its whole prologue (a conservative figure).
@@ -373,6 +422,16 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
             if (st) return st;
             pdl = false;                                  // only the first launch directly follows the ingest
         }
+    } else if (by_union) {
+        const size_t smem = union_smem_bytes(up.u_cap);
+        auto kern = fitness_union_kernel<kUnionCons>;
+        EBIC_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+        const int64_t P = (ctx->ld / kUnionTileRows) * up.n_batches;
+        const int64_t grid = std::min<int64_t>(ctx->sm_count, P);
+        ctx->last_grid = static_cast<int32_t>(grid);
+        ctx->last_T = kUnionTileRows;
+        ctx->launches++;
+        EBIC_TRY(launch_pdl(kern, dim3(static_cast<unsigned>(grid)), dim3((kUnionCons + 1) * 32), smem, stream, pdl, up));
     } else {
         const int64_t gx = ctx->ld / 256;
         int64_t gy = std::max<int64_t>(1, (8ll * ctx->sm_count + gx - 1) / gx);

@@ -256,7 +256,7 @@ int ebic_probe_fsetp_rate(double* gcompares_per_s) {
     ProbeTimer t;
     st = cuda_status(cudaMalloc(&sink, 4));
     if (!st) st = t.init();
-    const int32_t iters = 8192;
+    const int32_t iters = 2048;
     const int grid = sms * 8;
     double best = 0.0;
     for (int pass = 0; pass < 4 && !st; ++pass) {
@@ -265,7 +265,7 @@ int ebic_probe_fsetp_rate(double* gcompares_per_s) {
         probe_fsetp_kernel<<<grid, 256>>>(iters, 1.0f, 2.0f, sink);
         st = t.end(&ms);
         if (!st && pass > 0 && ms > 0.f)
-            best = std::max(best, static_cast<double>(grid) * 256.0 * iters * 16 / (ms * 1e-3) / 1e9);
+            best = std::max(best, static_cast<double>(grid) * 256.0 * iters * 48 / (ms * 1e-3) / 1e9);
     }
     if (!st) *gcompares_per_s = best;
     cudaFree(sink);

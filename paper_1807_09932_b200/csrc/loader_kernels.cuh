@@ -113,7 +113,13 @@ rank8_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint8_t* __
 
 // Pair bit columns (a2").  A lane OWNS one output word: lane l of a warp produces the word of rows
 // [1024 t + 32 l, + 32) of the bit column of pair (a, b), so a warp's 32 words are one coalesced 128-byte store
-// and a bit costs one FSETP + one predicated LOP3 -- no ballots.  A warp keeps its two `a` columns in registers
+// -- no ballots.  A bit costs two instructions on two different pipes: d = b - a (FADD) and a funnel shift that
+// moves d's sign bit into the word (SHF).  Why the sign of the float32 difference IS the ordered comparison
+// (DESIGN.md section 5): for two numbers b - a is negative iff b < a -- the subtraction is exact in sign (no
+// flush-to-zero: two distinct floats never give 0), inf - inf is the positive canonical NaN (">=" holds), and
+// the one wrong case, (-0) - (+0) = -0, is removed by turning every zero of the `a` column into -0 once
+// ((+0) - (-0) = (-0) - (-0) = +0).  A NaN operand is taken from the loader's NaN bitmask (one 128-byte load per
+// column and warp): the word is ANDed with "both present".  A warp keeps its two `a` columns in registers
 // (32 consecutive rows per lane each) and walks every column b; the b columns of the tile are staged through
 // shared memory in groups of kPairCB with cp.async, double-buffered, in a padded layout (a lane's 128 bytes start
 // every 144 bytes) that makes the lanes' 16-byte reads conflict-free.
@@ -124,15 +130,17 @@ constexpr int kPairLaneStride = 144;             // bytes between two lanes' 32-
 constexpr int kPairColBytes = 32 * kPairLaneStride;          // 4,608
 constexpr int kPairStageBytes = kPairCB * kPairColBytes;     // 36,864; two stages
 
+// `va`: zeros already turned into -0.  Returns bit j = !(vb[j] < va[j]) for numbers (garbage where either is NaN).
 __device__ __forceinline__ uint32_t pair_word(const float (&va)[32], const float (&vb)[32]) {
     uint32_t w = 0;
 #pragma unroll
-    for (int j = 0; j < 32; ++j) w |= (vb[j] >= va[j]) ? (1u << j) : 0u;      // ordered >=: false on NaN
-    return w;
+    for (int j = 31; j >= 0; --j) w = __funnelshift_l(__float_as_uint(vb[j] - va[j]), w, 1);   // w = w << 1 | sign
+    return ~w;
 }
 
 __global__ void __launch_bounds__(256, 2)
-pairbits_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint32_t* __restrict__ PB)
+pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanmask, int64_t ld, int32_t cols,
+                uint32_t* __restrict__ PB)
 {
     extern __shared__ __align__(16) unsigned char pb_stage[];   // 2 x kPairStageBytes
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -152,7 +160,16 @@ pairbits_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint32_t
             va0[4 * q] = x.x; va0[4 * q + 1] = x.y; va0[4 * q + 2] = x.z; va0[4 * q + 3] = x.w;
             va1[4 * q] = y.x; va1[4 * q + 1] = y.y; va1[4 * q + 2] = y.z; va1[4 * q + 3] = y.w;
         }
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {                           // +0 / -0 -> -0 (see the header)
+            va0[j] = (va0[j] == 0.0f) ? -0.0f : va0[j];
+            va1[j] = (va1[j] == 0.0f) ? -0.0f : va1[j];
+        }
     }
+    // "present" words of this lane's 32 rows: the NaN bitmask is [cols][ld / 32], bit set = missing
+    const uint32_t* nan_t = nanmask + t * 32 + lane;
+    const uint32_t pa0 = ~__ldg(nan_t + static_cast<int64_t>(min(a0, cols - 1)) * ldw);
+    const uint32_t pa1 = ~__ldg(nan_t + static_cast<int64_t>(min(a1, cols - 1)) * ldw);
     const uint32_t stage0 = smem_u32(pb_stage);
     // thread `tid` copies 16-byte unit `tid` (rows 4 tid .. 4 tid + 3) of each staged column
     const uint32_t my_dst = (tid >> 3) * kPairLaneStride + (tid & 7) * 16;
@@ -187,8 +204,9 @@ pairbits_kernel(const float* __restrict__ Mc, int64_t ld, int32_t cols, uint32_t
                 vb[4 * q + 2] = __uint_as_float(x.z); vb[4 * q + 3] = __uint_as_float(x.w);
             }
             const int64_t b = s * kPairCB + c;
-            if (a0 < cols) out0[b * ldw] = pair_word(va0, vb);
-            if (a1 < cols) out1[b * ldw] = pair_word(va1, vb);
+            const uint32_t pb = ~__ldg(nan_t + b * ldw);
+            if (a0 < cols) out0[b * ldw] = pair_word(va0, vb) & pa0 & pb;
+            if (a1 < cols) out1[b * ldw] = pair_word(va1, vb) & pa1 & pb;
         }
         __syncthreads();                                         // stage s may be overwritten by stage s + 2
     }

@@ -11,6 +11,13 @@ namespace ebic {
 
 constexpr int kProbeUnroll = 16;
 
+// volatile: ptxas may neither drop a repeated read of the same shared address nor narrow the vector
+__device__ __forceinline__ uint4 probe_lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.volatile.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+
 // Thread i of the grid reads vectors i, i + S, i + 2S, ... (S = grid size) of buf[0, n_vec): every pass reads the
 // whole buffer exactly once, each warp 512 contiguous bytes per load.  n_vec must be a multiple of kProbeUnroll * S.
 __global__ void __launch_bounds__(256)
@@ -33,8 +40,9 @@ probe_read_kernel(const uint4* __restrict__ buf, int64_t n_vec, int32_t reps, un
     if (acc == 0x9e3779b9u) *sink = acc;                        // keeps the loads alive
 }
 
-// 1,024 threads, 64 KB of shared memory; lane l of every warp reads 16 bytes at (l * 16 + k * 512) mod 64 KB:
-// a warp's request is 512 contiguous bytes = 4 conflict-free wavefronts.  8 independent LDS.128 per iteration.
+// 1,024 threads, 64 KB of shared memory; lane l of warp w reads 16 bytes at w * 2048 + u * 512 + l * 16 (+ a
+// per-iteration rotation): a warp's request is 512 contiguous bytes = 4 conflict-free wavefronts.  8 independent
+// LDS.128 per iteration, every loaded word used (ptxas narrows a vector load whose components are dead).
 __global__ void __launch_bounds__(1024, 1)
 probe_lds_kernel(int32_t iters, unsigned int* __restrict__ sink)
 {
@@ -42,61 +50,62 @@ probe_lds_kernel(int32_t iters, unsigned int* __restrict__ sink)
     uint4* s = reinterpret_cast<uint4*>(probe_smem);
     for (int i = threadIdx.x; i < 4096; i += blockDim.x) s[i] = make_uint4(i, i + 1, i + 2, i + 3);
     __syncthreads();
-    const uint32_t base = smem_u32(probe_smem);
-    uint32_t off = (threadIdx.x & 31) * 16 + (threadIdx.x >> 5) * 2048;
-    unsigned int acc = 0;
-    for (int32_t it = 0; it < iters; ++it) {
+    const uint32_t a0 = smem_u32(probe_smem) + (threadIdx.x & 31) * 16 + (threadIdx.x >> 5) * 2048;
+    const uint32_t a1 = smem_u32(probe_smem) + (threadIdx.x & 31) * 16 + ((threadIdx.x >> 5) ^ 16) * 2048;
+    uint4 acc = make_uint4(0u, 0u, 0u, 0u);
+    for (int32_t it = 0; it < iters; it += 2) {
         uint4 v[8];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) v[u] = lds128(base + ((off + u * 512) & 0xffffu));
+        for (int u = 0; u < 4; ++u) v[u] = probe_lds128(a0 + u * 512);
 #pragma unroll
-        for (int u = 0; u < 8; ++u) acc ^= v[u].x ^ v[u].w;
-        off += 4096;
+        for (int u = 0; u < 4; ++u) v[4 + u] = probe_lds128(a1 + u * 512);
+#pragma unroll
+        for (int u = 0; u < 8; u += 2) { acc.x ^= v[u].x ^ v[u + 1].x; acc.y ^= v[u].y ^ v[u + 1].y; acc.z ^= v[u].z ^ v[u + 1].z; acc.w ^= v[u].w ^ v[u + 1].w; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[u] = probe_lds128(a1 + u * 512);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v[4 + u] = probe_lds128(a0 + u * 512);
+#pragma unroll
+        for (int u = 0; u < 8; u += 2) { acc.x ^= v[u].x ^ v[u + 1].x; acc.y ^= v[u].y ^ v[u + 1].y; acc.z ^= v[u].z ^ v[u + 1].z; acc.w ^= v[u].w ^ v[u + 1].w; }
     }
-    if (acc == 0x9e3779b9u) *sink = acc;
+    if ((acc.x ^ acc.y ^ acc.z ^ acc.w) == 0x9e3779b9u) *sink = acc.x;
 }
 
-// 16 independent chains of setp.ge.and.f32 per iteration on register operands (one of which changes every
-// iteration, so no compare is loop-invariant); 256 threads per block.
+// Six independent chains of setp.ge.and.f32 (the form of the TILED_F32 inner loop: p = p & (cur >= prev)) per
+// thread -- the hardware has seven predicate registers --, unrolled 8 times; 256 threads per block.
 __global__ void __launch_bounds__(256)
 probe_fsetp_kernel(int32_t iters, float a, float b, unsigned int* __restrict__ sink)
 {
     const float x = a + threadIdx.x, y = b + threadIdx.x;
     unsigned int res;
+#define EBIC_FSETP6 \
+        "setp.ge.and.f32 p0, fx, fy, p0;\n\t setp.ge.and.f32 p1, fy, fx, p1;\n\t setp.ge.and.f32 p2, fx, fz, p2;\n\t" \
+        "setp.ge.and.f32 p3, fz, fx, p3;\n\t setp.ge.and.f32 p4, fy, fz, p4;\n\t setp.ge.and.f32 p5, fz, fy, p5;\n\t"
     asm volatile(
         "{\n\t"
-        ".reg .pred p<16>;\n\t"
+        ".reg .pred p<6>;\n\t"
         ".reg .pred q;\n\t"
         ".reg .s32 n;\n\t"
-        ".reg .f32 fx, fy;\n\t"
+        ".reg .f32 fx, fy, fz;\n\t"
         "mov.s32 n, %1;\n\t"
         "mov.f32 fx, %2;\n\t"
         "mov.f32 fy, %3;\n\t"
-        "setp.ge.f32 p0, fx, fy;\n\t  setp.ge.f32 p1, fy, fx;\n\t  setp.ge.f32 p2, fx, fy;\n\t  setp.ge.f32 p3, fy, fx;\n\t"
-        "setp.ge.f32 p4, fx, fy;\n\t  setp.ge.f32 p5, fy, fx;\n\t  setp.ge.f32 p6, fx, fy;\n\t  setp.ge.f32 p7, fy, fx;\n\t"
-        "setp.ge.f32 p8, fx, fy;\n\t  setp.ge.f32 p9, fy, fx;\n\t  setp.ge.f32 p10, fx, fy;\n\t setp.ge.f32 p11, fy, fx;\n\t"
-        "setp.ge.f32 p12, fx, fy;\n\t setp.ge.f32 p13, fy, fx;\n\t setp.ge.f32 p14, fx, fy;\n\t setp.ge.f32 p15, fy, fx;\n\t"
+        "add.f32 fz, fx, fy;\n\t"
+        "setp.ge.f32 p0, fx, fy;\n\t setp.ge.f32 p1, fy, fx;\n\t setp.ge.f32 p2, fx, fz;\n\t"
+        "setp.ge.f32 p3, fz, fx;\n\t setp.ge.f32 p4, fy, fz;\n\t setp.ge.f32 p5, fz, fy;\n\t"
         "PROBE_FSETP_LOOP:\n\t"
-        "setp.ge.and.f32 p0, fx, fy, p0;\n\t  setp.ge.and.f32 p1, fy, fx, p1;\n\t"
-        "setp.ge.and.f32 p2, fx, fy, p2;\n\t  setp.ge.and.f32 p3, fy, fx, p3;\n\t"
-        "setp.ge.and.f32 p4, fx, fy, p4;\n\t  setp.ge.and.f32 p5, fy, fx, p5;\n\t"
-        "setp.ge.and.f32 p6, fx, fy, p6;\n\t  setp.ge.and.f32 p7, fy, fx, p7;\n\t"
-        "setp.ge.and.f32 p8, fx, fy, p8;\n\t  setp.ge.and.f32 p9, fy, fx, p9;\n\t"
-        "setp.ge.and.f32 p10, fx, fy, p10;\n\t setp.ge.and.f32 p11, fy, fx, p11;\n\t"
-        "setp.ge.and.f32 p12, fx, fy, p12;\n\t setp.ge.and.f32 p13, fy, fx, p13;\n\t"
-        "setp.ge.and.f32 p14, fx, fy, p14;\n\t setp.ge.and.f32 p15, fy, fx, p15;\n\t"
+        EBIC_FSETP6 EBIC_FSETP6 EBIC_FSETP6 EBIC_FSETP6 EBIC_FSETP6 EBIC_FSETP6 EBIC_FSETP6 EBIC_FSETP6
         "add.f32 fx, fx, 0f3F800000;\n\t"
         "sub.s32 n, n, 1;\n\t"
         "setp.gt.s32 q, n, 0;\n\t"
         "@q bra PROBE_FSETP_LOOP;\n\t"
-        "and.pred p0, p0, p1;\n\t and.pred p2, p2, p3;\n\t and.pred p4, p4, p5;\n\t and.pred p6, p6, p7;\n\t"
-        "and.pred p8, p8, p9;\n\t and.pred p10, p10, p11;\n\t and.pred p12, p12, p13;\n\t and.pred p14, p14, p15;\n\t"
-        "and.pred p0, p0, p2;\n\t and.pred p4, p4, p6;\n\t and.pred p8, p8, p10;\n\t and.pred p12, p12, p14;\n\t"
-        "and.pred p0, p0, p4;\n\t and.pred p8, p8, p12;\n\t and.pred p0, p0, p8;\n\t"
+        "and.pred p0, p0, p1;\n\t and.pred p2, p2, p3;\n\t and.pred p4, p4, p5;\n\t"
+        "and.pred p0, p0, p2;\n\t and.pred p0, p0, p4;\n\t"
         "selp.u32 %0, 1, 0, p0;\n\t"
         "}"
         : "=r"(res)
         : "r"(iters), "f"(x), "f"(y));
+#undef EBIC_FSETP6
     if (res != 0u) atomicAdd(sink, res);                        // data-dependent: the chains cannot be dropped
 }
 

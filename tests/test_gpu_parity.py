@@ -1,7 +1,7 @@
 """Parity of the CUDA path (through the C ABI, via the thin binding) against the CPU oracle.
 
 Bar: bit-exact (integer counts and bitmasks from exact float32 comparisons; tolerance 0).
-Every fitness kernel (DIRECT, TILED_F32, RANK8, PAIRBITS) is compared with the oracle on the same seeded
+Every fitness kernel (DIRECT, TILED_F32, RANK8, PAIRBITS, UNION_F32) is compared with the oracle on the same seeded
 inputs.  All tests here need the B200.
 """
 from __future__ import annotations
@@ -28,7 +28,7 @@ def B():
 
 def kernels_for(eb, B):
     ks = [B.EBIC_KERNEL_DIRECT]
-    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_PAIRBITS):
+    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_UNION_F32):
         try:
             eb.set_kernel(k)
             ks.append(k)
@@ -221,8 +221,8 @@ def test_long_and_degenerate_chromosomes(B, oracle_mod):
 
 
 def test_wide_matrix_falls_back(B, oracle_mod):
-    """cols > 127: no rank tiles; cols so large that no float tile double-buffers: DIRECT only.  The pair
-    table still serves (PAIRBITS); without it AUTO falls back to TILED_F32 / DIRECT."""
+    """cols > 127: no rank tiles; cols so large that no float tile of all columns double-buffers: the column-union
+    kernel.  The pair table still serves (PAIRBITS); without it AUTO falls back to TILED_F32 / UNION_F32."""
     for cols in (128, 200, 500):
         m, off, ids = W.random_case(cols, 700, cols, 50, (0, 9), 0.02, False, True)
         with B.Ebic(m, ON) as eb:
@@ -231,7 +231,7 @@ def test_wide_matrix_falls_back(B, oracle_mod):
             assert eb.kernel == B.EBIC_KERNEL_PAIRBITS
             eb.set_pairbits(False)
             assert eb.info(14) == 0
-            expected = B.EBIC_KERNEL_TILED_F32 if cols <= 200 else B.EBIC_KERNEL_DIRECT
+            expected = B.EBIC_KERNEL_TILED_F32 if cols <= 200 else B.EBIC_KERNEL_UNION_F32
             assert eb.kernel == expected
             with pytest.raises(B.EbicError):
                 eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)
@@ -240,6 +240,43 @@ def test_wide_matrix_falls_back(B, oracle_mod):
             eb.set_pairbits(True)
             assert eb.kernel == B.EBIC_KERNEL_PAIRBITS
         check_all(B, oracle_mod, m, ON, off, ids, np.arange(0, 50, 7, dtype=np.int32))
+
+
+@pytest.mark.parametrize("cols,batch", [(310, 0), (310, 1), (310, 256), (500, 0), (500, 7), (500, 256), (40, 3), (3000, 0)])
+def test_column_union_kernel(B, oracle_mod, cols, batch):
+    """SURVEY.md 8(f) NEXT-2 / north_star (3) "(or the population's column union)": with the pair table refused
+    (ebic_set_pairbits(0)) a 310- or 500-column matrix runs the column-union kernel, not DIRECT.  Batches of 1
+    (every union fits), the default, and 256 individuals (the union overflows the tile: the individuals that do
+    not fit are evaluated from global memory by the same warps); chromosomes longer than the 32-id record,
+    duplicates and invalid individuals included; both early-exit modes."""
+    rows = 2_500
+    m, off, ids = W.random_case(cols + batch, rows, cols, 400, (0, 24), 0.02, cols <= 40, True)
+    rng = np.random.default_rng(cols)
+    extra = [rng.integers(0, cols, 40).tolist(), rng.integers(0, cols, 33).tolist(), [1, 1, 1], [cols - 1, 0],
+             rng.permutation(cols)[:min(cols, 300)].tolist(), [0, cols]]           # the last one is invalid
+    chroms = [ids[off[k]:off[k + 1]].tolist() for k in range(400)] + extra
+    off, ids = csr(chroms)
+    st, want = oracle_mod.eval_fitness(m, ON, off, ids)
+    assert st == B.EBIC_ERR_BAD_COLUMN
+    with B.Ebic(m, ON) as eb:
+        eb.set_pairbits(False)
+        if cols > 256:
+            assert eb.kernel == B.EBIC_KERNEL_UNION_F32          # what AUTO runs now
+        eb.set_kernel(B.EBIC_KERNEL_UNION_F32)
+        eb.set_tuning(B.TUNE_UNION_BATCH, batch)
+        for early_exit in (True, False):
+            eb.set_early_exit(early_exit)
+            got = gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_UNION_F32)
+            assert (got == want).all(), (early_exit, np.flatnonzero(got != want)[:10])
+            assert eb.last_kernel == B.EBIC_KERNEL_UNION_F32
+            assert eb.status() == st
+        # executed-work accounting: plain work visits every column of every valid chromosome of >= 2 columns
+        eb.set_early_exit(False)
+        eb.set_instrumentation(1)
+        gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_UNION_F32)
+        L = np.diff(off)[:-1]
+        assert eb.info(10) == eb.ld * int(L[L >= 2].sum())
+        eb.set_instrumentation(0)
 
 
 @pytest.mark.parametrize("sentinel", [999.0, 0.0, -1.5])
