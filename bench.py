@@ -273,7 +273,7 @@ def timed_ms(fn, reps, flush):
 
 def best_kernel_without_table(B, eb):
     """The fastest kernel that needs no pair table for this shape (what AUTO falls to when the table is refused)."""
-    for k in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_UNION_F32, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_DIRECT):
+    for k in (B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_UNION_F32, B.EBIC_KERNEL_DIRECT):
         try:
             eb.set_kernel(k)
             eb.set_kernel(B.EBIC_KERNEL_AUTO)

@@ -99,20 +99,25 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
     return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
 }
 
-// Rows per tile: largest multiple of `quantum` that double-buffers into shared memory, <= cap.
-int32_t pick_tile_rows(const ebic_ctx* ctx, int32_t elem, int32_t quantum, int32_t cap, int32_t n_ind_launch) {
+// Rows per tile: largest multiple of `quantum` that fits shared memory `nbuf` times, <= cap.
+int32_t pick_tile_rows(const ebic_ctx* ctx, int32_t elem, int32_t quantum, int32_t cap, int32_t n_ind_launch, int32_t nbuf = 2) {
     const int64_t cnt = (static_cast<int64_t>(n_ind_launch) * 4 + 127) & ~127ll;
     const int64_t avail = static_cast<int64_t>(ctx->smem_optin) - kSmemHeader - cnt;
     if (avail <= 0) return 0;
-    int64_t T = avail / (2ll * ctx->cols * elem);
+    int64_t T = avail / (static_cast<int64_t>(nbuf) * ctx->cols * elem);
     T = std::min<int64_t>(T, cap);
     T = std::min<int64_t>(T, ctx->ld);
     return static_cast<int32_t>(T / quantum * quantum);
 }
 
+// TILED_F32 double-buffers its tiles when two of them fit; a matrix too wide for that (221 < cols <= 445) gets one
+// 128-row tile: every individual of the population reuses it, so the load it can no longer hide is a few per cent.
+int32_t tile_bufs_f32(const ebic_ctx* ctx, int32_t n_ind_launch) {
+    return pick_tile_rows(ctx, 4, kRowsPerSlabF32, 1024, n_ind_launch, 2) > 0 ? 2 : 1;
+}
 int32_t tile_rows_f32(const ebic_ctx* ctx, int32_t n_ind_launch) {
-    if (ctx->cols > 256) return 0;          // the tiled kernels read byte ids
-    return pick_tile_rows(ctx, 4, kRowsPerSlabF32, 1024, n_ind_launch);
+    if (ctx->cols > 65535) return 0;        // the id records hold bytes (cols <= 256) or halfwords
+    return pick_tile_rows(ctx, 4, kRowsPerSlabF32, 1024, n_ind_launch, tile_bufs_f32(ctx, n_ind_launch));
 }
 int32_t tile_rows_r8(const ebic_ctx* ctx, int32_t n_ind_launch) {
     if (ctx->cols > kMaxColsRank8) return 0;
@@ -121,21 +126,21 @@ int32_t tile_rows_r8(const ebic_ctx* ctx, int32_t n_ind_launch) {
     if (T == 0) T = pick_tile_rows(ctx, 1, kRowsPerSlabR8, 4096, n_ind_launch);
     return T;
 }
-// UNION_F32: columns a staged 128-row tile can hold, double-buffered.
+// UNION_F32: columns a staged 128-row tile can hold, double-buffered, next to the records of a 256-individual batch.
 int32_t union_cap(const ebic_ctx* ctx) {
     if (ctx->cols > kUnionMaxCols) return 0;
-    const int64_t avail = static_cast<int64_t>(ctx->smem_optin) - kSmemHeader;
+    const int64_t avail = static_cast<int64_t>(ctx->smem_optin) - kSmemHeader - 2 * 256 * 40;
     return static_cast<int32_t>(std::min<int64_t>(std::min<int64_t>(avail / (2ll * kUnionTileRows * 4), 256), ctx->cols));
 }
 // Individuals per batch: the largest batch whose expected union, cols * (1 - exp(-batch * mean_L / cols)), still
 // fits 85 % of the tile (the plan kernel evaluates whatever does not fit from global memory).
 int32_t union_batch(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
-    if (ctx->union_batch > 0) return ctx->union_batch;
+    if (ctx->union_batch > 0) return (ctx->union_batch + 1) & ~1;
     const double cap = 0.85 * union_cap(ctx), cols = ctx->cols;
     const double mean_l = std::max(2.0, static_cast<double>(n_ids) / std::max(n_ind, 1));
     double b = 128.0;
     if (cap < cols) b = -cols / mean_l * std::log(1.0 - cap / cols);
-    return static_cast<int32_t>(std::max(4.0, std::min(128.0, b)));
+    return static_cast<int32_t>(std::max(4.0, std::min(128.0, b))) & ~1;       // even: the records are copied 16 bytes at a time
 }
 
 int32_t tile_rows(const ebic_ctx* ctx, int32_t kernel, int32_t n_ind_launch) {
@@ -146,7 +151,7 @@ int32_t tile_rows(const ebic_ctx* ctx, int32_t kernel, int32_t n_ind_launch) {
 // tiles, so a wide matrix gets a smaller population chunk rather than no tile at all.
 int32_t tiled_chunk(const ebic_ctx* ctx, int32_t kernel, int32_t n_ind) {
     int32_t n = std::min<int32_t>(n_ind, kMaxIndPerLaunch);
-    while (n > 64 && tile_rows(ctx, kernel, n) <= 0) n = (n + 1) / 2;
+    while (n > 1024 && tile_rows(ctx, kernel, n) <= 0) n = (n + 1) / 2;
     return n;
 }
 
@@ -180,8 +185,8 @@ bool kernel_applies(const ebic_ctx* ctx, int32_t kernel) {
     switch (kernel) {
         case EBIC_KERNEL_AUTO:
         case EBIC_KERNEL_DIRECT: return true;
-        case EBIC_KERNEL_TILED_F32: return tile_rows_f32(ctx, 64) > 0;
-        case EBIC_KERNEL_RANK8: return tile_rows_r8(ctx, 64) > 0;
+        case EBIC_KERNEL_TILED_F32: return tile_rows_f32(ctx, 1024) > 0;     // a tile next to >= 1,024 per-CTA counters
+        case EBIC_KERNEL_RANK8: return tile_rows_r8(ctx, 1024) > 0;
         case EBIC_KERNEL_PAIRBITS: return ctx->PB != nullptr;
         case EBIC_KERNEL_UNION_F32: return union_cap(ctx) >= 2;
         default: return false;
@@ -246,7 +251,7 @@ void free_pairbits(ebic_ctx* ctx) {
 
 namespace {
 
-template <class E, int NCONS>
+template <class E, int NCONS, class IW>
 int launch_tiled(ebic_ctx* ctx, const void* M, int32_t T, int32_t k0, int32_t n_ind, const int32_t* col_ids,
                  unsigned long long* counts, cudaStream_t stream, bool pdl) {
     TiledParams p;
@@ -254,16 +259,17 @@ int launch_tiled(ebic_ctx* ctx, const void* M, int32_t T, int32_t k0, int32_t n_
     p.ld = ctx->ld;
     p.cols = ctx->cols;
     p.T = T;
+    p.nbuf = sizeof(typename E::type) == 4 ? tile_bufs_f32(ctx, n_ind) : 2;
     p.n_tiles = (ctx->ld + T - 1) / T;
     p.meta = ctx->meta + k0;
-    p.idrec = ctx->idrec + 8ll * k0;
+    p.idrec = ctx->idrec + static_cast<int64_t>(32 / IW::kPerWord) * k0;
     p.col_ids = col_ids;
     p.n_ind = n_ind;
     p.early_exit = ctx->early_exit;
     p.counts = counts + k0;
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
-    const size_t smem = tiled_smem_bytes(ctx->cols, T, sizeof(typename E::type), n_ind);
-    auto kern = fitness_tiled_kernel<E, NCONS>;
+    const size_t smem = tiled_smem_bytes(ctx->cols, T, sizeof(typename E::type), n_ind, p.nbuf);
+    auto kern = fitness_tiled_kernel<E, NCONS, IW>;
     EBIC_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
     const int64_t P = p.n_tiles * n_ind;
     // at least one individual per consumer warp and CTA, never more CTAs than SMs (1 CTA / SM)
@@ -340,7 +346,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     const bool by_union = kernel0 == EBIC_KERNEL_UNION_F32;
     UnionParams up;
     if (tiled || by_union) {
-        st = grow(ctx, reinterpret_cast<void**>(&ctx->idrec), &ctx->idrec_cap, 32ll * n_ind);
+        st = grow(ctx, reinterpret_cast<void**>(&ctx->idrec), &ctx->idrec_cap, (ctx->cols > 256 && tiled ? 64ll : 32ll) * n_ind);
         if (st) return st;
     }
     if (by_union) {
@@ -367,6 +373,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     ip.nonmissing = ctx->nonmissing;
     ip.meta = ctx->meta;
     ip.idrec = tiled ? ctx->idrec : nullptr;
+    ip.id_wide = ctx->cols > 256;
     ip.prec = kernel0 == EBIC_KERNEL_PAIRBITS ? ctx->prec : nullptr;
     ip.pair_stride16 = static_cast<uint32_t>(ctx->ld / 128);
     ip.counts = counts;
@@ -416,14 +423,16 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
             const int32_t T = tile_rows(ctx, kernel0, n);
             if (T <= 0) return EBIC_ERR_ARG;
             if (kernel0 == EBIC_KERNEL_RANK8)
-                st = launch_tiled<ElemR8, kConsR8>(ctx, ctx->Rk, T, k0, n, col_ids, counts, stream, pdl);
+                st = launch_tiled<ElemR8, kConsR8, IdWords>(ctx, ctx->Rk, T, k0, n, col_ids, counts, stream, pdl);
+            else if (ctx->cols <= 256)
+                st = launch_tiled<ElemF32, kConsF32, IdWords>(ctx, ctx->Mc, T, k0, n, col_ids, counts, stream, pdl);
             else
-                st = launch_tiled<ElemF32, kConsF32>(ctx, ctx->Mc, T, k0, n, col_ids, counts, stream, pdl);
+                st = launch_tiled<ElemF32, kConsF32, IdWords16>(ctx, ctx->Mc, T, k0, n, col_ids, counts, stream, pdl);
             if (st) return st;
             pdl = false;                                  // only the first launch directly follows the ingest
         }
     } else if (by_union) {
-        const size_t smem = union_smem_bytes(up.u_cap);
+        const size_t smem = union_smem_bytes(up.u_cap, up.batch);
         auto kern = fitness_union_kernel<kUnionCons>;
         EBIC_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
         const int64_t P = (ctx->ld / kUnionTileRows) * up.n_batches;
@@ -431,7 +440,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         ctx->last_grid = static_cast<int32_t>(grid);
         ctx->last_T = kUnionTileRows;
         ctx->launches++;
-        EBIC_TRY(launch_pdl(kern, dim3(static_cast<unsigned>(grid)), dim3((kUnionCons + 1) * 32), smem, stream, pdl, up));
+        EBIC_TRY(launch_pdl(kern, dim3(static_cast<unsigned>(grid)), dim3((kUnionCons + kUnionProd) * 32), smem, stream, pdl, up));
     } else {
         const int64_t gx = ctx->ld / 256;
         int64_t gy = std::max<int64_t>(1, (8ll * ctx->sm_count + gx - 1) / gx);

@@ -76,6 +76,11 @@ __device__ __forceinline__ uint4 ldg128_ordered(const void* p) {
 __device__ __forceinline__ void cp_async16(uint32_t smem_dst, const void* gmem_src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_dst), "l"(gmem_src) : "memory");
 }
+// The executing thread's earlier cp.async copies, once they have all landed, count as ONE arrival on `bar` (the
+// arrival is part of the barrier's initial count: .noinc).
+__device__ __forceinline__ void cp_async_arrive_on(uint64_t* bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 

@@ -61,9 +61,11 @@ struct TiledParams {
     int64_t ld;
     int32_t cols;
     int32_t T;                       // rows per tile (multiple of the slab size)
+    int32_t nbuf;                    // tile buffers: 2 (the next tile travels while this one is evaluated), or 1 when a
+                                     // tile of all columns only fits once (wide matrices: loading is a few % of the work)
     int64_t n_tiles;                 // ceil(ld / T)
     const int2* meta;                // [n_ind] of this launch's population chunk
-    const uint32_t* idrec;           // [n_ind][8]: the first 32 ids of each individual as bytes (ingest_kernels.cuh)
+    const uint32_t* idrec;           // [n_ind][8] / [n_ind][16]: the first 32 ids of each individual as bytes / halfwords
     const int32_t* col_ids;          // the caller's ids: chromosomes with more than 32 columns continue from them
     int32_t n_ind;                   // individuals in this launch (<= kMaxIndPerLaunch)
     int32_t early_exit;              // stop a chain once no row of the warp's slab group is alive
@@ -74,9 +76,9 @@ struct TiledParams {
 constexpr int kMaxIndPerLaunch = 8192;
 constexpr int kSmemHeader = 128;     // 4 mbarriers, padded
 
-__host__ __device__ inline size_t tiled_smem_bytes(int32_t cols, int32_t T, int32_t elem, int32_t n_ind) {
+__host__ __device__ inline size_t tiled_smem_bytes(int32_t cols, int32_t T, int32_t elem, int32_t n_ind, int32_t nbuf) {
     size_t cnt = (static_cast<size_t>(n_ind) * 4 + 127) & ~static_cast<size_t>(127);
-    return kSmemHeader + cnt + 2 * static_cast<size_t>(cols) * T * elem;
+    return kSmemHeader + cnt + nbuf * static_cast<size_t>(cols) * T * elem;
 }
 
 __device__ __forceinline__ uint32_t id_byte(uint32_t w, int b) {   // b is a compile-time constant: one PRMT
@@ -166,6 +168,7 @@ struct ChainR8 {
 // The ids of one individual, four per 32-bit word: words 0..7 come from its id record (one warp-uniform load
 // each), later words are packed on the fly from the caller's int32 ids (valid individual: every id < cols <= 256).
 struct IdWords {
+    static constexpr int kPerWord = 4;
     const uint32_t* rec;             // idrec + 8 * k
     const int32_t* ids;              // col_ids + b
     int32_t L;
@@ -177,13 +180,52 @@ struct IdWords {
     }
 };
 
+// Matrices of more than 256 columns: two 16-bit ids per word, 16 words per record (ingest_kernels.cuh).
+struct IdWords16 {
+    static constexpr int kPerWord = 2;
+    const uint32_t* rec;             // idrec + 16 * k
+    const int32_t* ids;              // col_ids + b
+    int32_t L;
+    __device__ __forceinline__ uint32_t word(int32_t j) const {
+        if (j < 16) return __ldg(rec + j);
+        const int32_t i = 2 * j, last = L - 1;
+        return static_cast<uint32_t>(__ldg(ids + min(i, last))) | (static_cast<uint32_t>(__ldg(ids + min(i + 1, last))) << 16);
+    }
+};
+
+// The same for an id record that has been staged in shared memory (UNION_F32: admitted individuals have L <= 32).
+struct IdWordsShared {
+    static constexpr int kPerWord = 4;
+    const uint32_t* rec;
+    __device__ __forceinline__ uint32_t word(int32_t j) const { return rec[j]; }
+};
+
 // One chromosome on one slab group.  ids arrive four per word; w0 = first word (already loaded).
 // Full words run branch-free; the (at most two) ragged words go byte by byte.
 // Returns the number of matching rows; adds the number of columns actually visited to `steps`.
-template <class C>
-__device__ __forceinline__ int run_chain(C& c, const IdWords& iw, uint32_t w0, int32_t L,
+template <class C, class IW>
+__device__ __forceinline__ int run_chain(C& c, const IW& iw, uint32_t w0, int32_t L,
                                          bool early_exit, int32_t& steps)
 {
+    if constexpr (IW::kPerWord == 2) {                    // 16-bit ids, two per word
+        uint32_t w = w0;
+        uint32_t wn = (L > 2) ? iw.word(1) : 0u;
+        c.init(w & 0xffffu);
+        c.step(w >> 16);
+        int32_t rem = L - 2, done = 2, j = 1;
+        while (rem > 0) {
+            if (early_exit && (j & 1) && !__any_sync(0xffffffffu, c.alive())) break;
+            w = wn;
+            if (rem > 2) wn = iw.word(j + 1);
+            ++j;
+            c.step(w & 0xffffu);
+            if (rem >= 2) c.step(w >> 16);
+            done += min(rem, 2);
+            rem -= 2;
+        }
+        steps += done;
+        return c.count();
+    }
     uint32_t w = w0;
     uint32_t wn = (L > 4) ? iw.word(1) : 0u;
     c.init(id_byte(w, 0));
@@ -232,15 +274,10 @@ struct ElemR8 {
 };
 
 // All slabs of the tile for one individual.  Returns matches; `visited` += rows * columns actually visited.
-template <class E>
-__device__ __forceinline__ int eval_individual_on_tile(const typename E::type* tile, int32_t T, int32_t nslabs, int lane,
-                                                        const IdWords& iw, uint32_t w0, int32_t L, bool early_exit,
-                                                        unsigned long long& visited);
-
-template <>
-__device__ __forceinline__ int eval_individual_on_tile<ElemF32>(const float* tile, int32_t T, int32_t nslabs, int lane,
-                                                                const IdWords& iw, uint32_t w0, int32_t L,
-                                                                bool early_exit, unsigned long long& visited)
+template <class IW>
+__device__ __forceinline__ int eval_individual_on_tile(ElemF32, const float* tile, int32_t T, int32_t nslabs, int lane,
+                                                        const IW& iw, uint32_t w0, int32_t L,
+                                                        bool early_exit, unsigned long long& visited)
 {
     int cnt = 0;
     int32_t steps = 0;
@@ -254,10 +291,10 @@ __device__ __forceinline__ int eval_individual_on_tile<ElemF32>(const float* til
     return cnt;
 }
 
-template <>
-__device__ __forceinline__ int eval_individual_on_tile<ElemR8>(const uint8_t* tile, int32_t T, int32_t nslabs, int lane,
-                                                               const IdWords& iw, uint32_t w0, int32_t L,
-                                                               bool early_exit, unsigned long long& visited)
+template <class IW>
+__device__ __forceinline__ int eval_individual_on_tile(ElemR8, const uint8_t* tile, int32_t T, int32_t nslabs, int lane,
+                                                        const IW& iw, uint32_t w0, int32_t L,
+                                                        bool early_exit, unsigned long long& visited)
 {
     int cnt = 0;
     int32_t s = 0;
@@ -284,10 +321,12 @@ __device__ __forceinline__ int eval_individual_on_tile<ElemR8>(const uint8_t* ti
     return cnt;
 }
 
-template <class E, int NCONS>
+// IW = IdWords (byte ids, cols <= 256) or IdWords16 (16-bit ids, wider matrices).
+template <class E, int NCONS, class IW>
 __global__ void __launch_bounds__((NCONS + 1) * 32, 1)
 fitness_tiled_kernel(const TiledParams p)
 {
+    constexpr int kRecWords = 32 / IW::kPerWord;                 // words of an id record
     using elem_t = typename E::type;
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);          // [2]
@@ -319,8 +358,8 @@ fitness_tiled_kernel(const TiledParams p)
         // ---------------- producer warp (a4) ----------------
         const elem_t* M = reinterpret_cast<const elem_t*>(p.M);
         for (int32_t j = 0; j < ntl; ++j) {
-            const int buf = j & 1;
-            mbar_wait(&empty[buf], ((j >> 1) & 1) ^ 1);          // passes immediately for j < 2
+            const int buf = j % p.nbuf;
+            mbar_wait(&empty[buf], ((j / p.nbuf) & 1) ^ 1);      // passes immediately for j < nbuf
             const int64_t r0 = (t0 + j) * p.T;
             const int32_t nrows = static_cast<int32_t>(min(static_cast<int64_t>(p.T), p.ld - r0));
             const uint32_t col_bytes = static_cast<uint32_t>(nrows) * sizeof(elem_t);
@@ -339,7 +378,7 @@ fitness_tiled_kernel(const TiledParams p)
         unsigned long long visited = 0;
         const bool early_exit = p.early_exit != 0;
         for (int32_t j = 0; j < ntl; ++j) {
-            const int buf = j & 1;
+            const int buf = j % p.nbuf;
             const int64_t r0 = (t0 + j) * p.T;
             const int32_t nrows = static_cast<int32_t>(min(static_cast<int64_t>(p.T), p.ld - r0));
             const int32_t nslabs = nrows / E::kSlabRows;
@@ -352,19 +391,19 @@ fitness_tiled_kernel(const TiledParams p)
             uint32_t w_cur = 0;
             if (k < kb) {
                 m_cur = __ldg(&p.meta[k]);
-                w_cur = __ldg(p.idrec + 8ll * k);
+                w_cur = __ldg(p.idrec + static_cast<int64_t>(kRecWords) * k);
             }
-            mbar_wait(&full[buf], (j >> 1) & 1);
+            mbar_wait(&full[buf], (j / p.nbuf) & 1);
             for (; k < kb; k += NCONS) {
                 const int2 m = m_cur;
                 const uint32_t w0 = w_cur;
                 if (k + NCONS < kb) {
                     m_cur = __ldg(&p.meta[k + NCONS]);
-                    w_cur = __ldg(p.idrec + 8ll * (k + NCONS));
+                    w_cur = __ldg(p.idrec + static_cast<int64_t>(kRecWords) * (k + NCONS));
                 }
                 if (m.y < 2) continue;
-                const IdWords iw{p.idrec + 8ll * k, p.col_ids + m.x, m.y};
-                int cnt = eval_individual_on_tile<E>(tile, p.T, nslabs, lane, iw, w0, m.y, early_exit, visited);
+                const IW iw{p.idrec + static_cast<int64_t>(kRecWords) * k, p.col_ids + m.x, m.y};
+                int cnt = eval_individual_on_tile(E{}, tile, p.T, nslabs, lane, iw, w0, m.y, early_exit, visited);
                 cnt = __reduce_add_sync(0xffffffffu, cnt);
                 if (lane == 0 && cnt) atomicAdd(&s_cnt[k], static_cast<unsigned int>(cnt));
             }

@@ -7,8 +7,9 @@
 //
 //   meta[k]   = { b, L }: first entry of the chromosome in col_ids and its length; L = -1 = invalid individual
 //               (offsets[k] < 0, offsets[k+1] < offsets[k], offsets[k+1] > n_ids, or an id outside [0, cols)).
-//   idrec[k]  = (cols <= 256) the first 32 ids as bytes, eight 32-bit words, padded with the last id: the tiled
-//               kernels fetch four ids with one warp-uniform load.  Longer chromosomes continue from col_ids.
+//   idrec[k]  = the first 32 ids as bytes (cols <= 256: eight 32-bit words) or as halfwords (wider: sixteen words),
+//               padded with the last id: the tiled kernels fetch four / two ids with one warp-uniform load.
+//               Longer chromosomes continue from col_ids.
 //   prec[j]   = (pair table present) one 128-byte record per individual, read by a warp with ONE coalesced load:
 //               word 0 = L (-1 = invalid), word 1 = k, words 2..31 = the bit-column offsets of the first 30
 //               consecutive pairs (id_i, id_{i+1}) in the pair table, in 16-byte units,
@@ -39,7 +40,8 @@ struct IngestParams {
     int32_t sort_by_length;          // 0: records stay in population order
     const unsigned long long* nonmissing;
     int2* meta;
-    uint32_t* idrec;                 // [n_ind][8] or nullptr
+    uint32_t* idrec;                 // [n_ind][8] (byte ids) / [n_ind][16] (16-bit ids, id_wide) or nullptr
+    int32_t id_wide;                 // cols > 256: the id record holds halfwords
     uint32_t* prec;                  // [n_ind][32] or nullptr
     uint32_t pair_stride16;          // 16-byte units per bit column = ld / 128
     unsigned long long* counts;
@@ -109,7 +111,10 @@ ingest_population_kernel(const IngestParams p)
             bad |= (id < 0 || id >= p.cols);
         }
         bad = __any_sync(0xffffffffu, bad);
-        if (p.idrec != nullptr) {                           // four byte ids per word, 8 words
+        if (p.idrec != nullptr && p.id_wide) {              // two 16-bit ids per word, 16 words
+            const uint32_t i0 = __shfl_sync(0xffffffffu, mine, (2 * lane) & 31), i1 = __shfl_sync(0xffffffffu, mine, (2 * lane + 1) & 31);
+            if (lane < 16) p.idrec[16ll * k + lane] = i0 | (i1 << 16);
+        } else if (p.idrec != nullptr) {                    // four byte ids per word, 8 words
             const uint32_t i0 = __shfl_sync(0xffffffffu, mine, (4 * lane) & 31), i1 = __shfl_sync(0xffffffffu, mine, (4 * lane + 1) & 31);
             const uint32_t i2 = __shfl_sync(0xffffffffu, mine, (4 * lane + 2) & 31), i3 = __shfl_sync(0xffffffffu, mine, (4 * lane + 3) & 31);
             if (lane < 8) p.idrec[8ll * k + lane] = i0 | (i1 << 8) | (i2 << 16) | (i3 << 24);

@@ -130,12 +130,18 @@ constexpr int kPairLaneStride = 144;             // bytes between two lanes' 32-
 constexpr int kPairColBytes = 32 * kPairLaneStride;          // 4,608
 constexpr int kPairStageBytes = kPairCB * kPairColBytes;     // 36,864; two stages
 
-// `va`: zeros already turned into -0.  Returns bit j = !(vb[j] < va[j]) for numbers (garbage where either is NaN).
-__device__ __forceinline__ uint32_t pair_word(const float (&va)[32], const float (&vb)[32]) {
-    uint32_t w = 0;
+// `va0` / `va1`: zeros already turned into -0.  w0 / w1 bit j = !(vb[j] < va[j]) for numbers (garbage where either
+// is NaN).  The two words are built together: two independent FADD -> SHF chains per warp.
+__device__ __forceinline__ void pair_words(const float (&va0)[32], const float (&va1)[32], const float (&vb)[32],
+                                           uint32_t& w0, uint32_t& w1) {
+    uint32_t x0 = 0, x1 = 0;
 #pragma unroll
-    for (int j = 31; j >= 0; --j) w = __funnelshift_l(__float_as_uint(vb[j] - va[j]), w, 1);   // w = w << 1 | sign
-    return ~w;
+    for (int j = 31; j >= 0; --j) {
+        x0 = __funnelshift_l(__float_as_uint(vb[j] - va0[j]), x0, 1);          // x = x << 1 | sign(b - a)
+        x1 = __funnelshift_l(__float_as_uint(vb[j] - va1[j]), x1, 1);
+    }
+    w0 = ~x0;
+    w1 = ~x1;
 }
 
 __global__ void __launch_bounds__(256, 2)
@@ -205,8 +211,10 @@ pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanma
             }
             const int64_t b = s * kPairCB + c;
             const uint32_t pb = ~__ldg(nan_t + b * ldw);
-            if (a0 < cols) out0[b * ldw] = pair_word(va0, vb) & pa0 & pb;
-            if (a1 < cols) out1[b * ldw] = pair_word(va1, vb) & pa1 & pb;
+            uint32_t w0, w1;
+            pair_words(va0, va1, vb, w0, w1);
+            if (a0 < cols) out0[b * ldw] = w0 & pa0 & pb;
+            if (a1 < cols) out1[b * ldw] = w1 & pa1 & pb;
         }
         __syncthreads();                                         // stage s may be overwritten by stage s + 2
     }

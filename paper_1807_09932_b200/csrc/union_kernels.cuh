@@ -9,8 +9,8 @@
 // chromosome is longer than the record's 32 ids -- is evaluated by the same warps straight from global memory.
 // fitness_union_kernel: persistent CTAs (one per SM) over (row tile, batch) items in tile-major order, so the
 // tile's columns stay in L2 while the batches pass over it and HBM reads the matrix about once.  Per item the
-// producer warp stages the batch's U columns x kUnionTileRows rows with TMA bulk copies (double-buffered,
-// mbarrier full/empty pairs); each consumer warp takes every n_cons-th individual of the batch and runs the same
+// producer warp stages the batch's U columns x kUnionTileRows rows, and the batch's id records, with 16-byte
+// cp.async copies whose completion is counted on an mbarrier (double-buffered, full/empty pairs); each consumer warp takes every n_cons-th individual of the batch and runs the same
 // float32 chain as the TILED_F32 kernel (4 rows per lane, LDS.128 + 4 FSETP.GE.AND per column) on local ids.
 // Counts: warp reduce -> one global 64-bit atomic per (item, individual) with a non-zero count.
 #pragma once
@@ -21,7 +21,8 @@ namespace ebic {
 
 constexpr int kUnionTileRows = 128;          // one slab of the float32 chain: 4 rows per lane
 constexpr int kUnionMaxCols = 65536;         // the plan kernel keeps a bit per column in shared memory
-constexpr int kUnionCons = 15;               // consumer warps (+1 producer = 512 threads)
+constexpr int kUnionCons = 16;               // consumer warps
+constexpr int kUnionProd = 16;                // producer warps (512 threads in all)
 
 struct UnionParams {
     const float* Mc;
@@ -130,8 +131,13 @@ union_plan_kernel(const UnionParams p)
     }
 }
 
-__host__ __device__ inline size_t union_smem_bytes(int32_t u_cap) {
-    return kSmemHeader + 2 * static_cast<size_t>(u_cap) * kUnionTileRows * sizeof(float);
+// Shared memory of one buffer: the tile, then the batch's id records (32 bytes each) and meta entries (8 bytes
+// each), which travel with the tile so that the consumers never wait on a global load.
+__host__ __device__ inline size_t union_buffer_bytes(int32_t u_cap, int32_t batch) {
+    return static_cast<size_t>(u_cap) * kUnionTileRows * sizeof(float) + static_cast<size_t>(batch) * 40;
+}
+__host__ __device__ inline size_t union_smem_bytes(int32_t u_cap, int32_t batch) {
+    return kSmemHeader + 2 * union_buffer_bytes(u_cap, batch);
 }
 
 // Chain of one individual on 128 rows read straight from global memory (not admitted to its batch's union).
@@ -156,14 +162,15 @@ __device__ __forceinline__ int union_direct_chain(const float* __restrict__ Mc, 
 }
 
 template <int NCONS>
-__global__ void __launch_bounds__((NCONS + 1) * 32, 1)
+__global__ void __launch_bounds__((NCONS + kUnionProd) * 32, 1)
 fitness_union_kernel(const UnionParams p)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem);          // [2]
     uint64_t* empty = full + 2;                                  // [2]
-    float* tiles = reinterpret_cast<float*>(smem + kSmemHeader);
-    const size_t tile_elems = static_cast<size_t>(p.u_cap) * kUnionTileRows;
+    unsigned char* buffers = smem + kSmemHeader;
+    const size_t tile_bytes = static_cast<size_t>(p.u_cap) * kUnionTileRows * sizeof(float);
+    const size_t buf_bytes = union_buffer_bytes(p.u_cap, p.batch);     // tile | records [batch][8] | meta [batch]
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t n_tiles = p.ld / kUnionTileRows;
@@ -171,8 +178,8 @@ fitness_union_kernel(const UnionParams p)
     const int64_t pb = P * blockIdx.x / gridDim.x;
     const int64_t pe = P * (blockIdx.x + 1) / gridDim.x;
     if (tid == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
+        mbar_init(&full[0], kUnionProd * 32);                    // one arrival per producer lane, when its copies have landed
+        mbar_init(&full[1], kUnionProd * 32);
         mbar_init(&empty[0], NCONS);
         mbar_init(&empty[1], NCONS);
         fence_mbar_init();
@@ -180,23 +187,39 @@ fitness_union_kernel(const UnionParams p)
     __syncthreads();
     griddep_wait();                                              // the plan (and the ingest before it) has completed
 
-    if (warp == NCONS) {
-        // ---------------- producer warp (a4): the batch's columns of this tile ----------------
+    if (warp >= NCONS) {
+        const int pw = warp - NCONS;                             // producer warp pw copies columns pw, pw + 4, ...
+        // ---------------- producer warps (a4): the batch's columns of this tile + the batch's records ----------------
+        // 16-byte cp.async copies (LDGSTS), one 512-byte column run per warp instruction: 64 B/clk/SM, the rate of the
+        // SM's L2 port.  (TMA bulk copies of 512 bytes were measured at ~64 cycles each, 8 B/clk: the round-2 first
+        // version of this kernel spent 6.7 us per item in them.)
         for (int64_t it = pb; it < pe; ++it) {
             const int32_t j = static_cast<int32_t>(it - pb);
             const int buf = j & 1;
             const int64_t t = it / p.n_batches;
             const int32_t b = static_cast<int32_t>(it - t * p.n_batches);
             const int32_t U = __ldg(&p.ucount[b]);
+            const int32_t k0 = b * p.batch;
+            const int32_t nb = min(p.n_ind, k0 + p.batch) - k0;
             mbar_wait(&empty[buf], ((j >> 1) & 1) ^ 1);          // passes immediately for j < 2
-            if (lane == 0) mbar_arrive_expect_tx(&full[buf], static_cast<uint32_t>(U) * kUnionTileRows * 4u);
-            __syncwarp();
             const int32_t* ucols = p.ucols + static_cast<int64_t>(b) * p.u_cap;
-            float* dst = tiles + buf * tile_elems;
-            const float* src = p.Mc + t * kUnionTileRows;
-            for (int32_t c = lane; c < U; c += 32)
-                bulk_copy_g2s(dst + static_cast<size_t>(c) * kUnionTileRows, src + static_cast<int64_t>(__ldg(ucols + c)) * p.ld,
-                              kUnionTileRows * 4u, &full[buf]);
+            unsigned char* buffer = buffers + buf * buf_bytes;
+            const uint32_t dst = smem_u32(buffer) + lane * 16;
+            const float* src = p.Mc + t * kUnionTileRows + lane * 4;
+            for (int32_t c0 = pw * 32; c0 < U; c0 += kUnionProd * 32) {
+                const int32_t mine = (c0 + lane < U) ? __ldg(ucols + c0 + lane) : 0;
+                const int32_t n = min(32, U - c0);
+                for (int32_t i = 0; i < n; ++i)
+                    cp_async16(dst + (c0 + i) * (kUnionTileRows * 4), src + static_cast<int64_t>(__shfl_sync(0xffffffffu, mine, i)) * p.ld);
+            }
+            const uint32_t rec_dst = smem_u32(buffer + tile_bytes), meta_dst = rec_dst + p.batch * 32;
+            const unsigned char* rec_src = reinterpret_cast<const unsigned char*>(p.urec + 8ll * k0);
+            const unsigned char* meta_src = reinterpret_cast<const unsigned char*>(p.meta + k0);
+            if (pw == 0) {
+                for (int32_t u = lane; u < nb * 2; u += 32) cp_async16(rec_dst + u * 16, rec_src + u * 16);
+                for (int32_t u = lane; u < (nb + 1) / 2; u += 32) cp_async16(meta_dst + u * 16, meta_src + u * 16);
+            }
+            cp_async_arrive_on(&full[buf]);
         }
     } else {
         // ---------------- consumer warps (a5, a6) ----------------
@@ -208,19 +231,22 @@ fitness_union_kernel(const UnionParams p)
             const int64_t t = it / p.n_batches;
             const int32_t b = static_cast<int32_t>(it - t * p.n_batches);
             const int32_t k0 = b * p.batch, k1 = min(p.n_ind, k0 + p.batch);
-            const float* tile = tiles + buf * tile_elems;
+            const unsigned char* buffer = buffers + buf * buf_bytes;
+            const float* tile = reinterpret_cast<const float*>(buffer);
+            const uint32_t* s_rec = reinterpret_cast<const uint32_t*>(buffer + tile_bytes);
+            const int2* s_meta = reinterpret_cast<const int2*>(buffer + tile_bytes + static_cast<size_t>(p.batch) * 32);
             mbar_wait(&full[buf], (j >> 1) & 1);
             for (int32_t k = k0 + warp; k < k1; k += NCONS) {
-                const int2 m = __ldg(&p.meta[k]);
+                const int2 m = s_meta[k - k0];
                 if (m.y < 2) continue;
-                const uint32_t w0 = __ldg(p.urec + 8ll * k);
+                const IdWordsShared iw{s_rec + 8 * (k - k0)};                           // admitted: L <= 32, words 0..7 only
+                const uint32_t w0 = iw.word(0);
                 int cnt;
                 int32_t steps = 0;
                 if (w0 != 0xffffffffu) {
                     ChainF32 c;
                     c.base = smem_u32(tile) + lane * 16;
                     c.stride = kUnionTileRows * 4;
-                    const IdWords iw{p.urec + 8ll * k, p.col_ids + m.x, m.y};          // admitted: L <= 32, words 0..7 only
                     cnt = run_chain(c, iw, w0, m.y, early_exit, steps);
                 } else {
                     cnt = union_direct_chain(p.Mc, p.ld, t * kUnionTileRows, lane, p.col_ids + m.x, m.y, early_exit, steps);

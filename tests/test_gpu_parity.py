@@ -223,15 +223,15 @@ def test_long_and_degenerate_chromosomes(B, oracle_mod):
 def test_wide_matrix_falls_back(B, oracle_mod):
     """cols > 127: no rank tiles; cols so large that no float tile of all columns double-buffers: the column-union
     kernel.  The pair table still serves (PAIRBITS); without it AUTO falls back to TILED_F32 / UNION_F32."""
-    for cols in (128, 200, 500):
-        m, off, ids = W.random_case(cols, 700, cols, 50, (0, 9), 0.02, False, True)
+    for cols in (128, 200, 230, 300, 445, 446, 500):
+        m, off, ids = W.random_case(cols, 700, cols, 50, (0, 40), 0.02, False, True)
         with B.Ebic(m, ON) as eb:
             with pytest.raises(B.EbicError):
                 eb.set_kernel(B.EBIC_KERNEL_RANK8)
             assert eb.kernel == B.EBIC_KERNEL_PAIRBITS
             eb.set_pairbits(False)
             assert eb.info(14) == 0
-            expected = B.EBIC_KERNEL_TILED_F32 if cols <= 200 else B.EBIC_KERNEL_UNION_F32
+            expected = B.EBIC_KERNEL_TILED_F32 if cols <= 445 else B.EBIC_KERNEL_UNION_F32
             assert eb.kernel == expected
             with pytest.raises(B.EbicError):
                 eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)
@@ -260,8 +260,10 @@ def test_column_union_kernel(B, oracle_mod, cols, batch):
     assert st == B.EBIC_ERR_BAD_COLUMN
     with B.Ebic(m, ON) as eb:
         eb.set_pairbits(False)
-        if cols > 256:
+        if cols > 445:                                           # up to 445 columns one 128-row tile of ALL columns still fits
             assert eb.kernel == B.EBIC_KERNEL_UNION_F32          # what AUTO runs now
+        elif cols > 127:
+            assert eb.kernel == B.EBIC_KERNEL_TILED_F32
         eb.set_kernel(B.EBIC_KERNEL_UNION_F32)
         eb.set_tuning(B.TUNE_UNION_BATCH, batch)
         for early_exit in (True, False):
