@@ -49,7 +49,7 @@ METRIC = "row_pair_comparisons_per_s"
 UNIT = "comparisons/s"
 N_CHOSEN = 8
 WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4, "p1": 5, "p2": 6, "p3": 7}
-KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "union_f32": 5}
+KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "union_f32": 5, "prefix": 6}
 TRAFFIC_CSV = ROOT / "profiles" / "r02_dram_traffic.csv"
 KERNEL_SOURCES = ["pairbits_kernels.cuh", "fitness_kernels.cuh", "union_kernels.cuh", "ebic_device.cuh"]
 
@@ -199,7 +199,7 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
     pipe_basis = (f"max(stated {sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz = {pipe_stated:.0f} GB/s, "
                   f"LDS.128 probe {pipe_probe:.0f} GB/s)" if pipe_probe else
                   f"{sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz ({peaks_kind} sm_max_mhz)")
-    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "union_f32": 4, "direct": 4, "pairbits": 0.125}[kernel_name]
+    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "union_f32": 4, "direct": 4, "pairbits": 0.125, "prefix": 0.125}[kernel_name]
     achieved = visits_executed * bytes_per_visit / kernel_s / 1e9
     bound, peak, basis = "alu", pipe_gbs, pipe_basis
     resource = "shared-memory data pipe (128 B/clk/SM)"

@@ -22,7 +22,10 @@ enum {
     EBIC_KERNEL_TILED_F32 = 2, /* float32 row tiles of ALL columns staged in shared memory by TMA bulk copies  */
     EBIC_KERNEL_RANK8 = 3,     /* per-row order-preserving 8-bit rank tiles (cols <= 127)                      */
     EBIC_KERNEL_PAIRBITS = 4,  /* AND of pair-relation bit columns gathered through L2 (pair table built)      */
-    EBIC_KERNEL_UNION_F32 = 5  /* float32 tiles of the COLUMN UNION of a batch of individuals (any cols)       */
+    EBIC_KERNEL_UNION_F32 = 5, /* float32 tiles of the COLUMN UNION of a batch of individuals (any cols)       */
+    EBIC_KERNEL_PREFIX = 6     /* PAIRBITS with shared-prefix groups: individuals that start with the same
+                                  columns share the AND of those bit columns (population <= 8,192; larger
+                                  populations run plain PAIRBITS)                                              */
 };
 
 /* Selects the fitness kernel.  EBIC_ERR_ARG if it cannot run this shape (RANK8 builds its rank tiles on demand,

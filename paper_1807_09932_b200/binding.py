@@ -32,7 +32,8 @@ EBIC_KERNEL_TILED_F32 = 2
 EBIC_KERNEL_RANK8 = 3
 EBIC_KERNEL_PAIRBITS = 4
 EBIC_KERNEL_UNION_F32 = 5
-KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits", 5: "union_f32"}
+EBIC_KERNEL_PREFIX = 6
+KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits", 5: "union_f32", 6: "prefix"}
 # ebic_set_tuning knobs (include/ebic_debug.h)
 TUNE_PB_TASKS_PER_SLOT, TUNE_PB_PREFETCH, TUNE_PB_SMEM_RING, TUNE_SORT, TUNE_PDL, TUNE_UNION_BATCH = range(6)
 

@@ -18,6 +18,7 @@
 #include "ingest_kernels.cuh"
 #include "loader_kernels.cuh"
 #include "pairbits_kernels.cuh"
+#include "prefix_kernels.cuh"
 #include "union_kernels.cuh"
 
 using namespace ebic;
@@ -187,7 +188,8 @@ bool kernel_applies(const ebic_ctx* ctx, int32_t kernel) {
         case EBIC_KERNEL_DIRECT: return true;
         case EBIC_KERNEL_TILED_F32: return tile_rows_f32(ctx, 1024) > 0;     // a tile next to >= 1,024 per-CTA counters
         case EBIC_KERNEL_RANK8: return tile_rows_r8(ctx, 1024) > 0;
-        case EBIC_KERNEL_PAIRBITS: return ctx->PB != nullptr;
+        case EBIC_KERNEL_PAIRBITS:
+        case EBIC_KERNEL_PREFIX: return ctx->PB != nullptr;
         case EBIC_KERNEL_UNION_F32: return union_cap(ctx) >= 2;
         default: return false;
     }
@@ -294,8 +296,33 @@ bool pairbits_dense(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
     return n_ids - n_ind >= 2ll * ctx->cols * ctx->cols;
 }
 
-int launch_pairbits(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_ind, int64_t n_ids, unsigned long long* counts,
-                    cudaStream_t stream, bool pdl) {
+PairbitsParams pairbits_params(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_ind, int64_t n_ids, unsigned long long* counts);
+
+// Shared-prefix variant: plan (sort + groups) and the grouped evaluation.
+int launch_prefix(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_ind, int64_t n_ids, unsigned long long* counts,
+                  cudaStream_t stream, bool pdl) {
+    PrefixParams pp;
+    pp.pb = pairbits_params(ctx, col_ids, n_ind, n_ids, counts);
+    pp.pb.prefetch_dist = 0;                                 // groups walk the table in sorted-pair order, not all of it
+    pp.groups = ctx->ubatch;
+    pp.n_groups = ctx->ubatch + 8ll * n_ind;
+    int32_t n_pow2 = 1;
+    while (n_pow2 < n_ind) n_pow2 <<= 1;
+    const size_t plan_smem = 13ull * n_pow2;
+    EBIC_TRY(cudaFuncSetAttribute(prefix_plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(plan_smem)));
+    ctx->launches += 2;
+    EBIC_TRY(launch_pdl(prefix_plan_kernel, dim3(1), dim3(1024), plan_smem, stream, pdl, pp, n_pow2));
+    const int64_t tasks = static_cast<int64_t>(pp.pb.n_chunks) * n_ind;          // worst case: every individual alone
+    const int64_t grid = (tasks + kPairbitsWarps - 1) / kPairbitsWarps;
+    if (grid > 0x7fffffffll) return EBIC_ERR_ARG;
+    ctx->last_grid = static_cast<int32_t>(grid);
+    ctx->last_T = pp.pb.chunk_words * 32;
+    const dim3 g(static_cast<unsigned>(grid)), b(kPairbitsWarps * 32);
+    return ebic_host::cuda_status(ctx->early_exit ? launch_pdl(fitness_prefix_kernel<true>, g, b, 0, stream, pdl, pp)
+                                                  : launch_pdl(fitness_prefix_kernel<false>, g, b, 0, stream, pdl, pp));
+}
+
+PairbitsParams pairbits_params(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_ind, int64_t n_ids, unsigned long long* counts) {
     PairbitsParams p;
     p.PB = ctx->PB;
     p.ldw = ctx->ld / 32;
@@ -312,6 +339,13 @@ int launch_pairbits(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_ind, int64_
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
     p.n_pairs = ctx->cols * ctx->cols;
     p.prefetch_dist = pairbits_dense(ctx, n_ind, n_ids) ? ctx->pb_prefetch_dist : 0;
+    return p;
+}
+
+int launch_pairbits(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_ind, int64_t n_ids, unsigned long long* counts,
+                    cudaStream_t stream, bool pdl) {
+    const PairbitsParams p = pairbits_params(ctx, col_ids, n_ind, n_ids, counts);
+    const int64_t cw = p.chunk_words;
     const int64_t tasks = static_cast<int64_t>(p.n_chunks) * n_ind;
     const int64_t grid = (tasks + kPairbitsWarps - 1) / kPairbitsWarps;
     if (grid > 0x7fffffffll) return EBIC_ERR_ARG;
@@ -356,8 +390,14 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         st = grow(ctx, reinterpret_cast<void**>(&ctx->ubatch), &ctx->ubatch_cap, 4ll * up.n_batches * (up.u_cap + 1));
         if (st) return st;
     }
-    if (kernel0 == EBIC_KERNEL_PAIRBITS) {
+    const bool by_prefix = kernel0 == EBIC_KERNEL_PREFIX && n_ind <= kPrefixMaxInd;     // larger populations: plain PAIRBITS
+    const bool by_pairs = kernel0 == EBIC_KERNEL_PAIRBITS || kernel0 == EBIC_KERNEL_PREFIX;
+    if (by_pairs) {
         st = grow(ctx, reinterpret_cast<void**>(&ctx->prec), &ctx->prec_cap, 128ll * n_ind);
+        if (st) return st;
+    }
+    if (by_prefix) {
+        st = grow(ctx, reinterpret_cast<void**>(&ctx->ubatch), &ctx->ubatch_cap, 4ll * (8ll * n_ind + 4));
         if (st) return st;
     }
 
@@ -374,7 +414,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     ip.meta = ctx->meta;
     ip.idrec = tiled ? ctx->idrec : nullptr;
     ip.id_wide = ctx->cols > 256;
-    ip.prec = kernel0 == EBIC_KERNEL_PAIRBITS ? ctx->prec : nullptr;
+    ip.prec = by_pairs ? ctx->prec : nullptr;
     ip.pair_stride16 = static_cast<uint32_t>(ctx->ld / 128);
     ip.counts = counts;
     ip.err = ctx->d_err;
@@ -413,7 +453,11 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         EBIC_TRY(cudaEventRecord(ctx->ev_begin[slot], stream));
     }
     ctx->last_kernel = kernel0;
-    if (kernel0 == EBIC_KERNEL_PAIRBITS) {
+    if (by_prefix) {
+        st = launch_prefix(ctx, col_ids, n_ind, n_ids, counts, stream, pdl);
+        if (st) return st;
+    } else if (by_pairs) {
+        ctx->last_kernel = EBIC_KERNEL_PAIRBITS;
         st = launch_pairbits(ctx, col_ids, n_ind, n_ids, counts, stream, pdl);   // any population size in one launch
         if (st) return st;
     } else if (tiled) {

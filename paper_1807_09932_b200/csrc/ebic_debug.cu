@@ -20,7 +20,7 @@ using ebic_host::cuda_status;
 extern "C" {
 
 int ebic_set_kernel(ebic_ctx* ctx, int32_t kernel) {
-    if (!ctx || kernel < EBIC_KERNEL_AUTO || kernel > EBIC_KERNEL_UNION_F32) return EBIC_ERR_ARG;
+    if (!ctx || kernel < EBIC_KERNEL_AUTO || kernel > EBIC_KERNEL_PREFIX) return EBIC_ERR_ARG;
     if (!ebic_host::kernel_applies(ctx, kernel)) return EBIC_ERR_ARG;
     if (kernel == EBIC_KERNEL_RANK8) {
         if (cudaDeviceSynchronize() != cudaSuccess) return cuda_status(cudaGetLastError());

@@ -187,8 +187,11 @@ pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanma
                            tile + static_cast<int64_t>(b0 + c) * ld + 4 * tid);
         cp_async_commit();
     };
-    uint32_t* out0 = PB + static_cast<int64_t>(a0) * cols * ldw + t * 32 + lane;
-    uint32_t* out1 = PB + static_cast<int64_t>(a1) * cols * ldw + t * 32 + lane;
+    // running pointers: the words of pairs (a0, b) / (a1, b) and the NaN word of column b, b = 0, 1, 2, ...
+    uint32_t* out0 = PB + static_cast<int64_t>(min(a0, cols - 1)) * cols * ldw + t * 32 + lane;
+    uint32_t* out1 = PB + static_cast<int64_t>(min(a1, cols - 1)) * cols * ldw + t * 32 + lane;
+    const uint32_t* nan_b = nan_t;
+    const bool do0 = a0 < cols, do1 = a1 < cols;
     const int32_t n_stage = (cols + kPairCB - 1) / kPairCB;
     stage(0, 0);
     for (int32_t s = 0; s < n_stage; ++s) {
@@ -199,22 +202,21 @@ pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanma
             cp_async_wait_all();
         }
         __syncthreads();                                         // every thread's share of stage s has landed
-        const uint32_t src = stage0 + (s & 1) * kPairStageBytes + lane * kPairLaneStride;
+        uint32_t src = stage0 + (s & 1) * kPairStageBytes + lane * kPairLaneStride;
         const int32_t b_end = min(kPairCB, cols - s * kPairCB);
-        for (int32_t c = 0; c < b_end; ++c) {
+        for (int32_t c = 0; c < b_end; ++c, src += kPairColBytes, out0 += ldw, out1 += ldw, nan_b += ldw) {
             float vb[32];
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-                const uint4 x = lds128(src + c * kPairColBytes + q * 16);
+                const uint4 x = lds128(src + q * 16);
                 vb[4 * q] = __uint_as_float(x.x); vb[4 * q + 1] = __uint_as_float(x.y);
                 vb[4 * q + 2] = __uint_as_float(x.z); vb[4 * q + 3] = __uint_as_float(x.w);
             }
-            const int64_t b = s * kPairCB + c;
-            const uint32_t pb = ~__ldg(nan_t + b * ldw);
+            const uint32_t pb = ~__ldg(nan_b);
             uint32_t w0, w1;
             pair_words(va0, va1, vb, w0, w1);
-            if (a0 < cols) out0[b * ldw] = w0 & pa0 & pb;
-            if (a1 < cols) out1[b * ldw] = w1 & pa1 & pb;
+            if (do0) *out0 = w0 & pa0 & pb;
+            if (do1) *out1 = w1 & pa1 & pb;
         }
         __syncthreads();                                         // stage s may be overwritten by stage s + 2
     }

@@ -1,7 +1,7 @@
 """Parity of the CUDA path (through the C ABI, via the thin binding) against the CPU oracle.
 
 Bar: bit-exact (integer counts and bitmasks from exact float32 comparisons; tolerance 0).
-Every fitness kernel (DIRECT, TILED_F32, RANK8, PAIRBITS, UNION_F32) is compared with the oracle on the same seeded
+Every fitness kernel (DIRECT, TILED_F32, RANK8, PAIRBITS, UNION_F32, PREFIX) is compared with the oracle on the same seeded
 inputs.  All tests here need the B200.
 """
 from __future__ import annotations
@@ -28,7 +28,8 @@ def B():
 
 def kernels_for(eb, B):
     ks = [B.EBIC_KERNEL_DIRECT]
-    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_UNION_F32):
+    for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_UNION_F32,
+              B.EBIC_KERNEL_PREFIX):
         try:
             eb.set_kernel(k)
             ks.append(k)
@@ -365,6 +366,76 @@ def test_tuning_knobs_keep_parity(B, oracle_mod, knobs):
             eb.set_tuning(99, 0)
         with pytest.raises(B.EbicError):
             eb.set_tuning(B.TUNE_PB_TASKS_PER_SLOT, 0)
+
+
+def test_shared_prefix_evaluation(B, oracle_mod):
+    """SURVEY.md 8(f) NEXT-4, shared-prefix (trie) evaluation: a CONVERGED population -- 40 parents, every other
+    individual a parent with its tail re-drawn -- evaluated by EBIC_KERNEL_PREFIX: counts equal the oracle's, and
+    the executed-visit counter shows the shared prefixes were fetched once per group (plain work, early exit off:
+    PAIRBITS fetches padded rows * sum(L-1) bit-column rows, PREFIX far fewer); a uniformly random population shares
+    almost nothing and must cost no more than the nominal work."""
+    import torch
+    rows, cols = 30_001, 48
+    m, _, _ = W.random_case(77, rows, cols, 1, (1, 1), 0.01, False, True)
+    rng = np.random.default_rng(9)
+    parents = [rng.permutation(cols)[:rng.integers(8, 21)] for _ in range(40)]
+    chroms = []
+    for k in range(2_000):
+        par = parents[rng.integers(0, len(parents))]
+        keep = int(rng.integers(max(2, par.size - 4), par.size + 1))           # shared prefix of keep - 1 pairs
+        tail = rng.permutation(cols)[:rng.integers(0, 4)]
+        chroms.append(np.concatenate([par[:keep], tail]).tolist())
+    chroms += [[], [3], list(range(40)), [5, 5]]                                # L = 0, 1, 40 (never grouped), duplicate
+    for name, pop in (("converged", chroms), ("random", None)):
+        if pop is None:
+            _, off, ids = W.random_case(78, 8, cols, 2_000, (2, 16), 0.0, False, True)
+        else:
+            off, ids = csr(pop)
+        st, want = oracle_mod.eval_fitness(m, ON, off, ids)
+        nominal = None
+        with B.Ebic(m, ON) as eb:
+            nominal = eb.ld * int(np.maximum(np.diff(off) - 1, 0).sum())
+            seen = {}
+            for kern in (B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_PREFIX):
+                eb.set_kernel(kern)
+                for early_exit in (False, True):
+                    eb.set_early_exit(early_exit)
+                    eb.set_instrumentation(1)
+                    got = eb.eval_fitness(dev(off), dev(ids))
+                    torch.cuda.synchronize()
+                    seen[kern, early_exit] = eb.info(10)
+                    eb.set_instrumentation(0)
+                    assert (got.cpu().numpy().view(np.uint64) == want).all(), (name, B.KERNEL_NAMES[kern], early_exit)
+                    assert eb.last_kernel == kern
+            assert seen[B.EBIC_KERNEL_PAIRBITS, False] == nominal
+            assert seen[B.EBIC_KERNEL_PREFIX, False] <= nominal
+            if name == "converged":
+                assert seen[B.EBIC_KERNEL_PREFIX, False] < 0.55 * nominal, seen
+            assert eb.status() == 0
+
+
+def test_ring_path_stress(B, oracle_mod):
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.txt), so the PAIRBITS shared-memory landing
+    ring is stressed instead: 1,000 evaluations of freshly randomised populations whose chromosomes (9..24 columns)
+    all take the ring path, on a matrix of three row chunks with a ragged last step, both early-exit modes, every
+    count compared with the oracle.  A write-after-read hazard on the ring would corrupt some AND sooner or later."""
+    import torch
+    rows, cols, n_ind = 20_001, 24, 192
+    m, _, _ = W.random_case(123, rows, cols, 1, (1, 1), 0.01, True, True)
+    rng = np.random.default_rng(2024)
+    with B.Ebic(m, ON) as eb:
+        eb.set_kernel(B.EBIC_KERNEL_PAIRBITS)
+        for it in range(1000):
+            L = rng.integers(9, cols + 1, n_ind)
+            chroms = [rng.permutation(cols)[:l] if it % 3 else rng.integers(0, cols, l) for l in L]
+            off, ids = csr(chroms)
+            eb.set_early_exit(bool(it & 1))
+            got = eb.eval_fitness(dev(off), dev(ids))
+            st, want = oracle_mod.eval_fitness(m, ON, off, ids)
+            torch.cuda.synchronize()
+            got = got.cpu().numpy().view(np.uint64)
+            assert (got == want).all(), (it, np.flatnonzero(got != want)[:10])
+        assert eb.status() == 0
 
 
 def test_probe_read_bandwidth(B):
