@@ -346,7 +346,9 @@ def measure_workload(B, key, w, peaks, peaks_kind, probes, flush, reps, early_ex
         gain = alt_ms - kernel_ms
         entry["break_even"] = {"against": B.KERNEL_NAMES[alt], "its_kernel_ms": alt_ms, "its_build_ms": alt_build,
                                "pair_table_build_ms": breakdown["pair_table"],
-                               "evals": (breakdown["pair_table"] - alt_build) / gain if gain > 0 else None}
+                               # 0 = the table is cheaper to build than the other kernel's own derived data and
+                               # faster per evaluation; None = the other kernel is at least as fast (tiny inputs)
+                               "evals": max(0.0, (breakdown["pair_table"] - alt_build) / gain) if gain > 0 else None}
         eb.set_kernel(B.EBIC_KERNEL_AUTO)
     eb.close()
     return entry, roof
@@ -784,6 +786,48 @@ def run_table(args):
     return {"table": rows_out}
 
 
+def render_table(path):
+    """Markdown of a --table result (the tracked profiles/r02_table.json backs BASELINE.md section 4)."""
+    rows = json.loads(Path(path).read_text())
+    out = []
+    probes = [r for r in rows if r.get("kernel") == "probes"]
+    if probes:
+        pr = probes[0]
+        out.append(f"Probes in the same process: L2-resident read {pr['l2_read_gbs']:.0f} GB/s, HBM read {pr['hbm_read_gbs']:.0f} GB/s, "
+                   f"LDS.128 {pr['smem_lds128_gbs']:.0f} GB/s, FSETP {pr['fsetp_gcompares_per_s']:.0f} G compares/s.\n")
+    out.append("| workload | kernel | early exit | kernel ms | call ms | step ms | graph-replay step ms | comparisons/s (step) | "
+               "executed/nominal | bound | achieved GB/s | peak GB/s | roofline frac |")
+    out.append("|---|---|---|---:|---:|---:|---:|---:|---:|---|---:|---:|---:|")
+    for r in rows:
+        if "roofline_frac" not in r:
+            continue
+        g = r.get("graph_replay_step_ms")
+        out.append(f"| {r['workload']} | {r['kernel']} | {'on' if r['early_exit'] else 'off'} | {r['kernel_ms']:.4f} | "
+                   f"{r['call_ms_median']:.4f} | {r['step_ms_median']:.4f} | {g if g is None else format(g, '.4f')} | "
+                   f"{r['comparisons_per_s']:.3g} | {r['executed_over_nominal_visits']:.3f} | {r['roofline_bound']} | "
+                   f"{r['achieved_gbs']:.0f} | {r['peak_gbs']:.0f} | {r['roofline_frac']:.3f} |")
+    out.append("\n| workload | ebic_create: H2D + transpose ms | NaN mask ms | pair-table kernel ms | rank-tile kernel ms | total ms | "
+               "pair table bytes | device bytes |")
+    out.append("|---|---:|---:|---:|---:|---:|---:|---:|")
+    for r in rows:
+        if r.get("kernel") == "ebic_create":
+            b = r["create_breakdown_ms"]
+            out.append(f"| {r['workload']} | {b['h2d_transpose_pad']:.3f} | {b['nan_mask']:.3f} | {b['pair_table']:.3f} | "
+                       f"{b['rank_tiles']:.3f} | {b['total']:.3f} | {r['pair_table_bytes']:,} | {r['device_bytes']:,} |")
+    out.append("\n| workload | extraction source | n chosen | call ms | algorithmic bytes | GB/s | frac of HBM peak |")
+    out.append("|---|---|---:|---:|---:|---:|---:|")
+    for r in rows:
+        if r.get("kernel") == "extract_rows":
+            out.append(f"| {r['workload']} | {r['source']} | {r['n_chosen']} | {r['call_ms_median']:.4f} | {r['bytes']:,} | "
+                       f"{r['hbm_gbs']:.0f} | {r['hbm_frac']:.3f} |")
+    out.append("\n| workload | CPU oracle | rate | sample |")
+    out.append("|---|---|---:|---|")
+    for r in rows:
+        if r.get("kernel") == "cpu_oracle":
+            out.append(f"| {r['workload']} | {r['cores']} host threads | {r['value']:.3g} comparisons/s | {r['sample']} |")
+    return "\n".join(out)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -810,7 +854,12 @@ def main():
     ap.add_argument("--table", action="store_true")
     ap.add_argument("--table-workloads", default="c1,c2,c3,c4,c5")
     ap.add_argument("--table-out", default="table.json")
+    ap.add_argument("--render-table", default=None, metavar="JSON",
+                    help="print the markdown tables of a --table result (e.g. profiles/r02_table.json) and exit; no GPU needed")
     args = ap.parse_args()
+    if args.render_table:
+        print(render_table(args.render_table))
+        return
     if args.warmup < 3 and args.impl == "ebic" and not args.table:
         log("note: fewer than 3 warm-up steps requested; using 3 (timing rules)")
         args.warmup = 3

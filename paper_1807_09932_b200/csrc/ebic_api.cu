@@ -418,7 +418,7 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     ip.pair_stride16 = static_cast<uint32_t>(ctx->ld / 128);
     ip.counts = counts;
     ip.err = ctx->d_err;
-    ingest_population_kernel<<<(n_ind + kIngestBlock - 1) / kIngestBlock, 256, 0, stream>>>(ip);
+    ingest_population_kernel<<<(n_ind + kIngestBlock - 1) / kIngestBlock, kIngestThreads, 0, stream>>>(ip);
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());
 

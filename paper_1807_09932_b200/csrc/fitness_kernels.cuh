@@ -74,6 +74,7 @@ struct TiledParams {
 };
 
 constexpr int kMaxIndPerLaunch = 8192;
+constexpr int kRecIds = 32;          // ids held in an individual's id record (ingest_kernels.cuh)
 constexpr int kSmemHeader = 128;     // 4 mbarriers, padded
 
 __host__ __device__ inline size_t tiled_smem_bytes(int32_t cols, int32_t T, int32_t elem, int32_t n_ind, int32_t nbuf) {
@@ -165,56 +166,53 @@ struct ChainR8 {
     }
 };
 
-// The ids of one individual, four per 32-bit word: words 0..7 come from its id record (one warp-uniform load
-// each), later words are packed on the fly from the caller's int32 ids (valid individual: every id < cols <= 256).
+// The ids of one individual.  Its id record (ingest_kernels.cuh) holds the first 32 ids, four per 32-bit word
+// (cols <= 256) or two per word (wider matrices): one warp-uniform load per word.  A chromosome longer than the
+// record continues, id by id, from the caller's int32 ids (a valid individual: every id is inside [0, cols)); that
+// tail is kept out of the record loop so that the common case pays nothing for it.
 struct IdWords {
     static constexpr int kPerWord = 4;
     const uint32_t* rec;             // idrec + 8 * k
     const int32_t* ids;              // col_ids + b
-    int32_t L;
-    __device__ __forceinline__ uint32_t word(int32_t j) const {
-        if (j < 8) return __ldg(rec + j);
-        const int32_t i = 4 * j, last = L - 1;
-        return static_cast<uint32_t>(__ldg(ids + min(i, last))) | (static_cast<uint32_t>(__ldg(ids + min(i + 1, last))) << 8) |
-               (static_cast<uint32_t>(__ldg(ids + min(i + 2, last))) << 16) | (static_cast<uint32_t>(__ldg(ids + min(i + 3, last))) << 24);
-    }
+    __device__ __forceinline__ uint32_t word(int32_t j) const { return __ldg(rec + j); }
+    __device__ __forceinline__ uint32_t tail_id(int32_t i) const { return static_cast<uint32_t>(__ldg(ids + i)); }
 };
-
-// Matrices of more than 256 columns: two 16-bit ids per word, 16 words per record (ingest_kernels.cuh).
 struct IdWords16 {
     static constexpr int kPerWord = 2;
     const uint32_t* rec;             // idrec + 16 * k
-    const int32_t* ids;              // col_ids + b
-    int32_t L;
-    __device__ __forceinline__ uint32_t word(int32_t j) const {
-        if (j < 16) return __ldg(rec + j);
-        const int32_t i = 2 * j, last = L - 1;
-        return static_cast<uint32_t>(__ldg(ids + min(i, last))) | (static_cast<uint32_t>(__ldg(ids + min(i + 1, last))) << 16);
-    }
+    const int32_t* ids;
+    __device__ __forceinline__ uint32_t word(int32_t j) const { return __ldg(rec + j); }
+    __device__ __forceinline__ uint32_t tail_id(int32_t i) const { return static_cast<uint32_t>(__ldg(ids + i)); }
 };
-
-// The same for an id record that has been staged in shared memory (UNION_F32: admitted individuals have L <= 32).
+// An id record that has been staged in shared memory (UNION_F32: admitted individuals have L <= 32, no tail).
 struct IdWordsShared {
     static constexpr int kPerWord = 4;
     const uint32_t* rec;
     __device__ __forceinline__ uint32_t word(int32_t j) const { return rec[j]; }
+    __device__ __forceinline__ uint32_t tail_id(int32_t) const { return 0u; }
 };
 
-// One chromosome on one slab group.  ids arrive four per word; w0 = first word (already loaded).
-// Full words run branch-free; the (at most two) ragged words go byte by byte.
-// Returns the number of matching rows; adds the number of columns actually visited to `steps`.
-template <class C, class IW>
+// One chromosome on one slab group; w0 = first word of the id record (already loaded).  Full words run
+// branch-free; the ragged last word goes id by id.  Returns the number of matching rows; adds the number of
+// columns actually visited to `steps`.
+// TAIL = false: the caller guarantees L <= kRecIds (the instantiation the hot path runs: the tail's code, when
+// present in the same loop nest, cost the float32 kernel 6 % -- measured in round 2).
+template <bool TAIL, class C, class IW>
 __device__ __forceinline__ int run_chain(C& c, const IW& iw, uint32_t w0, int32_t L,
                                          bool early_exit, int32_t& steps)
 {
+    const int32_t Lr = TAIL ? min(L, kRecIds) : L;        // ids that live in the record
+    int32_t done;
+    bool dead = false;
     if constexpr (IW::kPerWord == 2) {                    // 16-bit ids, two per word
         uint32_t w = w0;
-        uint32_t wn = (L > 2) ? iw.word(1) : 0u;
+        uint32_t wn = (Lr > 2) ? iw.word(1) : 0u;
         c.init(w & 0xffffu);
         c.step(w >> 16);
-        int32_t rem = L - 2, done = 2, j = 1;
+        int32_t rem = Lr - 2, j = 1;
+        done = 2;
         while (rem > 0) {
-            if (early_exit && (j & 1) && !__any_sync(0xffffffffu, c.alive())) break;
+            if (early_exit && (j & 1) && !__any_sync(0xffffffffu, c.alive())) { dead = true; break; }
             w = wn;
             if (rem > 2) wn = iw.word(j + 1);
             ++j;
@@ -223,41 +221,47 @@ __device__ __forceinline__ int run_chain(C& c, const IW& iw, uint32_t w0, int32_
             done += min(rem, 2);
             rem -= 2;
         }
-        steps += done;
-        return c.count();
-    }
-    uint32_t w = w0;
-    uint32_t wn = (L > 4) ? iw.word(1) : 0u;
-    c.init(id_byte(w, 0));
-    int32_t rem = L - 1;                                  // steps still to do; L >= 2
-    int32_t done = 1;
-    {                                                     // bytes 1..3 of word 0
-        c.step(id_byte(w, 1));
-        if (rem >= 2) c.step(id_byte(w, 2));
-        if (rem >= 3) c.step(id_byte(w, 3));
-        const int32_t n0 = min(rem, 3);
-        rem -= n0;
-        done += n0;
-    }
-    int32_t j = 1;
-    while (rem > 0) {
-        if (early_exit && !__any_sync(0xffffffffu, c.alive())) break;
-        w = wn;
-        if (rem > 4) wn = iw.word(j + 1);
-        ++j;
-        if (rem >= 4) {
-            c.step(id_byte(w, 0));
+    } else {
+        uint32_t w = w0;
+        uint32_t wn = (Lr > 4) ? iw.word(1) : 0u;
+        c.init(id_byte(w, 0));
+        int32_t rem = Lr - 1;                             // steps still to do inside the record; L >= 2
+        done = 1;
+        {                                                 // bytes 1..3 of word 0
             c.step(id_byte(w, 1));
-            c.step(id_byte(w, 2));
-            c.step(id_byte(w, 3));
-            rem -= 4;
-            done += 4;
-        } else {
-            c.step(id_byte(w, 0));
-            if (rem >= 2) c.step(id_byte(w, 1));
-            if (rem >= 3) c.step(id_byte(w, 2));
-            done += rem;
-            rem = 0;
+            if (rem >= 2) c.step(id_byte(w, 2));
+            if (rem >= 3) c.step(id_byte(w, 3));
+            const int32_t n0 = min(rem, 3);
+            rem -= n0;
+            done += n0;
+        }
+        int32_t j = 1;
+        while (rem > 0) {
+            if (early_exit && !__any_sync(0xffffffffu, c.alive())) { dead = true; break; }
+            w = wn;
+            if (rem > 4) wn = iw.word(j + 1);
+            ++j;
+            if (rem >= 4) {
+                c.step(id_byte(w, 0));
+                c.step(id_byte(w, 1));
+                c.step(id_byte(w, 2));
+                c.step(id_byte(w, 3));
+                rem -= 4;
+                done += 4;
+            } else {
+                c.step(id_byte(w, 0));
+                if (rem >= 2) c.step(id_byte(w, 1));
+                if (rem >= 3) c.step(id_byte(w, 2));
+                done += rem;
+                rem = 0;
+            }
+        }
+    }
+    if (TAIL && L > kRecIds && !dead) {                   // rare: the chromosome continues beyond its record
+        for (int32_t i = kRecIds; i < L; ++i) {
+            if (early_exit && (i & 3) == 0 && !__any_sync(0xffffffffu, c.alive())) break;
+            c.step(iw.tail_id(i));
+            ++done;
         }
     }
     steps += done;
@@ -274,7 +278,7 @@ struct ElemR8 {
 };
 
 // All slabs of the tile for one individual.  Returns matches; `visited` += rows * columns actually visited.
-template <class IW>
+template <bool TAIL, class IW>
 __device__ __forceinline__ int eval_individual_on_tile(ElemF32, const float* tile, int32_t T, int32_t nslabs, int lane,
                                                         const IW& iw, uint32_t w0, int32_t L,
                                                         bool early_exit, unsigned long long& visited)
@@ -285,13 +289,13 @@ __device__ __forceinline__ int eval_individual_on_tile(ElemF32, const float* til
         ChainF32 c;
         c.base = smem_u32(tile) + (s * kRowsPerSlabF32 + lane * 4) * 4;
         c.stride = static_cast<uint32_t>(T) * 4;
-        cnt += run_chain(c, iw, w0, L, early_exit, steps);
+        cnt += run_chain<TAIL>(c, iw, w0, L, early_exit, steps);
     }
     visited += static_cast<unsigned long long>(steps) * kRowsPerSlabF32;
     return cnt;
 }
 
-template <class IW>
+template <bool TAIL, class IW>
 __device__ __forceinline__ int eval_individual_on_tile(ElemR8, const uint8_t* tile, int32_t T, int32_t nslabs, int lane,
                                                         const IW& iw, uint32_t w0, int32_t L,
                                                         bool early_exit, unsigned long long& visited)
@@ -303,19 +307,19 @@ __device__ __forceinline__ int eval_individual_on_tile(ElemR8, const uint8_t* ti
         ChainR8<4> c;
         c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
         c.stride = static_cast<uint32_t>(T);
-        cnt += run_chain(c, iw, w0, L, early_exit, steps4);
+        cnt += run_chain<TAIL>(c, iw, w0, L, early_exit, steps4);
     }
     for (; s + 2 <= nslabs; s += 2) {
         ChainR8<2> c;
         c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
         c.stride = static_cast<uint32_t>(T);
-        cnt += run_chain(c, iw, w0, L, early_exit, steps2);
+        cnt += run_chain<TAIL>(c, iw, w0, L, early_exit, steps2);
     }
     for (; s < nslabs; ++s) {
         ChainR8<1> c;
         c.base = smem_u32(tile) + s * kRowsPerSlabR8 + lane * 16;
         c.stride = static_cast<uint32_t>(T);
-        cnt += run_chain(c, iw, w0, L, early_exit, steps1);
+        cnt += run_chain<TAIL>(c, iw, w0, L, early_exit, steps1);
     }
     visited += static_cast<unsigned long long>(4 * steps4 + 2 * steps2 + steps1) * kRowsPerSlabR8;
     return cnt;
@@ -402,8 +406,10 @@ fitness_tiled_kernel(const TiledParams p)
                     w_cur = __ldg(p.idrec + static_cast<int64_t>(kRecWords) * (k + NCONS));
                 }
                 if (m.y < 2) continue;
-                const IW iw{p.idrec + static_cast<int64_t>(kRecWords) * k, p.col_ids + m.x, m.y};
-                int cnt = eval_individual_on_tile(E{}, tile, p.T, nslabs, lane, iw, w0, m.y, early_exit, visited);
+                const IW iw{p.idrec + static_cast<int64_t>(kRecWords) * k, p.col_ids + m.x};
+                int cnt = (m.y <= kRecIds)                       // warp-uniform
+                              ? eval_individual_on_tile<false>(E{}, tile, p.T, nslabs, lane, iw, w0, m.y, early_exit, visited)
+                              : eval_individual_on_tile<true>(E{}, tile, p.T, nslabs, lane, iw, w0, m.y, early_exit, visited);
                 cnt = __reduce_add_sync(0xffffffffu, cnt);
                 if (lane == 0 && cnt) atomicAdd(&s_cnt[k], static_cast<unsigned int>(cnt));
             }

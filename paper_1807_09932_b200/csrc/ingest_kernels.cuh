@@ -26,8 +26,8 @@
 namespace ebic {
 
 constexpr int kIngestBlock = 64;     // individuals per CTA = sorting block
+constexpr int kIngestThreads = 1024; // 32 warps: two individuals per warp, so the id loads of a block all overlap
 constexpr int kRecPairs = 30;        // pair offsets held in a record
-constexpr int kRecIds = 32;          // byte ids held in an id record
 
 struct IngestParams {
     const int32_t* offsets;
@@ -48,7 +48,7 @@ struct IngestParams {
     int32_t* err;
 };
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kIngestThreads)
 ingest_population_kernel(const IngestParams p)
 {
     __shared__ int32_t s_b[kIngestBlock];
@@ -83,7 +83,7 @@ ingest_population_kernel(const IngestParams p)
     }
     __syncthreads();
 
-    for (int t = warp; t < kIngestBlock; t += 8) {          // one warp per individual
+    for (int t = warp; t < kIngestBlock; t += kIngestThreads / 32) {   // one warp per individual
         const int32_t L = s_L[t];
         if (L == -2) continue;                              // warp-uniform
         const int32_t k = k0 + t;

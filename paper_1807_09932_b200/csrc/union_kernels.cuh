@@ -247,7 +247,7 @@ fitness_union_kernel(const UnionParams p)
                     ChainF32 c;
                     c.base = smem_u32(tile) + lane * 16;
                     c.stride = kUnionTileRows * 4;
-                    cnt = run_chain(c, iw, w0, m.y, early_exit, steps);
+                    cnt = run_chain<false>(c, iw, w0, m.y, early_exit, steps);
                 } else {
                     cnt = union_direct_chain(p.Mc, p.ld, t * kUnionTileRows, lane, p.col_ids + m.x, m.y, early_exit, steps);
                 }
