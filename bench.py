@@ -390,9 +390,14 @@ def run_gpu(args):
     if world != args.gpus:
         if world == 1 and args.gpus > 1:
             raise SystemExit("launch with torch.distributed.run --nproc-per-node N for --gpus N")
+    if args.one_device:                                        # functional check of the N > 1 path on a single GPU
+        local_rank = 0
     torch.cuda.set_device(local_rank)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if args.dist_backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        else:
+            dist.init_process_group(args.dist_backend)
     peaks, peaks_kind = measured_peaks()
     scaling = args.scaling if world > 1 else "weak"            # one GPU: fixed per-GPU work by definition
 
@@ -553,7 +558,9 @@ def run_gpu(args):
                        "early_exit": bool(args.early_exit), "rows_this_rank": int(local.shape[0]),
                        "l2": "flushed between steps (256 MiB write)",
                        "parallelism": (f"rows sharded x{world} ({scaling}), 1 all-reduce(int64[n_ind]) per step"
-                                       if world > 1 else "1 GPU")},
+                                       if world > 1 else "1 GPU"),
+                       **({"functional_check_only": "all ranks on one GPU: timings are not measurements"}
+                          if args.one_device and world > 1 else {})},
             "individuals_rows_per_s": w.n_ind * (w.rows if scaling == "strong" else w.rows * world) / (ms_per_step * 1e-3),
             "clocks": clk.summary(),
             "e2e": {"value": comparisons / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -842,6 +849,11 @@ def main():
     ap.add_argument("--scaling", default="strong", choices=["strong", "weak"],
                     help="N > 1: strong = one dataset split over the ranks by rows (PAPER.md Fig. 1), weak = every "
                          "rank holds its own `rows` rows")
+    ap.add_argument("--dist-backend", default="nccl", dest="dist_backend",
+                    help="torch.distributed backend for N > 1 (nccl; gloo only for the single-GPU functional check)")
+    ap.add_argument("--one-device", action="store_true", dest="one_device",
+                    help="put every rank on cuda:0: a FUNCTIONAL check of the N > 1 code path where only one GPU exists "
+                         "(with --dist-backend gloo); its timings are not measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-per-workload", action="store_true", help="skip the per_workload block (N = 1) / fig1_shapes")
     ap.add_argument("--per-workload", default="c1,c2,c3,c4,c5,p1,p2,p3", help="workloads of the per_workload block")
