@@ -49,7 +49,7 @@ METRIC = "row_pair_comparisons_per_s"
 UNIT = "comparisons/s"
 N_CHOSEN = 8
 WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4, "p1": 5, "p2": 6, "p3": 7}
-KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "union_f32": 5, "prefix": 6}
+KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "union_f32": 5, "prefix": 6, "pairtile": 7}
 TRAFFIC_CSV = ROOT / "profiles" / "r02_dram_traffic.csv"
 KERNEL_SOURCES = ["pairbits_kernels.cuh", "fitness_kernels.cuh", "union_kernels.cuh", "ebic_device.cuh"]
 
@@ -199,7 +199,8 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
     pipe_basis = (f"max(stated {sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz = {pipe_stated:.0f} GB/s, "
                   f"LDS.128 probe {pipe_probe:.0f} GB/s)" if pipe_probe else
                   f"{sm_count} SMs x 128 B/clk x {f_hz/1e6:.0f} MHz ({peaks_kind} sm_max_mhz)")
-    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "union_f32": 4, "direct": 4, "pairbits": 0.125, "prefix": 0.125}[kernel_name]
+    bytes_per_visit = {"rank8": 1, "tiled_f32": 4, "union_f32": 4, "direct": 4, "pairbits": 0.125, "prefix": 0.125,
+                       "pairtile": 0.125}[kernel_name]
     achieved = visits_executed * bytes_per_visit / kernel_s / 1e9
     bound, peak, basis = "alu", pipe_gbs, pipe_basis
     resource = "shared-memory data pipe (128 B/clk/SM)"
@@ -215,6 +216,20 @@ def roofline(kernel_name, visits_executed, kernel_s, peaks, peaks_kind, sm_count
             if t_hbm > t_pipe:
                 bound, peak, achieved = "hbm", hbm_peak, stage_bytes / kernel_s / 1e9
                 resource = "HBM read of the matrix tiles (staged once per evaluation; population too small to hide it)"
+                basis = f"{peaks_kind} hbm_gbs"
+                bytes_per_visit = stage_bytes / max(visits_executed, 1)
+    elif kernel_name == "pairtile":
+        # one bit per (row, pair) read from the staged tile with LDS.128; second floor: the tile-major table (ALL
+        # cols^2 bit columns) is staged from HBM once per evaluation
+        resource = "shared-memory data pipe (128 B/clk/SM): bit-column tiles staged by TMA, gathered with LDS.128"
+        if ld and cols:
+            stage_bytes = cols * cols * (ld // 8)
+            t_pipe, t_hbm = visits_executed * bytes_per_visit / (pipe_gbs * 1e9), stage_bytes / (hbm_peak * 1e9)
+            extra = {"pipe_floor_ms": t_pipe * 1e3, "hbm_floor_ms": t_hbm * 1e3,
+                     "pair_uses": pairs["uses"] if pairs else None}
+            if t_hbm > t_pipe:
+                bound, peak, achieved = "hbm", hbm_peak, stage_bytes / kernel_s / 1e9
+                resource = "HBM read of the bit-column tiles (staged once per evaluation; population too small to hide it)"
                 basis = f"{peaks_kind} hbm_gbs"
                 bytes_per_visit = stage_bytes / max(visits_executed, 1)
     elif kernel_name == "direct":
@@ -551,7 +566,7 @@ def run_gpu(args):
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": scaling,
-            "vs_baseline": None, "dtype": {"rank8": "u8", "pairbits": "u32"}.get(kernel_name, "f32"), "data": "synthetic",
+            "vs_baseline": None, "dtype": {"rank8": "u8", "pairbits": "u32", "pairtile": "u32", "prefix": "u32"}.get(kernel_name, "f32"), "data": "synthetic",
             "config": {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind,
                        "sum_L": int(w.lengths.sum()), "missing_mode": w.missing_mode, "kernel": kernel_name,
                        "rows_per_task_or_tile": eb.info(5), "ctas": eb.info(6), "n_chosen": int(len(chosen)),

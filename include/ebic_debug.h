@@ -16,16 +16,22 @@ extern "C" {
 
 /* Fitness kernels (all compute include/ebic.h's count[k] exactly). */
 enum {
-    EBIC_KERNEL_AUTO = 0,      /* PAIRBITS if the pair table exists, else RANK8 (cols <= 127), else UNION_F32 /
-                                  TILED_F32 (whichever applies), else DIRECT                                   */
+    EBIC_KERNEL_AUTO = 0,      /* PAIRTILE if the tile-major pair table exists and the matrix has at least SMs / 2
+                                  tiles of 1,024 rows and the population at least 256 individuals, else PAIRBITS
+                                  if the pair table exists, else RANK8 (cols <= 127), else TILED_F32 / UNION_F32
+                                  (whichever applies), else DIRECT                                             */
     EBIC_KERNEL_DIRECT = 1,    /* one thread per row, column-major global loads (any shape)                    */
     EBIC_KERNEL_TILED_F32 = 2, /* float32 row tiles of ALL columns staged in shared memory by TMA bulk copies  */
     EBIC_KERNEL_RANK8 = 3,     /* per-row order-preserving 8-bit rank tiles (cols <= 127)                      */
     EBIC_KERNEL_PAIRBITS = 4,  /* AND of pair-relation bit columns gathered through L2 (pair table built)      */
     EBIC_KERNEL_UNION_F32 = 5, /* float32 tiles of the COLUMN UNION of a batch of individuals (any cols)       */
-    EBIC_KERNEL_PREFIX = 6     /* PAIRBITS with shared-prefix groups: individuals that start with the same
+    EBIC_KERNEL_PREFIX = 6,    /* PAIRBITS with shared-prefix groups: individuals that start with the same
                                   columns share the AND of those bit columns (population <= 8,192; larger
                                   populations run plain PAIRBITS)                                              */
+    EBIC_KERNEL_PAIRTILE = 7   /* 1,024-row tiles of ALL cols^2 bit columns staged in shared memory by TMA and reused
+                                  by the whole population, lane = individual (cols <= 42; needs the tile-major copy
+                                  of the pair table, which ebic_create builds next to the pair-major one when a
+                                  tile fits shared memory)                                                     */
 };
 
 /* Selects the fitness kernel.  EBIC_ERR_ARG if it cannot run this shape (RANK8 builds its rank tiles on demand,
@@ -36,7 +42,9 @@ int ebic_set_kernel(ebic_ctx *ctx, int32_t kernel);
  * Pair-relation table: bit r of pair (a,b) = ( M[r][b] >= M[r][a] ), cols^2 * ceil(rows/1024) * 128 bytes of
  * device memory, one contiguous bit column per ordered pair.  on != 0 builds it if absent (EBIC_ERR_OOM if it
  * does not fit; EBIC_ERR_ARG if cols > 46340 or the table would exceed 64 GiB), on == 0 frees it (and builds
- * the rank tiles if cols <= 127, as ebic_create does when it builds no table).  Synchronises the device.
+ * the rank tiles if cols <= 127, as ebic_create does when it builds no table).  Where a 1,024-row tile of all
+ * cols^2 bit columns fits shared memory (cols <= 42) and memory allows, the build also writes the tile-major copy
+ * of the same bits that PAIRTILE stages (as many bytes again; ebic_set_tuning knob 6).  Synchronises the device.
  */
 int ebic_set_pairbits(ebic_ctx *ctx, int32_t on);
 
@@ -59,6 +67,8 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
  *      (default 1)
  *   4  programmatic dependent launch between the ingest, fitness and extraction kernels (default 1)
  *   5  UNION_F32: individuals per batch (default 0 = chosen from the shape; 1..256)
+ *   6  the next pair-table build also writes the tile-major copy PAIRTILE needs, when a tile fits (default 1)
+ *   7  AUTO picks PAIRTILE from this many 1,024-row tiles on (default 0 = half the SM count)
  * EBIC_ERR_ARG for an unknown knob or a value outside its range.
  */
 int ebic_set_tuning(ebic_ctx *ctx, int32_t knob, int32_t value);
@@ -80,12 +90,13 @@ int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
 
 /*
  * Introspection.  `what`:
- *   0 rows, 1 cols, 2 padded leading dimension ld, 3 missing_mode, 4 kernel ebic_eval_fitness will use,
+ *   0 rows, 1 cols, 2 padded leading dimension ld, 3 missing_mode, 4 kernel ebic_eval_fitness will use (for a
+ *   population of 256 individuals or more),
  *   5 rows per tile / per warp task of the last fitness launch, 6 CTAs of that launch, 7 SM count, 8 kernels
  *   launched by this context so far, 9 bytes of device memory the context owns, 10 executed visits since the
  *   last read, 11 mean fitness-kernel time in ns, 12 evals timed (see ebic_set_instrumentation), 13 early exit
  *   on/off, 14 bytes of the pair table (0 = absent), 15 kernel of the last fitness launch (0 = none yet),
- *   16 bytes of the rank tiles (0 = absent),
+ *   16 bytes of the rank tiles (0 = absent), 17 bytes of the tile-major copy of the pair table (0 = absent),
  *   20..24 ebic_create's time in ns, CUDA events on the legacy stream: 20 host-to-device copy + transpose +
  *   padding, 21 NaN bitmask, 22 pair-table kernel, 23 rank-tile kernel (22 / 23 also when built later on demand;
  *   allocations excluded), 24 all of ebic_create including the allocations.
@@ -97,7 +108,8 @@ int64_t ebic_get_info(ebic_ctx *ctx, int32_t what);
  * Read-back of loader products for parity tests (synchronous D2H copies on the legacy stream).
  *   what = 0 column-major matrix float32 [cols][ld]; 1 NaN bitmask uint32 [cols][ld/32]; 2 per-column
  *   non-missing counts uint64 [cols]; 3 rank tiles uint8 [cols][ld] (EBIC_ERR_ARG if not built);
- *   4 pair table uint32 [cols*cols][ld/32], pair (a,b) = a*cols + b (EBIC_ERR_ARG if not built).
+ *   4 pair table uint32 [cols*cols][ld/32], pair (a,b) = a*cols + b (EBIC_ERR_ARG if not built);
+ *   5 its tile-major copy uint32 [ld/1024][cols*cols][32] (EBIC_ERR_ARG if not built).
  *   dst_bytes must equal the product's size.
  */
 int ebic_debug_read(const ebic_ctx *ctx, int32_t what, void *dst, int64_t dst_bytes);

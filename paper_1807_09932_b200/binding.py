@@ -33,7 +33,9 @@ EBIC_KERNEL_RANK8 = 3
 EBIC_KERNEL_PAIRBITS = 4
 EBIC_KERNEL_UNION_F32 = 5
 EBIC_KERNEL_PREFIX = 6
-KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits", 5: "union_f32", 6: "prefix"}
+EBIC_KERNEL_PAIRTILE = 7
+KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits", 5: "union_f32", 6: "prefix",
+                7: "pairtile"}
 # ebic_set_tuning knobs (include/ebic_debug.h)
 TUNE_PB_TASKS_PER_SLOT, TUNE_PB_PREFETCH, TUNE_PB_SMEM_RING, TUNE_SORT, TUNE_PDL, TUNE_UNION_BATCH = range(6)
 
@@ -456,6 +458,8 @@ class Ebic:
             dst = np.empty((cols, ld), dtype=np.uint8)
         elif what == 4:
             dst = np.empty((cols * cols, ld // 32), dtype=np.uint32)
+        elif what == 5:
+            dst = np.empty((ld // 1024, cols * cols, 32), dtype=np.uint32)
         else:
             raise ValueError(what)
         ebic_debug_read(self._ctx, what, dst)

@@ -18,6 +18,7 @@
 #include "ingest_kernels.cuh"
 #include "loader_kernels.cuh"
 #include "pairbits_kernels.cuh"
+#include "pairtile_kernels.cuh"
 #include "prefix_kernels.cuh"
 #include "union_kernels.cuh"
 
@@ -144,6 +145,17 @@ int32_t union_batch(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
     return static_cast<int32_t>(std::max(4.0, std::min(128.0, b))) & ~1;       // even: the records are copied 16 bytes at a time
 }
 
+// PAIRTILE: a 1,024-row tile of all cols^2 bit columns next to one 4-byte counter per individual of the launch.
+int64_t pairtile_smem(const ebic_ctx* ctx, int32_t n_ind_launch) {
+    return kPtHeader + static_cast<int64_t>(ctx->cols) * ctx->cols * 128 + 4ll * ((n_ind_launch + 31) / 32 * 32);
+}
+bool pairtile_fits(const ebic_ctx* ctx) { return ctx->cols <= 90 && pairtile_smem(ctx, 1024) <= ctx->smem_optin; }
+// Individuals per launch: as many counters as fit next to the tile, at most kMaxIndPerLaunch.
+int32_t pairtile_chunk(const ebic_ctx* ctx, int32_t n_ind) {
+    const int64_t room = (static_cast<int64_t>(ctx->smem_optin) - pairtile_smem(ctx, 0)) / 4 / 32 * 32;
+    return static_cast<int32_t>(std::min<int64_t>(std::min<int64_t>(n_ind, kMaxIndPerLaunch), room));
+}
+
 int32_t tile_rows(const ebic_ctx* ctx, int32_t kernel, int32_t n_ind_launch) {
     return kernel == EBIC_KERNEL_RANK8 ? tile_rows_r8(ctx, n_ind_launch) : tile_rows_f32(ctx, n_ind_launch);
 }
@@ -190,13 +202,17 @@ bool kernel_applies(const ebic_ctx* ctx, int32_t kernel) {
         case EBIC_KERNEL_RANK8: return tile_rows_r8(ctx, 1024) > 0;
         case EBIC_KERNEL_PAIRBITS:
         case EBIC_KERNEL_PREFIX: return ctx->PB != nullptr;
+        case EBIC_KERNEL_PAIRTILE: return ctx->PBT != nullptr;
         case EBIC_KERNEL_UNION_F32: return union_cap(ctx) >= 2;
         default: return false;
     }
 }
 
-int32_t resolve_kernel(const ebic_ctx* ctx, int32_t /*n_ind_launch*/) {
+int32_t resolve_kernel(const ebic_ctx* ctx, int32_t n_ind_launch) {
     if (ctx->kernel_request != EBIC_KERNEL_AUTO) return ctx->kernel_request;
+    // tiles in shared memory pay once there are enough (tile, group) items to keep every SM busy for a while
+    const int64_t min_tiles = ctx->pt_min_tiles > 0 ? ctx->pt_min_tiles : ctx->sm_count / 2;
+    if (ctx->PBT && ctx->ld / kPairTileRows >= min_tiles && n_ind_launch >= 256) return EBIC_KERNEL_PAIRTILE;
     if (ctx->PB) return EBIC_KERNEL_PAIRBITS;
     if (ctx->Rk && kernel_applies(ctx, EBIC_KERNEL_RANK8)) return EBIC_KERNEL_RANK8;
     if (kernel_applies(ctx, EBIC_KERNEL_TILED_F32)) return EBIC_KERNEL_TILED_F32;   // every column fits a tile
@@ -232,9 +248,17 @@ int build_pairbits(ebic_ctx* ctx) {
     int st = dev_alloc(ctx, reinterpret_cast<void**>(&ctx->PB), bytes);
     if (st) return st;
     ctx->pb_bytes = bytes;
+    // the tile-major copy for PAIRTILE, when a tile fits shared memory and the memory is there (never an error)
+    if (ctx->pt_build && pairtile_fits(ctx)) {
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess && bytes <= static_cast<int64_t>(free_b / 2) &&
+            dev_alloc(ctx, reinterpret_cast<void**>(&ctx->PBT), bytes) == EBIC_OK)
+            ctx->pbt_bytes = bytes;
+        cudaGetLastError();
+    }
     BuildTimer timer(&ctx->create_ms[2]);                        // the kernel, not the allocation
     EBIC_TRY(cudaFuncSetAttribute(pairbits_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * kPairStageBytes));
-    pairbits_kernel<<<grid, 256, 2 * kPairStageBytes>>>(ctx->Mc, ctx->nanmask, ctx->ld, ctx->cols, ctx->PB);
+    pairbits_kernel<<<grid, 256, 2 * kPairStageBytes>>>(ctx->Mc, ctx->nanmask, ctx->ld, ctx->cols, ctx->PB, ctx->PBT);
     ctx->launches++;
     st = cuda_status(cudaGetLastError());
     if (!st) st = cuda_status(cudaDeviceSynchronize());
@@ -247,6 +271,12 @@ void free_pairbits(ebic_ctx* ctx) {
     ctx->bytes_owned -= ctx->pb_bytes;
     ctx->PB = nullptr;
     ctx->pb_bytes = 0;
+    if (ctx->PBT) {
+        cudaFree(ctx->PBT);
+        ctx->bytes_owned -= ctx->pbt_bytes;
+        ctx->PBT = nullptr;
+        ctx->pbt_bytes = 0;
+    }
 }
 
 }  // namespace ebic_host
@@ -365,6 +395,36 @@ int launch_pairbits(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_ind, int64_
     return ebic_host::cuda_status(e);
 }
 
+// PAIRTILE: plan (sort by length, transposed pair-slot records) + the persistent tile kernel, per population chunk.
+int launch_pairtile(ebic_ctx* ctx, const int32_t* col_ids, int32_t k0, int32_t n_ind, unsigned long long* counts,
+                    cudaStream_t stream, bool pdl_plan, bool pdl_fit, bool with_events, int slot) {
+    PairtileParams p;
+    p.PBT = ctx->PBT;
+    p.n_tiles = ctx->ld / kPairTileRows;
+    p.n_pairs = ctx->cols * ctx->cols;
+    p.cols = ctx->cols;
+    p.n_ind = n_ind;
+    p.n_groups = (n_ind + 31) / 32;
+    p.meta = ctx->meta + k0;
+    p.col_ids = col_ids;
+    p.gmeta = static_cast<int2*>(ctx->tplan);
+    p.tids = reinterpret_cast<uint4*>(static_cast<unsigned char*>(ctx->tplan) + 256ll * ((kMaxIndPerLaunch + 31) / 32));
+    p.counts = counts + k0;
+    p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
+    ctx->launches += 2;
+    EBIC_TRY(launch_pdl(pairtile_plan_kernel, dim3((n_ind + kPtPlanThreads - 1) / kPtPlanThreads), dim3(kPtPlanThreads), 0,
+                        stream, pdl_plan, p));
+    if (with_events) EBIC_TRY(cudaEventRecord(ctx->ev_begin[slot], stream));
+    const size_t smem = static_cast<size_t>(pairtile_smem(ctx, n_ind));
+    EBIC_TRY(cudaFuncSetAttribute(fitness_pairtile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+    const int64_t items = p.n_tiles * p.n_groups;
+    const int64_t grid = std::min<int64_t>(ctx->sm_count, items);
+    ctx->last_grid = static_cast<int32_t>(grid);
+    ctx->last_T = kPairTileRows;
+    return ebic_host::cuda_status(launch_pdl(fitness_pairtile_kernel, dim3(static_cast<unsigned>(grid)), dim3(kPtWarps * 32), smem,
+                                             stream, pdl_fit, p));
+}
+
 // Population already on the device: ingest + chain kernels.
 int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, int32_t n_ind, int64_t n_ids,
                 unsigned long long* counts, cudaStream_t stream) {
@@ -388,6 +448,11 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
         up.n_batches = (n_ind + up.batch - 1) / up.batch;
         up.u_cap = union_cap(ctx);
         st = grow(ctx, reinterpret_cast<void**>(&ctx->ubatch), &ctx->ubatch_cap, 4ll * up.n_batches * (up.u_cap + 1));
+        if (st) return st;
+    }
+    const bool by_tile = kernel0 == EBIC_KERNEL_PAIRTILE;
+    if (by_tile) {                                          // gmeta (8 B) + four uint4 of pair slots (64 B) per sorted position
+        st = grow(ctx, &ctx->tplan, &ctx->tplan_cap, (256ll + 2048ll) * ((kMaxIndPerLaunch + 31) / 32));
         if (st) return st;
     }
     const bool by_prefix = kernel0 == EBIC_KERNEL_PREFIX && n_ind <= kPrefixMaxInd;     // larger populations: plain PAIRBITS
@@ -450,10 +515,20 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
             EBIC_TRY(cudaEventCreate(&ctx->ev_begin[slot]));
             EBIC_TRY(cudaEventCreate(&ctx->ev_end[slot]));
         }
-        EBIC_TRY(cudaEventRecord(ctx->ev_begin[slot], stream));
+        if (!by_tile) EBIC_TRY(cudaEventRecord(ctx->ev_begin[slot], stream));   // PAIRTILE: behind its plan kernel (a3)
     }
     ctx->last_kernel = kernel0;
-    if (by_prefix) {
+    if (by_tile) {
+        const int32_t per_launch = pairtile_chunk(ctx, n_ind);
+        for (int32_t k0 = 0; k0 < n_ind; k0 += per_launch) {
+            const int32_t n = std::min<int32_t>(per_launch, n_ind - k0);
+            // only the first chunk follows the ingest directly; later chunks reuse the plan buffers, so they are
+            // ordered behind the previous chunk's kernel
+            st = launch_pairtile(ctx, col_ids, k0, n, counts, stream, ctx->pdl && k0 == 0, pdl && k0 == 0,
+                                 ctx->time_kernels && k0 == 0, slot);
+            if (st) return st;
+        }
+    } else if (by_prefix) {
         st = launch_prefix(ctx, col_ids, n_ind, n_ids, counts, stream, pdl);
         if (st) return st;
     } else if (by_pairs) {
@@ -663,6 +738,8 @@ int ebic_destroy(ebic_ctx* ctx) {
     cudaFree(ctx->nonmissing);
     cudaFree(ctx->Rk);
     cudaFree(ctx->PB);
+    cudaFree(ctx->PBT);
+    cudaFree(ctx->tplan);
     cudaFree(ctx->prec);
     cudaFree(ctx->d_err);
     cudaFree(ctx->meta);

@@ -21,6 +21,8 @@ struct ebic_ctx {
     uint8_t* Rk = nullptr;                     // [cols][ld] rank tiles, built when AUTO would use them or on request
     uint32_t* PB = nullptr;                    // pair bit columns [cols*cols][ld/32] or nullptr
     int64_t pb_bytes = 0;
+    uint32_t* PBT = nullptr;                   // the same bits, tile-major [ld/1024][cols*cols][32 words] (PAIRTILE) or nullptr
+    int64_t pbt_bytes = 0;
     int32_t* d_err = nullptr;                  // sticky device error (+ the executed-visit counter behind it)
     unsigned long long* d_visits = nullptr;
 
@@ -31,6 +33,8 @@ struct ebic_ctx {
     int64_t idrec_cap = 0;
     uint32_t* prec = nullptr;                  // 128 bytes per individual (pair table present)
     int64_t prec_cap = 0;
+    void* tplan = nullptr;                     // PAIRTILE: sorted {k, n} and the transposed pair-slot records
+    int64_t tplan_cap = 0;
     int32_t* ubatch = nullptr;                 // column-union kernel: per-batch column lists and remapped ids
     int64_t ubatch_cap = 0;
     void* stage[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // staging for host-pointer calls
@@ -43,6 +47,8 @@ struct ebic_ctx {
     int32_t pb_tasks_per_slot = 8;             // PAIRBITS: warp tasks per resident warp slot
     int32_t pb_prefetch_dist = 1;              // PAIRBITS: L2 prefetch distance in chunks (0 = off)
     int32_t pb_smem_ring = 1;                  // PAIRBITS: shared-memory landing ring for long chromosomes
+    int32_t pt_build = 1;                      // build the tile-major copy of the pair table when a tile fits shared memory
+    int32_t pt_min_tiles = 0;                  // AUTO picks PAIRTILE from this many 1,024-row tiles on (0 = half the SM count)
     int32_t pb_sort = 1;                       // ingest sorts each 64-individual block by length
     int32_t pdl = 1;                           // programmatic dependent launch between ingest / fitness / extraction
     int32_t union_batch = 0;                   // UNION_F32: individuals per batch (0 = chosen from the shape)

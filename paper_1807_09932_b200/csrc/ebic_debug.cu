@@ -20,7 +20,7 @@ using ebic_host::cuda_status;
 extern "C" {
 
 int ebic_set_kernel(ebic_ctx* ctx, int32_t kernel) {
-    if (!ctx || kernel < EBIC_KERNEL_AUTO || kernel > EBIC_KERNEL_PREFIX) return EBIC_ERR_ARG;
+    if (!ctx || kernel < EBIC_KERNEL_AUTO || kernel > EBIC_KERNEL_PAIRTILE) return EBIC_ERR_ARG;
     if (!ebic_host::kernel_applies(ctx, kernel)) return EBIC_ERR_ARG;
     if (kernel == EBIC_KERNEL_RANK8) {
         if (cudaDeviceSynchronize() != cudaSuccess) return cuda_status(cudaGetLastError());
@@ -36,7 +36,9 @@ int ebic_set_pairbits(ebic_ctx* ctx, int32_t on) {
     if (cudaDeviceSynchronize() != cudaSuccess) return cuda_status(cudaGetLastError());
     if (on == 0) {
         ebic_host::free_pairbits(ctx);
-        if (ctx->kernel_request == EBIC_KERNEL_PAIRBITS) ctx->kernel_request = EBIC_KERNEL_AUTO;
+        if (ctx->kernel_request == EBIC_KERNEL_PAIRBITS || ctx->kernel_request == EBIC_KERNEL_PREFIX ||
+            ctx->kernel_request == EBIC_KERNEL_PAIRTILE)
+            ctx->kernel_request = EBIC_KERNEL_AUTO;
         if (ctx->cols <= 127) return ebic_host::build_rank_tiles(ctx);
         return EBIC_OK;
     }
@@ -75,6 +77,11 @@ int ebic_set_tuning(ebic_ctx* ctx, int32_t knob, int32_t value) {
             if (value < 0 || value > 256) return EBIC_ERR_ARG;
             ctx->union_batch = value;
             return EBIC_OK;
+        case 6: ctx->pt_build = value ? 1 : 0; return EBIC_OK;
+        case 7:
+            if (value < 0) return EBIC_ERR_ARG;
+            ctx->pt_min_tiles = value;
+            return EBIC_OK;
         default: return EBIC_ERR_ARG;
     }
 }
@@ -94,7 +101,7 @@ int64_t ebic_get_info(ebic_ctx* ctx, int32_t what) {
         case 1: return ctx->cols;
         case 2: return ctx->ld;
         case 3: return ctx->missing_mode;
-        case 4: return ebic_host::resolve_kernel(ctx, 1);
+        case 4: return ebic_host::resolve_kernel(ctx, 0x7fffffff);
         case 5: return ctx->last_T;
         case 6: return ctx->last_grid;
         case 7: return ctx->sm_count;
@@ -132,6 +139,7 @@ int64_t ebic_get_info(ebic_ctx* ctx, int32_t what) {
         case 14: return ctx->pb_bytes;
         case 15: return ctx->last_kernel;
         case 16: return ctx->Rk ? ctx->ld * ctx->cols : 0;
+        case 17: return ctx->pbt_bytes;
         case 20: case 21: case 22: case 23: case 24:
             return static_cast<int64_t>(static_cast<double>(ctx->create_ms[what - 20]) * 1e6);
         default: return -1;
@@ -149,6 +157,7 @@ int ebic_debug_read(const ebic_ctx* ctx, int32_t what, void* dst, int64_t dst_by
         case 2: src = ctx->nonmissing; bytes = static_cast<int64_t>(ctx->cols) * 8; break;
         case 3: src = ctx->Rk; bytes = n; break;
         case 4: src = ctx->PB; bytes = ctx->pb_bytes; break;
+        case 5: src = ctx->PBT; bytes = ctx->pbt_bytes; break;
         default: return EBIC_ERR_ARG;
     }
     if (!src || bytes != dst_bytes) return EBIC_ERR_ARG;

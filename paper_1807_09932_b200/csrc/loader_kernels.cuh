@@ -146,7 +146,7 @@ __device__ __forceinline__ void pair_words(const float (&va0)[32], const float (
 
 __global__ void __launch_bounds__(256, 2)
 pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanmask, int64_t ld, int32_t cols,
-                uint32_t* __restrict__ PB)
+                uint32_t* __restrict__ PB, uint32_t* __restrict__ PBT)
 {
     extern __shared__ __align__(16) unsigned char pb_stage[];   // 2 x kPairStageBytes
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -190,6 +190,11 @@ pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanma
     // running pointers: the words of pairs (a0, b) / (a1, b) and the NaN word of column b, b = 0, 1, 2, ...
     uint32_t* out0 = PB + static_cast<int64_t>(min(a0, cols - 1)) * cols * ldw + t * 32 + lane;
     uint32_t* out1 = PB + static_cast<int64_t>(min(a1, cols - 1)) * cols * ldw + t * 32 + lane;
+    // optional second copy, TILE-major PBT[tile][pair][32 words] (pairtile_kernels.cuh stages whole tiles): the
+    // same 128-byte store, 128 bytes further on for every b
+    const bool tiled = PBT != nullptr;
+    uint32_t* tout0 = PBT + (t * cols * cols + static_cast<int64_t>(min(a0, cols - 1)) * cols) * 32 + lane;
+    uint32_t* tout1 = PBT + (t * cols * cols + static_cast<int64_t>(min(a1, cols - 1)) * cols) * 32 + lane;
     const uint32_t* nan_b = nan_t;
     const bool do0 = a0 < cols, do1 = a1 < cols;
     const int32_t n_stage = (cols + kPairCB - 1) / kPairCB;
@@ -204,7 +209,7 @@ pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanma
         __syncthreads();                                         // every thread's share of stage s has landed
         uint32_t src = stage0 + (s & 1) * kPairStageBytes + lane * kPairLaneStride;
         const int32_t b_end = min(kPairCB, cols - s * kPairCB);
-        for (int32_t c = 0; c < b_end; ++c, src += kPairColBytes, out0 += ldw, out1 += ldw, nan_b += ldw) {
+        for (int32_t c = 0; c < b_end; ++c, src += kPairColBytes, out0 += ldw, out1 += ldw, tout0 += 32, tout1 += 32, nan_b += ldw) {
             float vb[32];
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
@@ -215,8 +220,12 @@ pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanma
             const uint32_t pb = ~__ldg(nan_b);
             uint32_t w0, w1;
             pair_words(va0, va1, vb, w0, w1);
-            if (do0) *out0 = w0 & pa0 & pb;
-            if (do1) *out1 = w1 & pa1 & pb;
+            w0 &= pa0 & pb;
+            w1 &= pa1 & pb;
+            if (do0) *out0 = w0;
+            if (do1) *out1 = w1;
+            if (tiled && do0) *tout0 = w0;
+            if (tiled && do1) *tout1 = w1;
         }
         __syncthreads();                                         // stage s may be overwritten by stage s + 2
     }

@@ -1,7 +1,7 @@
 """Parity of the CUDA path (through the C ABI, via the thin binding) against the CPU oracle.
 
 Bar: bit-exact (integer counts and bitmasks from exact float32 comparisons; tolerance 0).
-Every fitness kernel (DIRECT, TILED_F32, RANK8, PAIRBITS, UNION_F32, PREFIX) is compared with the oracle on the same seeded
+Every fitness kernel (DIRECT, TILED_F32, RANK8, PAIRBITS, UNION_F32, PREFIX, PAIRTILE) is compared with the oracle on the same seeded
 inputs.  All tests here need the B200.
 """
 from __future__ import annotations
@@ -29,7 +29,7 @@ def B():
 def kernels_for(eb, B):
     ks = [B.EBIC_KERNEL_DIRECT]
     for k in (B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_UNION_F32,
-              B.EBIC_KERNEL_PREFIX):
+              B.EBIC_KERNEL_PREFIX, B.EBIC_KERNEL_PAIRTILE):
         try:
             eb.set_kernel(k)
             ks.append(k)
@@ -133,6 +133,12 @@ def test_loader_products(B, rows, cols, nan_rate):
             want = np.ascontiguousarray(np.packbits(ge.reshape(ld, cols * cols).T, axis=1,
                                                     bitorder="little")).view(np.uint32)
             assert (pb == want).all()
+            if cols * cols * 128 + 128 + 4096 <= 232448:       # a 1,024-row tile of all bit columns fits shared memory:
+                pbt = eb.debug_read(5)                         # the tile-major copy holds the same words
+                assert eb.info(17) == pbt.nbytes
+                assert (pbt == want.reshape(cols * cols, ld // 1024, 32).transpose(1, 0, 2)).all()
+            else:
+                assert eb.info(17) == 0
 
 
 # ------------------------------------------------------------------------- hand fixtures on the GPU
