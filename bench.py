@@ -716,7 +716,7 @@ def run_table(args):
         d_masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
         d_mcnt = torch.empty(len(chosen), dtype=torch.int64, device="cuda")
         pstats = pair_stats(w)
-        for kname, ee in (("pairbits", 0), ("pairbits", 1), ("rank8", 0), ("rank8", 1), ("tiled_f32", 0),
+        for kname, ee in (("pairtile", 0), ("pairbits", 0), ("pairbits", 1), ("rank8", 0), ("rank8", 1), ("tiled_f32", 0),
                           ("tiled_f32", 1), ("union_f32", 0), ("union_f32", 1), ("direct", 0)):
             if kname == "direct" and w.comparisons > 2e10:
                 continue

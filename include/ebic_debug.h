@@ -16,10 +16,11 @@ extern "C" {
 
 /* Fitness kernels (all compute include/ebic.h's count[k] exactly). */
 enum {
-    EBIC_KERNEL_AUTO = 0,      /* PAIRTILE if the tile-major pair table exists and the matrix has at least SMs / 2
-                                  tiles of 1,024 rows and the population at least 256 individuals, else PAIRBITS
-                                  if the pair table exists, else RANK8 (cols <= 127), else TILED_F32 / UNION_F32
-                                  (whichever applies), else DIRECT                                             */
+    EBIC_KERNEL_AUTO = 0,      /* PAIRTILE if the tile-major pair table exists and the evaluation is large enough
+                                  for staged tiles to pay (>= 4e6 (tile, pair-use) units, more when the
+                                  population uses each bit column fewer than 16 times), else PAIRBITS if the pair
+                                  table exists, else RANK8 (cols <= 127), else TILED_F32 / UNION_F32 (whichever
+                                  applies), else DIRECT                                                        */
     EBIC_KERNEL_DIRECT = 1,    /* one thread per row, column-major global loads (any shape)                    */
     EBIC_KERNEL_TILED_F32 = 2, /* float32 row tiles of ALL columns staged in shared memory by TMA bulk copies  */
     EBIC_KERNEL_RANK8 = 3,     /* per-row order-preserving 8-bit rank tiles (cols <= 127)                      */
@@ -68,7 +69,9 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
  *   4  programmatic dependent launch between the ingest, fitness and extraction kernels (default 1)
  *   5  UNION_F32: individuals per batch (default 0 = chosen from the shape; 1..256)
  *   6  the next pair-table build also writes the tile-major copy PAIRTILE needs, when a tile fits (default 1)
- *   7  AUTO picks PAIRTILE from this many 1,024-row tiles on (default 0 = half the SM count)
+ *   7  AUTO picks PAIRTILE from this many (1,024-row tile, consecutive-pair use) units on (default 0 = the rule
+ *      stated at EBIC_KERNEL_AUTO)
+ *   8  PAIRTILE loads the part of the next tile that fits shared memory a second time one tile ahead (default 1)
  * EBIC_ERR_ARG for an unknown knob or a value outside its range.
  */
 int ebic_set_tuning(ebic_ctx *ctx, int32_t knob, int32_t value);
@@ -90,8 +93,8 @@ int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
 
 /*
  * Introspection.  `what`:
- *   0 rows, 1 cols, 2 padded leading dimension ld, 3 missing_mode, 4 kernel ebic_eval_fitness will use (for a
- *   population of 256 individuals or more),
+ *   0 rows, 1 cols, 2 padded leading dimension ld, 3 missing_mode, 4 kernel ebic_eval_fitness will use for a
+ *   population shaped like the last one evaluated (before any: 1,600 individuals of 11 columns),
  *   5 rows per tile / per warp task of the last fitness launch, 6 CTAs of that launch, 7 SM count, 8 kernels
  *   launched by this context so far, 9 bytes of device memory the context owns, 10 executed visits since the
  *   last read, 11 mean fitness-kernel time in ns, 12 evals timed (see ebic_set_instrumentation), 13 early exit

@@ -149,6 +149,13 @@ int32_t union_batch(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
 int64_t pairtile_smem(const ebic_ctx* ctx, int32_t n_ind_launch) {
     return kPtHeader + static_cast<int64_t>(ctx->cols) * ctx->cols * 128 + 4ll * ((n_ind_launch + 31) / 32 * 32);
 }
+// Slots of a tile that fit a second time next to the tile and the counters (0: not worth splitting).
+int32_t pairtile_lo_slots(const ebic_ctx* ctx, int32_t n_ind_launch) {
+    const int64_t n_pairs = static_cast<int64_t>(ctx->cols) * ctx->cols;
+    const int64_t room = (static_cast<int64_t>(ctx->smem_optin) - pairtile_smem(ctx, n_ind_launch)) / 128;
+    const int64_t lo = std::min<int64_t>(std::max<int64_t>(room, 0), n_pairs);
+    return lo * 8 >= n_pairs ? static_cast<int32_t>(lo) : 0;
+}
 bool pairtile_fits(const ebic_ctx* ctx) { return ctx->cols <= 90 && pairtile_smem(ctx, 1024) <= ctx->smem_optin; }
 // Individuals per launch: as many counters as fit next to the tile, at most kMaxIndPerLaunch.
 int32_t pairtile_chunk(const ebic_ctx* ctx, int32_t n_ind) {
@@ -208,11 +215,22 @@ bool kernel_applies(const ebic_ctx* ctx, int32_t kernel) {
     }
 }
 
-int32_t resolve_kernel(const ebic_ctx* ctx, int32_t n_ind_launch) {
+// PAIRTILE against PAIRBITS (both need the table; measured on 20 / 32 / 40 columns x 30 k .. 1.5 M rows x 128 .. 4,096
+// individuals): staging whole tiles pays once (a) there are enough (tile, pair-use) units to keep
+// every SM busy past the fixed cost of the extra launch, and (b) the population uses every staged bit column
+// several times -- a small population reads only the columns it needs through PAIRBITS.
+bool pairtile_pays(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
+    if (!ctx->PBT) return false;
+    const int64_t tiles = ctx->ld / kPairTileRows, uses = std::max<int64_t>(n_ids - n_ind, 0);
+    const int64_t n_pairs = static_cast<int64_t>(ctx->cols) * ctx->cols;
+    if (ctx->pt_min_work > 0) return tiles * uses >= ctx->pt_min_work;
+    const double reuse_penalty = std::max(1.0, 16.0 * n_pairs / static_cast<double>(std::max<int64_t>(uses, 1)));
+    return static_cast<double>(tiles) * uses >= 4.0e6 * reuse_penalty;
+}
+
+int32_t resolve_kernel(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
     if (ctx->kernel_request != EBIC_KERNEL_AUTO) return ctx->kernel_request;
-    // tiles in shared memory pay once there are enough (tile, group) items to keep every SM busy for a while
-    const int64_t min_tiles = ctx->pt_min_tiles > 0 ? ctx->pt_min_tiles : ctx->sm_count / 2;
-    if (ctx->PBT && ctx->ld / kPairTileRows >= min_tiles && n_ind_launch >= 256) return EBIC_KERNEL_PAIRTILE;
+    if (pairtile_pays(ctx, n_ind, n_ids)) return EBIC_KERNEL_PAIRTILE;
     if (ctx->PB) return EBIC_KERNEL_PAIRBITS;
     if (ctx->Rk && kernel_applies(ctx, EBIC_KERNEL_RANK8)) return EBIC_KERNEL_RANK8;
     if (kernel_applies(ctx, EBIC_KERNEL_TILED_F32)) return EBIC_KERNEL_TILED_F32;   // every column fits a tile
@@ -405,6 +423,7 @@ int launch_pairtile(ebic_ctx* ctx, const int32_t* col_ids, int32_t k0, int32_t n
     p.cols = ctx->cols;
     p.n_ind = n_ind;
     p.n_groups = (n_ind + 31) / 32;
+    p.lo_slots = ctx->pt_split ? pairtile_lo_slots(ctx, n_ind) : 0;
     p.meta = ctx->meta + k0;
     p.col_ids = col_ids;
     p.gmeta = static_cast<int2*>(ctx->tplan);
@@ -415,7 +434,7 @@ int launch_pairtile(ebic_ctx* ctx, const int32_t* col_ids, int32_t k0, int32_t n
     EBIC_TRY(launch_pdl(pairtile_plan_kernel, dim3((n_ind + kPtPlanThreads - 1) / kPtPlanThreads), dim3(kPtPlanThreads), 0,
                         stream, pdl_plan, p));
     if (with_events) EBIC_TRY(cudaEventRecord(ctx->ev_begin[slot], stream));
-    const size_t smem = static_cast<size_t>(pairtile_smem(ctx, n_ind));
+    const size_t smem = static_cast<size_t>(pairtile_smem(ctx, n_ind)) + 128ull * p.lo_slots;
     EBIC_TRY(cudaFuncSetAttribute(fitness_pairtile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
     const int64_t items = p.n_tiles * p.n_groups;
     const int64_t grid = std::min<int64_t>(ctx->sm_count, items);
@@ -428,7 +447,9 @@ int launch_pairtile(ebic_ctx* ctx, const int32_t* col_ids, int32_t k0, int32_t n
 // Population already on the device: ingest + chain kernels.
 int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, int32_t n_ind, int64_t n_ids,
                 unsigned long long* counts, cudaStream_t stream) {
-    const int32_t kernel0 = ebic_host::resolve_kernel(ctx, n_ind);
+    const int32_t kernel0 = ebic_host::resolve_kernel(ctx, n_ind, n_ids);
+    ctx->last_n_ind = n_ind;
+    ctx->last_n_ids = n_ids;
     if (!ebic_host::kernel_applies(ctx, kernel0)) return EBIC_ERR_ARG;
     const bool tiled = kernel0 == EBIC_KERNEL_RANK8 || kernel0 == EBIC_KERNEL_TILED_F32;
     if (kernel0 == EBIC_KERNEL_RANK8 && !ctx->Rk) {

@@ -48,7 +48,8 @@ struct ebic_ctx {
     int32_t pb_prefetch_dist = 1;              // PAIRBITS: L2 prefetch distance in chunks (0 = off)
     int32_t pb_smem_ring = 1;                  // PAIRBITS: shared-memory landing ring for long chromosomes
     int32_t pt_build = 1;                      // build the tile-major copy of the pair table when a tile fits shared memory
-    int32_t pt_min_tiles = 0;                  // AUTO picks PAIRTILE from this many 1,024-row tiles on (0 = half the SM count)
+    int32_t pt_split = 1;                      // PAIRTILE: load the part of the next tile that fits a second time ahead
+    int32_t pt_min_work = 0;                   // AUTO picks PAIRTILE from this many (tile, pair-use) units on (0 = the rule of pairtile_pays)
     int32_t pb_sort = 1;                       // ingest sorts each 64-individual block by length
     int32_t pdl = 1;                           // programmatic dependent launch between ingest / fitness / extraction
     int32_t union_batch = 0;                   // UNION_F32: individuals per batch (0 = chosen from the shape)
@@ -67,6 +68,8 @@ struct ebic_ctx {
     int32_t last_grid = 0;
     int32_t last_T = 0;
     int32_t last_kernel = 0;                   // kernel of the last fitness launch (0 = none yet)
+    int32_t last_n_ind = 1600;                 // shape of the last population (before any: the paper's typical 1,600
+    int64_t last_n_ids = 17600;                // individuals, of 11 columns): what info(4) resolves AUTO for
 };
 
 namespace ebic_host {
@@ -75,7 +78,7 @@ int cuda_status(cudaError_t e);
 int build_pairbits(ebic_ctx* ctx);             // synchronous; EBIC_OK if already built
 void free_pairbits(ebic_ctx* ctx);
 int build_rank_tiles(ebic_ctx* ctx);           // synchronous; EBIC_ERR_ARG if cols > 127
-int32_t resolve_kernel(const ebic_ctx* ctx, int32_t n_ind_launch);
+int32_t resolve_kernel(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids);
 bool kernel_applies(const ebic_ctx* ctx, int32_t kernel);
 
 }  // namespace ebic_host

@@ -80,8 +80,9 @@ int ebic_set_tuning(ebic_ctx* ctx, int32_t knob, int32_t value) {
         case 6: ctx->pt_build = value ? 1 : 0; return EBIC_OK;
         case 7:
             if (value < 0) return EBIC_ERR_ARG;
-            ctx->pt_min_tiles = value;
+            ctx->pt_min_work = value;
             return EBIC_OK;
+        case 8: ctx->pt_split = value ? 1 : 0; return EBIC_OK;
         default: return EBIC_ERR_ARG;
     }
 }
@@ -101,7 +102,7 @@ int64_t ebic_get_info(ebic_ctx* ctx, int32_t what) {
         case 1: return ctx->cols;
         case 2: return ctx->ld;
         case 3: return ctx->missing_mode;
-        case 4: return ebic_host::resolve_kernel(ctx, 0x7fffffff);
+        case 4: return ebic_host::resolve_kernel(ctx, ctx->last_n_ind, ctx->last_n_ids);
         case 5: return ctx->last_T;
         case 6: return ctx->last_grid;
         case 7: return ctx->sm_count;

@@ -26,9 +26,11 @@
 // columns continue from the caller's col_ids.
 //
 // Persistent CTAs, one per SM, 16 warps.  Work = (tile, group) items in tile-major order cut into equal contiguous
-// ranges (a tile is staged by at most two CTAs more than necessary).  One tile buffer: while the warps work on tile
-// t, tile t + 1 is requested into L2 (cp.async.bulk.prefetch.L2); when the last warp is done the buffer is refilled
-// from L2 with one TMA bulk copy per 16 KB, completion on an mbarrier.
+// ranges (a tile is staged by at most two CTAs more than necessary); inside a tile the groups are handed out
+// longest first through a shared-memory cursor.  Tiles are staged with TMA bulk copies (16 KB each), completion on
+// mbarriers.  Two whole tiles do not fit at 32 columns (2 x 128 KB), so the buffer is split: the slots that fit
+// twice are loaded a whole tile ahead, the rest is requested into L2 ahead (cp.async.bulk.prefetch.L2) and copied
+// when the last warp has finished the current tile.
 #pragma once
 #include "ebic_device.cuh"
 
@@ -47,6 +49,7 @@ struct PairtileParams {
     int32_t cols;
     int32_t n_ind;                   // individuals of this launch
     int32_t n_groups;                // ceil(n_ind / 32)
+    int32_t lo_slots;                // slots [0, lo_slots) of a tile alternate between two regions (see the kernel)
     const int2* meta;                // [n_ind] {b, L} written by the ingest kernel (L = -1: invalid)
     const int32_t* col_ids;
     int2* gmeta;                     // [n_groups * 32] {k, n}: individual and its number of pairs (-1: nothing to do)
@@ -135,34 +138,60 @@ pairtile_plan_kernel(const PairtileParams p)
     rec[96] = make_uint4(w[12], w[13], w[14], w[15]);
 }
 
-// AND the 1,024 rows of slot `off16` (16-byte units from the tile start) into acc; `lanebase` = shared address of
-// the tile + 16 * (lane & 7).
-__device__ __forceinline__ void pairtile_and2(uint4 (&acc)[8], uint32_t lanebase, uint32_t off_a, uint32_t off_b) {
-    const uint32_t a = lanebase + off_a * 16u, b = lanebase + off_b * 16u;
+// AND the 1,024 rows of the slots at `off_a` / `off_b` (16-byte units from the tile start) into acc.  `lo` / `hi`:
+// shared address of the region that holds slots below / from `split` on, + 16 * (lane & 7).
+struct PtBases {
+    uint32_t lo, hi, split;
+    __device__ __forceinline__ uint32_t at(uint32_t off) const { return (off < split ? lo : hi) + off * 16u; }
+};
+__device__ __forceinline__ void pairtile_and2(uint4 (&acc)[8], const PtBases& base, uint32_t off_a, uint32_t off_b) {
+    const uint32_t a = base.at(off_a), b = base.at(off_b);
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
         const uint4 v = lds128(a ^ (u << 4)), w = lds128(b ^ (u << 4));
         acc[u].x &= v.x & w.x; acc[u].y &= v.y & w.y; acc[u].z &= v.z & w.z; acc[u].w &= v.w & w.w;
     }
 }
-
-// Eight record entries (one uint4 of halfwords), of which the first `n_left` (warp-uniform, >= 1) are needed; an odd
-// count visits one padded entry more (AND is idempotent).
-__device__ __forceinline__ void pairtile_chunk(uint4 (&acc)[8], uint32_t lanebase, const uint4& ids, int32_t n_left) {
-    pairtile_and2(acc, lanebase, ids.x & 0xffffu, ids.x >> 16);
-    if (n_left > 2) pairtile_and2(acc, lanebase, ids.y & 0xffffu, ids.y >> 16);
-    if (n_left > 4) pairtile_and2(acc, lanebase, ids.z & 0xffffu, ids.z >> 16);
-    if (n_left > 6) pairtile_and2(acc, lanebase, ids.w & 0xffffu, ids.w >> 16);
+__device__ __forceinline__ void pairtile_and1(uint4 (&acc)[8], const PtBases& base, uint32_t off_a) {
+    const uint32_t a = base.at(off_a);
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+        const uint4 v = lds128(a ^ (u << 4));
+        acc[u].x &= v.x; acc[u].y &= v.y; acc[u].z &= v.z; acc[u].w &= v.w;
+    }
 }
 
+// Eight record entries (one uint4 of halfwords), of which the first `n_left` (warp-uniform, >= 1) are needed.
+__device__ __forceinline__ void pairtile_chunk(uint4 (&acc)[8], const PtBases& base, const uint4& ids, int32_t n_left) {
+    const uint32_t w[4] = {ids.x, ids.y, ids.z, ids.w};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if (n_left >= 2 * j + 2) {
+            pairtile_and2(acc, base, w[j] & 0xffffu, w[j] >> 16);
+        } else {
+            if (n_left == 2 * j + 1) pairtile_and1(acc, base, w[j] & 0xffffu);
+            return;
+        }
+    }
+}
+
+// Shared memory: [header: mbarriers + group cursors][main: n_pairs slots][extra: lo_slots slots][counters].
+// Tile i of the CTA (i = 0, 1, ...) keeps its slots [0, lo_slots) in main (i even) or extra (i odd) and its slots
+// [lo_slots, n_pairs) always in main.  The "lo" part of tile i + 1 is therefore loaded a whole tile ahead, into the
+// region tile i does not use; only the "hi" part has to wait until tile i is finished (lo_slots = n_pairs: two whole
+// buffers; lo_slots = 0: one buffer).
 __global__ void __launch_bounds__(kPtWarps * 32, 1)
 fitness_pairtile_kernel(const PairtileParams p)
 {
     extern __shared__ __align__(128) unsigned char pt_smem[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(pt_smem);
-    unsigned char* tile = pt_smem + kPtHeader;
+    uint64_t* full_lo = reinterpret_cast<uint64_t*>(pt_smem);                    // [2]
+    uint64_t* full_hi = full_lo + 2;
+    int32_t* cursor = reinterpret_cast<int32_t*>(pt_smem + 32);                   // [2] next group of the even / odd tile
+    unsigned char* main_buf = pt_smem + kPtHeader;
     const uint32_t tile_bytes = static_cast<uint32_t>(p.n_pairs) * 128u;
-    uint32_t* counters = reinterpret_cast<uint32_t*>(tile + tile_bytes);          // [n_groups * 32]
+    const uint32_t lo_bytes = static_cast<uint32_t>(p.lo_slots) * 128u, hi_bytes = tile_bytes - lo_bytes;
+    unsigned char* extra_buf = main_buf + tile_bytes;
+    uint32_t* counters = reinterpret_cast<uint32_t*>(extra_buf + lo_bytes);       // [n_groups * 32]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     // this CTA's contiguous range of (tile, group) items
@@ -172,77 +201,96 @@ fitness_pairtile_kernel(const PairtileParams p)
     griddep_launch_dependents();                 // a dependent extraction launch may be scheduled
     if (i0 >= i1) return;
     const int64_t t_first = i0 / p.n_groups, t_last = (i1 - 1) / p.n_groups;
+    const unsigned char* table = reinterpret_cast<const unsigned char*>(p.PBT);
 
-    auto stage = [&](int64_t t) {                // one thread: refill the tile buffer, completion on `full`
-        const unsigned char* src = reinterpret_cast<const unsigned char*>(p.PBT) + t * static_cast<int64_t>(tile_bytes);
-        mbar_arrive_expect_tx(full, tile_bytes);
-        for (uint32_t o = 0; o < tile_bytes; o += kPtCopyBytes)
-            bulk_copy_g2s(tile + o, src + o, min(kPtCopyBytes, tile_bytes - o), full);
+    auto copy = [&](unsigned char* dst, const unsigned char* src, uint32_t bytes, uint64_t* bar) {   // one thread
+        if (bytes == 0) return;
+        mbar_arrive_expect_tx(bar, bytes);
+        for (uint32_t o = 0; o < bytes; o += kPtCopyBytes) bulk_copy_g2s(dst + o, src + o, min(kPtCopyBytes, bytes - o), bar);
+    };
+    auto stage_lo = [&](int64_t t) {             // slots [0, lo_slots) of tile t into the region of its parity
+        const int q = static_cast<int>((t - t_first) & 1);
+        copy(q ? extra_buf : main_buf, table + t * static_cast<int64_t>(tile_bytes), lo_bytes, &full_lo[q]);
+    };
+    auto stage_hi = [&](int64_t t) {
+        copy(main_buf + lo_bytes, table + t * static_cast<int64_t>(tile_bytes) + lo_bytes, hi_bytes, full_hi);
     };
     if (tid == 0) {
-        mbar_init(full, 1);
+        mbar_init(&full_lo[0], 1);
+        mbar_init(&full_lo[1], 1);
+        mbar_init(full_hi, 1);
         fence_mbar_init();
-        stage(t_first);                          // the table depends on the matrix only: overlaps ingest + plan
+        stage_lo(t_first);                       // the table depends on the matrix only: overlaps ingest + plan
+        stage_hi(t_first);
+        if (t_first < t_last) stage_lo(t_first + 1);
+        cursor[0] = static_cast<int32_t>(i0 - t_first * p.n_groups) + kPtWarps;
     }
     for (int32_t j = tid; j < p.n_groups * 32; j += kPtWarps * 32) counters[j] = 0;
     __syncthreads();
     griddep_wait();                              // gmeta / tids (plan kernel), counts initialised (ingest kernel)
 
-    const uint32_t lanebase = smem_u32(tile) + ((lane & 7) << 4);
+    const uint32_t lane16 = (lane & 7) << 4;
+    const uint32_t main_s = smem_u32(main_buf) + lane16, extra_s = smem_u32(extra_buf) + lane16;
     unsigned long long executed = 0;
-    uint32_t phase = 0;
+    // Groups are handed out longest first through a shared cursor (the first kPtWarps of a tile statically: group
+    // g_lo + warp); a warp's next group is drawn, and its records requested, before the current one is evaluated --
+    // the first group of the NEXT tile before the barrier that ends this one, so that no warp starts a tile by
+    // waiting for its records.
+    int32_t g = static_cast<int32_t>(i0 - t_first * p.n_groups) + warp;
+    int2 gm = make_int2(0, -1);
+    uint4 ids0 = make_uint4(0u, 0u, 0u, 0u), ids1 = ids0;
+    auto request = [&](int32_t grp) {
+        gm = __ldg(p.gmeta + grp * 32 + lane);
+        const uint4* rec = p.tids + static_cast<int64_t>(grp) * 128 + lane;
+        ids0 = __ldg(rec); ids1 = __ldg(rec + 32);
+    };
+    if (g < (t_first == t_last ? static_cast<int32_t>(i1 - t_first * p.n_groups) : p.n_groups)) request(g);
     for (int64_t t = t_first; t <= t_last; ++t) {
-        const int32_t g_lo = t == t_first ? static_cast<int32_t>(i0 - t * p.n_groups) : 0;
+        const int64_t i = t - t_first;
+        const int q = static_cast<int>(i & 1);
         const int32_t g_hi = t == t_last ? static_cast<int32_t>(i1 - t * p.n_groups) : p.n_groups;
-        if (t < t_last && tid < 32) {            // next tile: HBM -> L2 while this one is evaluated
-            const unsigned char* nxt = reinterpret_cast<const unsigned char*>(p.PBT) + (t + 1) * static_cast<int64_t>(tile_bytes);
-            for (uint32_t o = lane * kPtCopyBytes; o < tile_bytes; o += 32 * kPtCopyBytes)
-                bulk_prefetch_l2(nxt + o, min(kPtCopyBytes, tile_bytes - o));
+        if (t < t_last && tid < 32) {
+            // the part of the next tile that has to wait for this one: HBM -> L2 meanwhile
+            const unsigned char* nxt = table + (t + 1) * static_cast<int64_t>(tile_bytes) + lo_bytes;
+            for (uint32_t o = lane * kPtCopyBytes; o < hi_bytes; o += 32 * kPtCopyBytes)
+                bulk_prefetch_l2(nxt + o, min(kPtCopyBytes, hi_bytes - o));
+            if (lane == 0) cursor[q ^ 1] = kPtWarps;       // the next tile starts at group 0; nobody reads this cursor now
         }
-        // first group of this warp: its records are requested before the tile is awaited (entries 0..15; the rare
-        // longer chromosome fetches entries 16..31 when it gets there)
-        int32_t g = g_lo + warp;
-        int2 gm = make_int2(0, -1);
-        uint4 ids0 = make_uint4(0u, 0u, 0u, 0u), ids1 = ids0;
-        if (g < g_hi) {
-            gm = __ldg(p.gmeta + g * 32 + lane);
-            const uint4* rec = p.tids + static_cast<int64_t>(g) * 128 + lane;
-            ids0 = __ldg(rec); ids1 = __ldg(rec + 32);
-        }
-        mbar_wait(full, phase);
-        phase ^= 1;
+        PtBases base;
+        base.lo = q ? extra_s : main_s;
+        base.hi = main_s;
+        base.split = static_cast<uint32_t>(p.lo_slots) * 8u;
+        if (lo_bytes) mbar_wait(&full_lo[q], static_cast<uint32_t>(i >> 1) & 1u);
+        if (hi_bytes) mbar_wait(full_hi, static_cast<uint32_t>(i) & 1u);
         while (g < g_hi) {
             const int32_t n = gm.y;
             const int32_t maxn = __reduce_max_sync(0xffffffffu, n);
             const int2 gm_cur = gm;
             const uint4 cur0 = ids0, cur1 = ids1;
-            const int32_t g_next = g + kPtWarps;
-            if (g_next < g_hi) {                 // next group's records: in flight during this group's evaluation
-                gm = __ldg(p.gmeta + g_next * 32 + lane);
-                const uint4* rec = p.tids + static_cast<int64_t>(g_next) * 128 + lane;
-                ids0 = __ldg(rec); ids1 = __ldg(rec + 32);
-            }
+            int32_t g_next = 0;
+            if (lane == 0) g_next = atomicAdd(&cursor[q], 1);
+            g_next = __shfl_sync(0xffffffffu, g_next, 0);
+            if (g_next < g_hi) request(g_next);  // in flight during this group's evaluation
             if (maxn >= 1) {
                 uint4 acc[8];
 #pragma unroll
                 for (int u = 0; u < 8; ++u) acc[u] = make_uint4(~0u, ~0u, ~0u, ~0u);
                 const int32_t m = min(maxn, kPtRecIds);
-                pairtile_chunk(acc, lanebase, cur0, m);
-                if (m > 8) pairtile_chunk(acc, lanebase, cur1, m - 8);
+                pairtile_chunk(acc, base, cur0, m);
+                if (m > 8) pairtile_chunk(acc, base, cur1, m - 8);
                 if (m > 16) {
                     const uint4* rec = p.tids + static_cast<int64_t>(g) * 128 + lane;
                     const uint4 cur2 = __ldg(rec + 64), cur3 = __ldg(rec + 96);
-                    pairtile_chunk(acc, lanebase, cur2, m - 16);
-                    if (m > 24) pairtile_chunk(acc, lanebase, cur3, m - 24);
+                    pairtile_chunk(acc, base, cur2, m - 16);
+                    if (m > 24) pairtile_chunk(acc, base, cur3, m - 24);
                 }
                 if (maxn > kPtRecIds && n > kPtRecIds) {
                     // pairs beyond the record come from the caller's ids (a VALID individual)
                     const int32_t* ids_g = p.col_ids + __ldg(&p.meta[gm_cur.x]).x;
                     int32_t a = __ldg(ids_g + kPtRecIds);
-                    for (int32_t i = kPtRecIds; i < n; ++i) {
-                        const int32_t c = __ldg(ids_g + i + 1);
-                        const uint32_t off = static_cast<uint32_t>(a * p.cols + c) * 8u;
-                        pairtile_and2(acc, lanebase, off, off);
+                    for (int32_t j = kPtRecIds; j < n; ++j) {
+                        const int32_t c = __ldg(ids_g + j + 1);
+                        pairtile_and1(acc, base, static_cast<uint32_t>(a * p.cols + c) * 8u);
                         a = c;
                     }
                 }
@@ -256,8 +304,15 @@ fitness_pairtile_kernel(const PairtileParams p)
             }
             g = g_next;
         }
+        if (t < t_last) {                        // first group of the next tile (it starts at group 0)
+            g = warp;
+            if (g < (t + 1 == t_last ? static_cast<int32_t>(i1 - t_last * p.n_groups) : p.n_groups)) request(g);
+        }
         __syncthreads();                         // every warp is done with the tile (and with its counters)
-        if (t < t_last && tid == 0) stage(t + 1);
+        if (tid == 0) {
+            if (t < t_last) stage_hi(t + 1);
+            if (t + 1 < t_last) stage_lo(t + 2); // into the region this tile has just released
+        }
     }
     // one 64-bit global atomic per (CTA, individual)
     for (int32_t j = tid; j < p.n_groups * 32; j += kPtWarps * 32) {

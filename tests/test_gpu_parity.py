@@ -227,6 +227,58 @@ def test_long_and_degenerate_chromosomes(B, oracle_mod):
         check_all(B, oracle_mod, m, mode, off, ids)
 
 
+@pytest.mark.parametrize("rows,cols,n_ind,max_len", [(1, 3, 5, 3), (3_000, 7, 33, 5), (70_001, 40, 1_000, 40),
+                                                     (5_003, 32, 300, 80), (200_000, 25, 9_000, 12),
+                                                     (160_000, 42, 7_000, 9)])
+def test_pairtile_kernel(B, oracle_mod, rows, cols, n_ind, max_len):
+    """PAIRTILE (bit-column tiles staged in shared memory, lane = individual): ragged row counts, more tiles than
+    SMs and fewer, a population larger than one launch's counters (9,000 at 25 columns: 8,192 + 808; 7,000 at 42
+    columns: the tile leaves room for 1,632 counters), chromosomes longer than the 32-entry record, empty / length-1 /
+    duplicate-column / invalid individuals, both missing modes, with and without the split tile buffer, and the
+    executed-visit counter (early exit does not apply: executed == nominal)."""
+    import torch
+    rng = np.random.default_rng(rows + cols)
+    m = rng.standard_normal((rows, cols), dtype=np.float32)
+    m[rng.random((rows, cols)) < 0.02] = np.nan
+    m[: rows // 3] = np.sort(m[: rows // 3], axis=1)           # rows that match increasing-id chromosomes
+    chroms = [rng.integers(0, cols, size=rng.integers(0, max_len + 1)).tolist() for _ in range(n_ind)]
+    if n_ind > 20:
+        chroms[7] = [0, cols]                                  # invalid id: count 0, sticky BAD_COLUMN, others unaffected
+        chroms[11] = sorted(rng.permutation(cols)[:min(cols, 6)].tolist())
+    off, ids = csr(chroms)
+    for mode in (ON, OFF):
+        st, want = oracle_mod.eval_fitness(m, mode, off, ids)
+        with B.Ebic(m, mode) as eb:
+            assert eb.info(17) == eb.info(14) > 0              # the tile-major copy exists: as many bytes as the table
+            got = gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_AUTO)
+            assert (got == want).all() and eb.last_kernel in (B.EBIC_KERNEL_PAIRTILE, B.EBIC_KERNEL_PAIRBITS)
+            if rows < 10_000:                                  # far too small for staged tiles to pay
+                assert eb.last_kernel == B.EBIC_KERNEL_PAIRBITS
+            eb.status()
+            for split in (1, 0):
+                eb.set_tuning(8, split)
+                got = gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_PAIRTILE)
+                assert (got == want).all(), (mode, split, np.flatnonzero(got != want)[:10])
+                assert eb.last_kernel == B.EBIC_KERNEL_PAIRTILE
+                assert eb.status() == st
+            eb.set_kernel(B.EBIC_KERNEL_PAIRTILE)
+            eb.set_instrumentation(1)
+            got = eb.eval_fitness(dev(off), dev(ids))
+            torch.cuda.synchronize()
+            lens = np.diff(off)
+            lens[7 if n_ind > 20 else 0:8 if n_ind > 20 else 0] = 0      # the invalid individual executes nothing
+            assert eb.info(10) == eb.ld * int(np.maximum(lens - 1, 0).sum())
+            eb.set_instrumentation(0)
+            assert (got.cpu().numpy().view(np.uint64) == want).all()
+            assert eb.status() == st
+            eb.set_tuning(6, 0)                                # rebuild the table without the tile-major copy
+            eb.set_pairbits(False)
+            eb.set_pairbits(True)
+            assert eb.info(17) == 0 and eb.kernel == B.EBIC_KERNEL_PAIRBITS
+            with pytest.raises(B.EbicError):
+                eb.set_kernel(B.EBIC_KERNEL_PAIRTILE)
+
+
 def test_wide_matrix_falls_back(B, oracle_mod):
     """cols > 127: no rank tiles; cols so large that no float tile of all columns double-buffers: the column-union
     kernel.  The pair table still serves (PAIRBITS); without it AUTO falls back to TILED_F32 / UNION_F32."""
@@ -674,9 +726,10 @@ def test_c5_full_size(B, oracle_mod):
         eb.set_early_exit(False)                                 # bench.py's headline configuration
         got = eb.eval_fitness(d_off, d_ids)
         torch.cuda.synchronize()
-        assert eb.last_kernel == B.EBIC_KERNEL_PAIRBITS          # what AUTO (and bench.py) runs on C5
+        assert eb.last_kernel == B.EBIC_KERNEL_PAIRTILE          # what AUTO (and bench.py) runs on C5
         assert (got.cpu().numpy().view(np.uint64) == want).all()
-        for kern in (B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32, B.EBIC_KERNEL_DIRECT):
+        for kern in (B.EBIC_KERNEL_PAIRTILE, B.EBIC_KERNEL_PAIRBITS, B.EBIC_KERNEL_RANK8, B.EBIC_KERNEL_TILED_F32,
+                     B.EBIC_KERNEL_DIRECT):
             eb.set_kernel(kern)
             for early_exit in ((True,) if kern == B.EBIC_KERNEL_DIRECT else (True, False)):
                 eb.set_early_exit(early_exit)
