@@ -51,7 +51,7 @@ N_CHOSEN = 8
 WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4, "p1": 5, "p2": 6, "p3": 7}
 KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "union_f32": 5, "prefix": 6, "pairtile": 7}
 TRAFFIC_CSV = ROOT / "profiles" / "r02_dram_traffic.csv"
-KERNEL_SOURCES = ["pairbits_kernels.cuh", "fitness_kernels.cuh", "union_kernels.cuh", "ebic_device.cuh"]
+KERNEL_SOURCES = ["pairbits_kernels.cuh", "pairtile_kernels.cuh", "fitness_kernels.cuh", "union_kernels.cuh", "ebic_device.cuh"]
 
 
 def log(*a):
@@ -340,10 +340,11 @@ def measure_workload(B, key, w, peaks, peaks_kind, probes, flush, reps, early_ex
              "step_ms": step_ms, "kernel_ms": kernel_ms, "comparisons_per_s": w.comparisons / (step_ms * 1e-3),
              "bound": roof["bound"], "frac": roof["frac"], "achieved_gbs": roof["achieved"], "peak_gbs": roof["peak"],
              "create_ms": create_ms, "create_breakdown_ms": breakdown, "device_bytes": eb.info(9),
-             "pair_table_bytes": eb.info(14)}
-    # the pair table's builder against its own HBM floor: read the float32 matrix once, write the table once
+             "pair_table_bytes": eb.info(14), "pair_table_tile_major_bytes": eb.info(17)}
+    # the pair table's builder against its own HBM floor: read the float32 matrix once, write the table once (and
+    # its tile-major copy, where PAIRTILE applies)
     if eb.info(14):
-        floor_ms = (eb.ld * w.cols * 4 + eb.info(14)) / (float(peaks["hbm_gbs"]) * 1e9) * 1e3
+        floor_ms = (eb.ld * w.cols * 4 + eb.info(14) + eb.info(17)) / (float(peaks["hbm_gbs"]) * 1e9) * 1e3
         entry["pair_table_build"] = {"ms": breakdown["pair_table"], "hbm_floor_ms": floor_ms,
                                      "frac_of_hbm_floor": floor_ms / max(breakdown["pair_table"], 1e-9)}
     # break-even: evaluations after which building the table has paid for itself against the best kernel that
@@ -587,7 +588,7 @@ def run_gpu(args):
             "probes": probes.as_dict(),
             "ms_per_step_without_kernel_events": plain_ms,
             "create_ms": create_ms, "create_breakdown_ms": breakdown,
-            "pair_table_bytes": eb.info(14), "device_bytes": eb.info(9),
+            "pair_table_bytes": eb.info(14), "pair_table_tile_major_bytes": eb.info(17), "device_bytes": eb.info(9),
             "generate_s": gen_s, "wall_s_timed_region": wall_s,
             "step_ms_min_max": [min(step_ms), max(step_ms)],
         }

@@ -72,6 +72,7 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
  *   7  AUTO picks PAIRTILE from this many (1,024-row tile, consecutive-pair use) units on (default 0 = the rule
  *      stated at EBIC_KERNEL_AUTO)
  *   8  PAIRTILE loads the part of the next tile that fits shared memory a second time one tile ahead (default 1)
+ *   9  PAIRBITS row chunks requested into L2 by the kernel's prologue (default 1; 1..16, at least the distance)
  * EBIC_ERR_ARG for an unknown knob or a value outside its range.
  */
 int ebic_set_tuning(ebic_ctx *ctx, int32_t knob, int32_t value);

@@ -387,6 +387,7 @@ PairbitsParams pairbits_params(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
     p.n_pairs = ctx->cols * ctx->cols;
     p.prefetch_dist = pairbits_dense(ctx, n_ind, n_ids) ? ctx->pb_prefetch_dist : 0;
+    p.prologue_chunks = std::max(p.prefetch_dist, p.prefetch_dist > 0 ? ctx->pb_prologue_chunks : 0);
     return p;
 }
 

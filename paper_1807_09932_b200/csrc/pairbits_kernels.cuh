@@ -37,7 +37,8 @@ struct PairbitsParams {
     unsigned long long* visits;      // executed (row, pair) visits (instrumented) or nullptr
     int32_t n_pairs;                 // cols * cols bit columns in PB
     int32_t prefetch_dist;           // tasks of chunk g prefetch a slice of the bit columns of chunk g + dist into L2 (0 = off);
-                                     // chunks 0 .. dist-1 are requested by the kernel's prologue, before it waits for the ingest
+    int32_t prologue_chunks;         // chunks 0 .. prologue_chunks-1 (>= dist) are requested by the kernel's prologue,
+                                     // before it waits for the ingest
 };
 
 __device__ __forceinline__ void and4(uint4& a, const uint4& v) {
@@ -152,7 +153,7 @@ __device__ __forceinline__ void pairbits_task(const PairbitsParams& p, int64_t t
         // the demand loads that arrive `dist` chunks later then hit L2.  (Chunks 0 .. dist-1: the kernel's prologue.)
         const int32_t per = (p.n_pairs + p.n_ind - 1) / p.n_ind;     // columns per task
         const int64_t pw = (g + p.prefetch_dist) * p.chunk_words;
-        if (pw < p.ldw) {
+        if (pw < p.ldw && g + p.prefetch_dist >= p.prologue_chunks) {
             const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.chunk_words), p.ldw - pw)) * 4u;
             for (int32_t q = lane; q < per; q += 32) {
                 const int64_t pair = static_cast<int64_t>(j) * per + q;
@@ -209,10 +210,10 @@ fitness_pairbits_kernel(const PairbitsParams p)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     griddep_launch_dependents();                                 // a dependent extraction launch may be scheduled
     if (p.prefetch_dist > 0) {
-        // chunks 0 .. dist-1 of every bit column, each requested exactly once, spread over the first CTAs
+        // chunks 0 .. prologue_chunks-1 of every bit column, each requested exactly once, spread over the first CTAs
         const int64_t n_pro = min(static_cast<int64_t>(gridDim.x), static_cast<int64_t>(p.n_pairs + 63) / 64);
         if (blockIdx.x < n_pro) {
-            const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.prefetch_dist) * p.chunk_words, p.ldw)) * 4u;
+            const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.prologue_chunks) * p.chunk_words, p.ldw)) * 4u;
             for (int64_t pair = static_cast<int64_t>(blockIdx.x) * 64 + threadIdx.x; pair < p.n_pairs; pair += n_pro * 64)
                 bulk_prefetch_l2(p.PB + pair * p.ldw, bytes);
         }
