@@ -581,7 +581,7 @@ def run_gpu(args):
             "clocks": clk.summary(),
             "e2e": {"value": comparisons / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
-                    "how": "one ebic_eval_extract call with pinned host buffers: population in, counts + masks out"},
+                    "how": "one ebic_eval_extract call with pinned host buffers: population in, counts + masks out (the masks are extracted first and copied back on a second stream while the fitness kernel runs)"},
             "gpu_launches": int(launches_per_step * args.steps),
             "gpu_launches_per_step": int(launches_per_step),
             "roofline": roof,

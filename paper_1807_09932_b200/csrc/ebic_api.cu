@@ -768,6 +768,9 @@ int ebic_destroy(ebic_ctx* ctx) {
     cudaFree(ctx->idrec);
     cudaFree(ctx->ubatch);
     for (void* s : ctx->stage) cudaFree(s);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->ev_masks_ready) cudaEventDestroy(ctx->ev_masks_ready);
+    if (ctx->ev_masks_copied) cudaEventDestroy(ctx->ev_masks_copied);
     for (int i = 0; i < ebic_ctx::kTimingRing; ++i) {
         if (ctx->ev_begin[i]) cudaEventDestroy(ctx->ev_begin[i]);
         if (ctx->ev_end[i]) cudaEventDestroy(ctx->ev_end[i]);
@@ -820,16 +823,34 @@ static int eval_extract_impl(ebic_ctx* ctx, const int32_t* offsets, const int32_
     }
     const bool fused = do_eval && do_extract;
     if (fused && d_mcnt) EBIC_TRY(cudaMemsetAsync(d_mcnt, 0, static_cast<size_t>(n_chosen) * 8, stream));   // ahead of the kernel chain
+    // One generation with HOST outputs: the masks are the large result (rows / 8 bytes per chosen individual) and the
+    // extraction does not depend on the fitness kernel, so it runs FIRST and its device-to-host copy proceeds on the
+    // context's copy stream while the fitness kernel works.
+    const bool masks_first = fused && !out_dev;
+    if (masks_first) {
+        if (!ctx->copy_stream) {
+            EBIC_TRY(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+            EBIC_TRY(cudaEventCreateWithFlags(&ctx->ev_masks_ready, cudaEventDisableTiming));
+            EBIC_TRY(cudaEventCreateWithFlags(&ctx->ev_masks_copied, cudaEventDisableTiming));
+        }
+        if ((st = extract_device(ctx, d_off, d_ids, n_ind, n_ids, d_chosen, n_chosen, d_masks, d_mcnt, stream, false))) return st;
+        EBIC_TRY(cudaEventRecord(ctx->ev_masks_ready, stream));
+        EBIC_TRY(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_masks_ready, 0));
+        EBIC_TRY(cudaMemcpyAsync(masks, d_masks, static_cast<size_t>(n_chosen) * words * 8, cudaMemcpyDeviceToHost, ctx->copy_stream));
+        if (mask_counts) EBIC_TRY(cudaMemcpyAsync(mask_counts, d_mcnt, static_cast<size_t>(n_chosen) * 8, cudaMemcpyDeviceToHost, ctx->copy_stream));
+        EBIC_TRY(cudaEventRecord(ctx->ev_masks_copied, ctx->copy_stream));
+    }
     if (do_eval && (st = eval_device(ctx, d_off, d_ids, n_ind, n_ids, d_counts, stream))) return st;
-    if (do_extract &&
+    if (do_extract && !masks_first &&
         (st = extract_device(ctx, d_off, d_ids, n_ind, n_ids, d_chosen, n_chosen, d_masks, d_mcnt, stream, fused)))
         return st;
     if (!out_dev) {
         if (do_eval) EBIC_TRY(cudaMemcpyAsync(counts, d_counts, static_cast<size_t>(n_ind) * 8, cudaMemcpyDeviceToHost, stream));
-        if (do_extract) {
+        if (do_extract && !masks_first) {
             EBIC_TRY(cudaMemcpyAsync(masks, d_masks, static_cast<size_t>(n_chosen) * words * 8, cudaMemcpyDeviceToHost, stream));
             if (mask_counts) EBIC_TRY(cudaMemcpyAsync(mask_counts, d_mcnt, static_cast<size_t>(n_chosen) * 8, cudaMemcpyDeviceToHost, stream));
         }
+        if (masks_first) EBIC_TRY(cudaStreamWaitEvent(stream, ctx->ev_masks_copied, 0));
         EBIC_TRY(cudaStreamSynchronize(stream));
     } else if (!pop_dev) {
         EBIC_TRY(cudaStreamSynchronize(stream));   // host population buffers may be reused on return

@@ -39,6 +39,9 @@ struct ebic_ctx {
     int64_t ubatch_cap = 0;
     void* stage[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // staging for host-pointer calls
     int64_t stage_cap[6] = {0, 0, 0, 0, 0, 0};
+    cudaStream_t copy_stream = nullptr;        // ebic_eval_extract with host outputs: the masks go back on this stream
+    cudaEvent_t ev_masks_ready = nullptr;      // while the fitness kernel runs
+    cudaEvent_t ev_masks_copied = nullptr;
 
     // ---- knobs (include/ebic_debug.h); the defaults are the product configuration
     int32_t kernel_request = 0;                // EBIC_KERNEL_AUTO
