@@ -122,9 +122,10 @@ int ebic_extract_rows(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_
 
 /*
  * One GA generation in one call: ebic_eval_fitness followed by ebic_extract_rows on the same population, with
- * the population uploaded once (host pointers) and one stream synchronisation; on the device the extraction
+ * the population uploaded once (host pointers) and one stream synchronisation; with device outputs the extraction
  * kernel is chained behind the fitness kernel with programmatic dependent launch and runs alongside its last
- * wave.  Arguments as in the two calls (`mask_counts` may be NULL).  n_ind == 0 or n_chosen == 0 skips that
+ * wave; with host outputs the masks -- which do not depend on the counts -- are extracted first and copied back on
+ * a stream the context owns while the fitness kernel runs (everything has completed when the call returns).  Arguments as in the two calls (`mask_counts` may be NULL).  n_ind == 0 or n_chosen == 0 skips that
  * half.  `counts`, `masks` and `mask_counts` must not overlap each other (the two kernels may run concurrently).
  */
 int ebic_eval_extract(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_ids, int32_t n_ind,
