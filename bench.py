@@ -409,6 +409,9 @@ def run_gpu(args):
     if args.one_device:                                        # functional check of the N > 1 path on a single GPU
         local_rank = 0
     torch.cuda.set_device(local_rank)
+    # Everything below runs on one non-default stream: the library replays a repeated all-device call from a captured
+    # CUDA graph (include/ebic.h, ebic_eval_extract), which the legacy default stream does not allow.
+    torch.cuda.set_stream(torch.cuda.Stream())
     if world > 1:
         if args.dist_backend == "nccl":
             dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
@@ -699,6 +702,7 @@ def run_table(args):
     from paper_1807_09932_b200 import binding as B
     peaks, peaks_kind = measured_peaks()
     torch.cuda.set_device(0)
+    torch.cuda.set_stream(torch.cuda.Stream())                  # see run_bench: graph replay needs a non-default stream
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     probes = Probes(B)
     log("probes:", json.dumps(probes.as_dict()))

@@ -125,7 +125,12 @@ int ebic_extract_rows(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_
  * the population uploaded once (host pointers) and one stream synchronisation; with device outputs the extraction
  * kernel is chained behind the fitness kernel with programmatic dependent launch and runs alongside its last
  * wave; with host outputs the masks -- which do not depend on the counts -- are extracted first and copied back on
- * a stream the context owns while the fitness kernel runs (everything has completed when the call returns).  Arguments as in the two calls (`mask_counts` may be NULL).  n_ind == 0 or n_chosen == 0 skips that
+ * a stream the context owns while the fitness kernel runs (everything has completed when the call returns).
+ * Repetition: a GA loop passes the same device buffers every generation.  When a call with device pointers on a
+ * non-default stream repeats the previous call's arguments exactly (pointers, sizes, stream), the library captures
+ * its launch sequence into a CUDA graph and replays that graph from then on -- the results are those of the plain
+ * launches; only the launch overhead changes (ebic_eval_fitness and ebic_extract_rows do the same).  Buffers passed
+ * to such a call must therefore stay valid until the work has run, as with any stream-ordered call.  Arguments as in the two calls (`mask_counts` may be NULL).  n_ind == 0 or n_chosen == 0 skips that
  * half.  `counts`, `masks` and `mask_counts` must not overlap each other (the two kernels may run concurrently).
  */
 int ebic_eval_extract(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_ids, int32_t n_ind,

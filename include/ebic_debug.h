@@ -73,6 +73,7 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
  *      stated at EBIC_KERNEL_AUTO)
  *   8  PAIRTILE loads the part of the next tile that fits shared memory a second time one tile ahead (default 1)
  *   9  PAIRBITS row chunks requested into L2 by the kernel's prologue (default 1; 1..16, at least the distance)
+ *  10  replay a repeated all-device call from a captured CUDA graph (default 1; include/ebic.h, ebic_eval_extract)
  * EBIC_ERR_ARG for an unknown knob or a value outside its range.
  */
 int ebic_set_tuning(ebic_ctx *ctx, int32_t knob, int32_t value);
@@ -101,6 +102,7 @@ int ebic_set_instrumentation(ebic_ctx *ctx, int32_t on);
  *   last read, 11 mean fitness-kernel time in ns, 12 evals timed (see ebic_set_instrumentation), 13 early exit
  *   on/off, 14 bytes of the pair table (0 = absent), 15 kernel of the last fitness launch (0 = none yet),
  *   16 bytes of the rank tiles (0 = absent), 17 bytes of the tile-major copy of the pair table (0 = absent),
+ *   18 kernels in the captured CUDA graph the next identical call would replay (0 = no graph held),
  *   20..24 ebic_create's time in ns, CUDA events on the legacy stream: 20 host-to-device copy + transpose +
  *   padding, 21 NaN bitmask, 22 pair-table kernel, 23 rank-tile kernel (22 / 23 also when built later on demand;
  *   allocations excluded), 24 all of ebic_create including the allocations.

@@ -768,6 +768,7 @@ int ebic_destroy(ebic_ctx* ctx) {
     cudaFree(ctx->idrec);
     cudaFree(ctx->ubatch);
     for (void* s : ctx->stage) cudaFree(s);
+    if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->ev_masks_ready) cudaEventDestroy(ctx->ev_masks_ready);
     if (ctx->ev_masks_copied) cudaEventDestroy(ctx->ev_masks_copied);
@@ -822,6 +823,63 @@ static int eval_extract_impl(ebic_ctx* ctx, const int32_t* offsets, const int32_
         }
     }
     const bool fused = do_eval && do_extract;
+    // A GA loop calls this with the SAME device buffers every generation (only their contents change), so the launch
+    // sequence is captured into a CUDA graph the second time a call repeats the previous one's arguments and replayed
+    // from the third on: one graph launch instead of three or four kernel launches and a memset (the launch overhead
+    // is a third of the step on the paper's dataset shapes).  Any change of a knob, a pointer or a size
+    // starts over; instrumented calls, host pointers, the legacy default stream and a stream that is already being
+    // captured by the caller always take the plain path.
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    const bool graphable = ctx->use_graphs && pop_dev && out_dev && stream != nullptr && stream != cudaStreamLegacy &&
+                           stream != cudaStreamPerThread && !ctx->time_kernels && !ctx->count_visits &&
+                           cudaStreamIsCapturing(stream, &cap) == cudaSuccess && cap == cudaStreamCaptureStatusNone;
+    bool capture = false;
+    if (graphable) {
+        ebic_ctx::GraphKey key = {};                          // zeroed, padding included: compared with memcmp
+        key.offsets = offsets; key.col_ids = col_ids; key.counts = counts; key.chosen = chosen; key.masks = masks;
+        key.mask_counts = mask_counts; key.stream = stream; key.n_ids = n_ids; key.n_ind = n_ind; key.n_chosen = n_chosen;
+        key.epoch = ctx->epoch; key.flags = (do_eval ? 1 : 0) | (do_extract ? 2 : 0);
+        if (ctx->graph_state != 0 && std::memcmp(&key, &ctx->graph_key, sizeof(key)) == 0) {
+            if (ctx->graph_exec) {
+                ctx->launches += ctx->graph_launches;
+                return ebic_host::cuda_status(cudaGraphLaunch(ctx->graph_exec, stream));
+            }
+            capture = ctx->graph_state == 1;                  // second sighting; 2 = capture failed once: stay plain
+        } else {
+            if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
+            ctx->graph_exec = nullptr;
+            ctx->graph_key = key;
+            ctx->graph_state = 1;
+        }
+    } else {
+        cudaGetLastError();
+    }
+    const int64_t launches0 = ctx->launches;
+    if (capture && cudaStreamBeginCapture(stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+        cudaGetLastError();
+        capture = false;
+        ctx->graph_state = 2;
+    }
+    if (capture) {
+        // the buffers were grown by the identical plain call before this one: nothing allocates during the capture
+        st = EBIC_OK;
+        if (fused && d_mcnt) st = ebic_host::cuda_status(cudaMemsetAsync(d_mcnt, 0, static_cast<size_t>(n_chosen) * 8, stream));
+        if (!st && do_eval) st = eval_device(ctx, d_off, d_ids, n_ind, n_ids, d_counts, stream);
+        if (!st && do_extract) st = extract_device(ctx, d_off, d_ids, n_ind, n_ids, d_chosen, n_chosen, d_masks, d_mcnt, stream, fused);
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(stream, &graph);
+        if (!st && e == cudaSuccess && graph && cudaGraphInstantiate(&ctx->graph_exec, graph, 0) != cudaSuccess) ctx->graph_exec = nullptr;
+        if (graph) cudaGraphDestroy(graph);
+        if (!st && e == cudaSuccess && ctx->graph_exec) {
+            ctx->graph_launches = ctx->launches - launches0;
+            return ebic_host::cuda_status(cudaGraphLaunch(ctx->graph_exec, stream));
+        }
+        cudaGetLastError();                                   // the capture did not work out: plain launches, now and later
+        if (ctx->graph_exec) cudaGraphExecDestroy(ctx->graph_exec);
+        ctx->graph_exec = nullptr;
+        ctx->graph_state = 2;
+        ctx->launches = launches0;
+    }
     if (fused && d_mcnt) EBIC_TRY(cudaMemsetAsync(d_mcnt, 0, static_cast<size_t>(n_chosen) * 8, stream));   // ahead of the kernel chain
     // One generation with HOST outputs: the masks are the large result (rows / 8 bytes per chosen individual) and the
     // extraction does not depend on the fitness kernel, so it runs FIRST and its device-to-host copy proceeds on the

@@ -39,6 +39,19 @@ struct ebic_ctx {
     int64_t ubatch_cap = 0;
     void* stage[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};   // staging for host-pointer calls
     int64_t stage_cap[6] = {0, 0, 0, 0, 0, 0};
+    // ---- the launch sequence of a repeated all-device call, captured once and replayed (ebic_api.cu eval_extract_impl)
+    struct GraphKey {
+        const void *offsets, *col_ids, *counts, *chosen, *masks, *mask_counts, *stream;
+        int64_t n_ids;
+        int32_t n_ind, n_chosen, epoch, flags;
+    };
+    GraphKey graph_key = {};
+    int32_t graph_state = 0;                   // 0 nothing seen, 1 key seen once (plain call done), 2 capture failed for this key
+    cudaGraphExec_t graph_exec = nullptr;
+    int64_t graph_launches = 0;                // kernels in the captured sequence (the launch counter follows replays)
+    int32_t epoch = 0;                         // bumped by every knob: a captured sequence never outlives its configuration
+    int32_t use_graphs = 1;
+
     cudaStream_t copy_stream = nullptr;        // ebic_eval_extract with host outputs: the masks go back on this stream
     cudaEvent_t ev_masks_ready = nullptr;      // while the fitness kernel runs
     cudaEvent_t ev_masks_copied = nullptr;

@@ -20,6 +20,7 @@ using ebic_host::cuda_status;
 extern "C" {
 
 int ebic_set_kernel(ebic_ctx* ctx, int32_t kernel) {
+    if (ctx) ctx->epoch++;
     if (!ctx || kernel < EBIC_KERNEL_AUTO || kernel > EBIC_KERNEL_PAIRTILE) return EBIC_ERR_ARG;
     if (!ebic_host::kernel_applies(ctx, kernel)) return EBIC_ERR_ARG;
     if (kernel == EBIC_KERNEL_RANK8) {
@@ -33,6 +34,7 @@ int ebic_set_kernel(ebic_ctx* ctx, int32_t kernel) {
 
 int ebic_set_pairbits(ebic_ctx* ctx, int32_t on) {
     if (!ctx) return EBIC_ERR_ARG;
+    ctx->epoch++;
     if (cudaDeviceSynchronize() != cudaSuccess) return cuda_status(cudaGetLastError());
     if (on == 0) {
         ebic_host::free_pairbits(ctx);
@@ -50,17 +52,20 @@ int ebic_set_pairbits(ebic_ctx* ctx, int32_t on) {
 int ebic_set_extract_source(ebic_ctx* ctx, int32_t use_pairbits) {
     if (!ctx) return EBIC_ERR_ARG;
     ctx->extract_pairbits = use_pairbits ? 1 : 0;
+    ctx->epoch++;
     return EBIC_OK;
 }
 
 int ebic_set_early_exit(ebic_ctx* ctx, int32_t on) {
     if (!ctx) return EBIC_ERR_ARG;
     ctx->early_exit = on ? 1 : 0;
+    ctx->epoch++;
     return EBIC_OK;
 }
 
 int ebic_set_tuning(ebic_ctx* ctx, int32_t knob, int32_t value) {
     if (!ctx) return EBIC_ERR_ARG;
+    ctx->epoch++;
     switch (knob) {
         case 0:
             if (value < 1 || value > 64) return EBIC_ERR_ARG;
@@ -87,12 +92,14 @@ int ebic_set_tuning(ebic_ctx* ctx, int32_t knob, int32_t value) {
             if (value < 1 || value > 16) return EBIC_ERR_ARG;
             ctx->pb_prologue_chunks = value;
             return EBIC_OK;
+        case 10: ctx->use_graphs = value ? 1 : 0; return EBIC_OK;
         default: return EBIC_ERR_ARG;
     }
 }
 
 int ebic_set_instrumentation(ebic_ctx* ctx, int32_t on) {
     if (!ctx) return EBIC_ERR_ARG;
+    ctx->epoch++;
     ctx->count_visits = (on & 1) ? 1 : 0;
     ctx->time_kernels = (on & 2) ? 1 : 0;
     ctx->timed_evals = 0;
@@ -145,6 +152,7 @@ int64_t ebic_get_info(ebic_ctx* ctx, int32_t what) {
         case 15: return ctx->last_kernel;
         case 16: return ctx->Rk ? ctx->ld * ctx->cols : 0;
         case 17: return ctx->pbt_bytes;
+        case 18: return ctx->graph_exec ? ctx->graph_launches : 0;
         case 20: case 21: case 22: case 23: case 24:
             return static_cast<int64_t>(static_cast<double>(ctx->create_ms[what - 20]) * 1e6);
         default: return -1;

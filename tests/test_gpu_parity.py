@@ -640,6 +640,79 @@ def test_eval_extract_one_call(B, oracle_mod):
         assert eb.status() == 0
 
 
+def test_repeated_calls_replay_a_graph(B, oracle_mod):
+    """A GA loop passes the same device buffers every generation: from the second identical call on a non-default
+    stream the library captures its launch sequence into a CUDA graph and replays it (include/ebic.h,
+    ebic_eval_extract).  Five generations with the population REWRITTEN IN PLACE between them, every kernel, all three
+    hot calls: each generation's counts and masks equal the oracle's; a knob change, different buffers, a host-pointer
+    call and the default stream all fall back to plain launches."""
+    import torch
+    rows, cols, n_ind = 70_001, 32, 600
+    m, off0, ids0 = W.random_case(321, rows, cols, n_ind, (0, 12), 0.02, False, True)
+    side = torch.cuda.Stream()
+    chosen = np.array([1, 5, 17, n_ind - 1], dtype=np.int32)
+    rng = np.random.default_rng(4)
+    with B.Ebic(m, ON) as eb:
+        d_off, d_ids, d_ch = dev(off0), dev(ids0), dev(chosen)
+        counts = torch.empty(n_ind, dtype=torch.int64, device="cuda")
+        masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
+        mcnt = torch.empty(len(chosen), dtype=torch.int64, device="cuda")
+        for kern in kernels_for(eb, B):
+            eb.set_kernel(kern)
+            replayed = 0
+            for gen in range(5):
+                ids = ids0.copy()
+                flip = rng.random(ids.size) < 0.3                      # same CSR shape, new columns
+                ids[flip] = rng.integers(0, cols, size=int(flip.sum()), dtype=np.int32)
+                d_ids.copy_(torch.from_numpy(ids))
+                torch.cuda.synchronize()
+                st, want = oracle_mod.eval_fitness(m, ON, off0, ids)
+                _, wm, wc = oracle_mod.extract_rows(m, ON, off0, ids, chosen)
+                with torch.cuda.stream(side):
+                    eb.eval_extract(d_off, d_ids, d_ch, counts=counts, masks=masks, mask_counts=mcnt, stream=side)
+                side.synchronize()
+                replayed += eb.info(18) > 0
+                assert (counts.cpu().numpy().view(np.uint64) == want).all(), (B.KERNEL_NAMES[kern], gen)
+                assert (masks.cpu().numpy().view(np.uint64) == wm).all() and (mcnt.cpu().numpy().view(np.uint64) == wc).all()
+            assert replayed == 4, (B.KERNEL_NAMES[kern], replayed)     # captured at the second call, held ever since
+            n0 = eb.info(8)
+            with torch.cuda.stream(side):
+                eb.eval_extract(d_off, d_ids, d_ch, counts=counts, masks=masks, mask_counts=mcnt, stream=side)
+            side.synchronize()
+            assert eb.info(8) - n0 == eb.info(18) >= 2                 # the launch counter follows replays
+            # the two single calls are replayed as well
+            for _ in range(3):
+                with torch.cuda.stream(side):
+                    eb.eval_fitness(d_off, d_ids, counts=counts, stream=side)
+                side.synchronize()
+                assert (counts.cpu().numpy().view(np.uint64) == want).all()
+            assert eb.info(18) > 0
+            for _ in range(3):
+                with torch.cuda.stream(side):
+                    eb.extract_rows(d_off, d_ids, d_ch, masks=masks, counts=mcnt, stream=side)
+                side.synchronize()
+                assert (masks.cpu().numpy().view(np.uint64) == wm).all()
+            assert eb.info(18) > 0
+            # plain paths: other buffers, the default stream, host pointers, a knob
+            other = torch.empty_like(counts)
+            with torch.cuda.stream(side):
+                eb.eval_fitness(d_off, d_ids, counts=other, stream=side)
+            side.synchronize()
+            assert eb.info(18) == 0 and (other.cpu().numpy().view(np.uint64) == want).all()
+            c = eb.eval_fitness(d_off, d_ids)
+            torch.cuda.synchronize()
+            assert eb.info(18) == 0 and (c.cpu().numpy().view(np.uint64) == want).all()
+            assert (eb.eval_fitness(off0, ids) == want).all()
+            eb.set_tuning(10, 0)                                       # graphs off
+            for _ in range(3):
+                with torch.cuda.stream(side):
+                    eb.eval_fitness(d_off, d_ids, counts=counts, stream=side)
+                side.synchronize()
+            assert eb.info(18) == 0 and (counts.cpu().numpy().view(np.uint64) == want).all()
+            eb.set_tuning(10, 1)
+        assert eb.status() == 0
+
+
 def test_binding_refuses_wrong_dtypes(B):
     """The C ABI takes raw addresses: the binding must refuse what would be read as garbage (advisor finding)."""
     w = W.make_workload(0)
