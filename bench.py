@@ -170,10 +170,13 @@ class Probes:
         self.hbm_read_gbs = B.ebic_probe_read_bandwidth(4 << 30, 2)  # far larger than the 126 MB L2
         self.smem_gbs = B.ebic_probe_smem_bandwidth()                # conflict-free LDS.128, all SMs
         self.fsetp_gcmp = B.ebic_probe_fsetp_rate()                  # 1e9 ordered float compares / s, all SMs
+        self.gather_gbs = B.ebic_probe_smem_gather(True)             # PAIRTILE's pattern: per-lane slots, rotated units
+        self.gather_unrotated_gbs = B.ebic_probe_smem_gather(False)  # the same without the rotation (8-way conflicts)
 
     def as_dict(self):
         return {"l2_read_gbs": self.l2_gbs, "hbm_read_gbs": self.hbm_read_gbs, "smem_lds128_gbs": self.smem_gbs,
-                "fsetp_gcompares_per_s": self.fsetp_gcmp}
+                "fsetp_gcompares_per_s": self.fsetp_gcmp, "smem_gather_rotated_gbs": self.gather_gbs,
+                "smem_gather_unrotated_gbs": self.gather_unrotated_gbs}
 
 
 def pair_stats(w):

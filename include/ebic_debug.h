@@ -130,10 +130,15 @@ int ebic_debug_read(const ebic_ctx *ctx, int32_t what, void *dst, int64_t dst_by
  *   A buffer that fits the L2 gives the L2 -> SM bandwidth, one far larger than the L2 gives HBM read bandwidth.
  * ebic_probe_smem_bandwidth: GB/s of conflict-free LDS.128 from shared memory, all SMs (the 128 B/clk/SM data
  *   pipe the tiled kernels are bound by).
+ * ebic_probe_smem_gather: GB/s of the PAIRTILE access pattern on its own -- every lane its own pseudo-random
+ *   128-byte slot of a 128 KB shared-memory tile, read as eight LDS.128 with the 16-byte unit rotated per lane
+ *   (rotate != 0) or not (rotate == 0: the 8-way bank conflicts the rotation removes), AND + popcount as in the
+ *   kernel, 16 warps per SM, no staging.
  * ebic_probe_fsetp_rate: ordered float32 compares (FSETP.GE) per second, all SMs, in units of 1e9 lane-compares/s.
  */
 int ebic_probe_read_bandwidth(int64_t buffer_bytes, int32_t reps, double *gb_per_s);
 int ebic_probe_smem_bandwidth(double *gb_per_s);
+int ebic_probe_smem_gather(int32_t rotate, double *gb_per_s);
 int ebic_probe_fsetp_rate(double *gcompares_per_s);
 
 #ifdef __cplusplus

@@ -70,6 +70,7 @@ DEBUG_SYMBOLS = {
     "ebic_debug_read": (ctypes.c_int, [_vp, _i32, _vp, _i64]),
     "ebic_probe_read_bandwidth": (ctypes.c_int, [_i64, _i32, _f64p]),
     "ebic_probe_smem_bandwidth": (ctypes.c_int, [_f64p]),
+    "ebic_probe_smem_gather": (ctypes.c_int, [_i32, _f64p]),
     "ebic_probe_fsetp_rate": (ctypes.c_int, [_f64p]),
 }
 
@@ -225,6 +226,14 @@ def ebic_probe_smem_bandwidth() -> float:
     st = load_library().ebic_probe_smem_bandwidth(ctypes.byref(out))
     if st != EBIC_OK:
         raise EbicError(st, "ebic_probe_smem_bandwidth")
+    return out.value
+
+
+def ebic_probe_smem_gather(rotate: bool = True) -> float:
+    out = ctypes.c_double(0.0)
+    st = load_library().ebic_probe_smem_gather(1 if rotate else 0, ctypes.byref(out))
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_probe_smem_gather")
     return out.value
 
 

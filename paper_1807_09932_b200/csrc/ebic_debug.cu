@@ -268,6 +268,32 @@ int ebic_probe_smem_bandwidth(double* gb_per_s) {
     return st;
 }
 
+int ebic_probe_smem_gather(int32_t rotate, double* gb_per_s) {
+    if (!gb_per_s) return EBIC_ERR_ARG;
+    *gb_per_s = 0.0;
+    int sms = 0;
+    int st = sm_count(&sms);
+    if (st) return st;
+    unsigned int* sink = nullptr;
+    ProbeTimer t;
+    st = cuda_status(cudaMalloc(&sink, 4));
+    if (!st) st = t.init();
+    if (!st) st = cuda_status(cudaFuncSetAttribute(probe_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 131072));
+    const int32_t iters = rotate ? 2048 : 256;
+    double best = 0.0;
+    for (int pass = 0; pass < 4 && !st; ++pass) {
+        float ms = 0.f;
+        t.begin();
+        probe_gather_kernel<<<sms, 512, 131072>>>(iters, rotate ? 1 : 0, sink);
+        st = t.end(&ms);
+        if (!st && pass > 0 && ms > 0.f)     // 512 lanes x 8 slots x 128 bytes per iteration
+            best = std::max(best, static_cast<double>(sms) * 512.0 * iters * 8 * 128 / (ms * 1e-3) / 1e9);
+    }
+    if (!st) *gb_per_s = best;
+    cudaFree(sink);
+    return st;
+}
+
 int ebic_probe_fsetp_rate(double* gcompares_per_s) {
     if (!gcompares_per_s) return EBIC_ERR_ARG;
     *gcompares_per_s = 0.0;

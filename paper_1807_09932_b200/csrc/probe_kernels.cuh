@@ -3,7 +3,11 @@
 //   probe_read_kernel  L2 -> SM (buffer inside the 126 MB L2) or HBM (buffer far larger) read bandwidth with
 //                      plain coalesced 128-bit loads that bypass L1, 16 independent loads per thread in flight;
 //   probe_lds_kernel   conflict-free LDS.128 rate: the 128 B/clk/SM shared-memory data pipe of the tiled kernels;
-//   probe_fsetp_kernel issue rate of ordered float32 compares (FSETP.GE), the other pipe of the TILED_F32 kernel.
+//   probe_fsetp_kernel issue rate of ordered float32 compares (FSETP.GE), the other pipe of the TILED_F32 kernel;
+//   probe_gather_kernel the PAIRTILE access pattern on its own: every lane reads its own pseudo-random 128-byte slot
+//                      of a 128 KB shared-memory tile as eight LDS.128, the 16-byte unit rotated per lane (or not:
+//                      `rotate` = 0 shows the 8-way bank conflicts the rotation removes), AND + popcount as in the
+//                      kernel, no staging and no records.
 #pragma once
 #include "ebic_device.cuh"
 
@@ -69,6 +73,38 @@ probe_lds_kernel(int32_t iters, unsigned int* __restrict__ sink)
         for (int u = 0; u < 8; u += 2) { acc.x ^= v[u].x ^ v[u + 1].x; acc.y ^= v[u].y ^ v[u + 1].y; acc.z ^= v[u].z ^ v[u + 1].z; acc.w ^= v[u].w ^ v[u + 1].w; }
     }
     if ((acc.x ^ acc.y ^ acc.z ^ acc.w) == 0x9e3779b9u) *sink = acc.x;
+}
+
+// 512 threads, 128 KB of shared memory = 1,024 slots of 128 bytes.  Per iteration a lane ANDs the 1,024 "rows" of
+// 8 slots (two per step, as fitness_pairtile_kernel does) into 32 accumulator registers and popcounts them.
+__global__ void __launch_bounds__(512, 1)
+probe_gather_kernel(int32_t iters, int32_t rotate, unsigned int* __restrict__ sink)
+{
+    extern __shared__ __align__(128) unsigned char probe_smem[];
+    for (int i = threadIdx.x; i < 32768; i += blockDim.x) reinterpret_cast<uint32_t*>(probe_smem)[i] = ~0u ^ ((i * 2654435761u) >> 31);
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    const uint32_t base = smem_u32(probe_smem) + (rotate ? ((lane & 7) << 4) : 0u);
+    uint32_t state = threadIdx.x * 747796405u + blockIdx.x * 2891336453u + 1u;
+    unsigned int cnt = 0;
+    for (int32_t it = 0; it < iters; ++it) {
+        uint4 acc[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc[u] = make_uint4(~0u, ~0u, ~0u, ~0u);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            state = state * 1664525u + 1013904223u;
+            const uint32_t a = base + ((state >> 12) & 1023u) * 128u, b = base + ((state >> 22) & 1023u) * 128u;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const uint4 v = lds128(a ^ (u << 4)), w = lds128(b ^ (u << 4));
+                acc[u].x &= v.x & w.x; acc[u].y &= v.y & w.y; acc[u].z &= v.z & w.z; acc[u].w &= v.w & w.w;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) cnt += __popc(acc[u].x) + __popc(acc[u].y) + __popc(acc[u].z) + __popc(acc[u].w);
+    }
+    if (cnt == 0x9e3779b9u) *sink = cnt;
 }
 
 // Six independent chains of setp.ge.and.f32 (the form of the TILED_F32 inner loop: p = p & (cur >= prev)) per

@@ -508,6 +508,9 @@ def test_probe_read_bandwidth(B):
     fsetp = B.ebic_probe_fsetp_rate()
     assert 10_000 < smem < 60_000, smem
     assert 2_000 < fsetp < 80_000, fsetp
+    # PAIRTILE's gather (one slot per lane): conflict-free only with the per-lane rotation of the 16-byte unit
+    rotated, plain = B.ebic_probe_smem_gather(True), B.ebic_probe_smem_gather(False)
+    assert 10_000 < rotated < 60_000 and plain < rotated / 4, (rotated, plain)
 
 
 def test_empty_calls(B):
