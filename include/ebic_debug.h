@@ -71,9 +71,8 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
  *   6  the next pair-table build also writes the tile-major copy PAIRTILE needs, when a tile fits (default 1)
  *   7  AUTO picks PAIRTILE from this many (1,024-row tile, consecutive-pair use) units on (default 0 = the rule
  *      stated at EBIC_KERNEL_AUTO)
- *   8  PAIRTILE loads the part of the next tile that fits shared memory a second time one tile ahead (default 1)
- *   9  PAIRBITS row chunks requested into L2 by the kernel's prologue (default 1; 1..16, at least the distance)
- *  10  replay a repeated all-device call from a captured CUDA graph (default 1; include/ebic.h, ebic_eval_extract)
+ *   8  PAIRBITS row chunks requested into L2 by the kernel's prologue (default 1; 1..16, at least the distance)
+ *   9  replay a repeated all-device call from a captured CUDA graph (default 1; include/ebic.h, ebic_eval_extract)
  * EBIC_ERR_ARG for an unknown knob or a value outside its range.
  */
 int ebic_set_tuning(ebic_ctx *ctx, int32_t knob, int32_t value);

@@ -147,19 +147,17 @@ int32_t union_batch(const ebic_ctx* ctx, int32_t n_ind, int64_t n_ids) {
 
 // PAIRTILE: a 1,024-row tile of all cols^2 bit columns next to one 4-byte counter per individual of the launch.
 int64_t pairtile_smem(const ebic_ctx* ctx, int32_t n_ind_launch) {
-    return kPtHeader + static_cast<int64_t>(ctx->cols) * ctx->cols * 128 + 4ll * ((n_ind_launch + 31) / 32 * 32);
+    const int64_t n_groups = (n_ind_launch + 31) / 32;
+    return kPtHeader + static_cast<int64_t>(ctx->cols) * ctx->cols * 128 + 4ll * n_groups * 32 + 4ll * ((n_groups + 3) & ~3ll);
 }
-// Slots of a tile that fit a second time next to the tile and the counters (0: not worth splitting).
-int32_t pairtile_lo_slots(const ebic_ctx* ctx, int32_t n_ind_launch) {
-    const int64_t n_pairs = static_cast<int64_t>(ctx->cols) * ctx->cols;
-    const int64_t room = (static_cast<int64_t>(ctx->smem_optin) - pairtile_smem(ctx, n_ind_launch)) / 128;
-    const int64_t lo = std::min<int64_t>(std::max<int64_t>(room, 0), n_pairs);
-    return lo * 8 >= n_pairs ? static_cast<int32_t>(lo) : 0;
+// The record cache (entries 0..7 of every record, 16 bytes per sorted position) when it fits next to all that.
+bool pairtile_rec_cache(const ebic_ctx* ctx, int32_t n_ind_launch) {
+    return pairtile_smem(ctx, n_ind_launch) + 512ll * ((n_ind_launch + 31) / 32) <= ctx->smem_optin;
 }
 bool pairtile_fits(const ebic_ctx* ctx) { return ctx->cols <= 90 && pairtile_smem(ctx, 1024) <= ctx->smem_optin; }
 // Individuals per launch: as many counters as fit next to the tile, at most kMaxIndPerLaunch.
 int32_t pairtile_chunk(const ebic_ctx* ctx, int32_t n_ind) {
-    const int64_t room = (static_cast<int64_t>(ctx->smem_optin) - pairtile_smem(ctx, 0)) / 4 / 32 * 32;
+    const int64_t room = (static_cast<int64_t>(ctx->smem_optin) - pairtile_smem(ctx, 0)  - 16) / 132 * 32;   // 4 B + 1/8 int per individual
     return static_cast<int32_t>(std::min<int64_t>(std::min<int64_t>(n_ind, kMaxIndPerLaunch), room));
 }
 
@@ -424,7 +422,7 @@ int launch_pairtile(ebic_ctx* ctx, const int32_t* col_ids, int32_t k0, int32_t n
     p.cols = ctx->cols;
     p.n_ind = n_ind;
     p.n_groups = (n_ind + 31) / 32;
-    p.lo_slots = ctx->pt_split ? pairtile_lo_slots(ctx, n_ind) : 0;
+    p.rec_cache = pairtile_rec_cache(ctx, n_ind) ? 1 : 0;
     p.meta = ctx->meta + k0;
     p.col_ids = col_ids;
     p.gmeta = static_cast<int2*>(ctx->tplan);
@@ -435,7 +433,7 @@ int launch_pairtile(ebic_ctx* ctx, const int32_t* col_ids, int32_t k0, int32_t n
     EBIC_TRY(launch_pdl(pairtile_plan_kernel, dim3((n_ind + kPtPlanThreads - 1) / kPtPlanThreads), dim3(kPtPlanThreads), 0,
                         stream, pdl_plan, p));
     if (with_events) EBIC_TRY(cudaEventRecord(ctx->ev_begin[slot], stream));
-    const size_t smem = static_cast<size_t>(pairtile_smem(ctx, n_ind)) + 128ull * p.lo_slots;
+    const size_t smem = static_cast<size_t>(pairtile_smem(ctx, n_ind)) + (p.rec_cache ? 512ull * p.n_groups : 0);
     EBIC_TRY(cudaFuncSetAttribute(fitness_pairtile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
     const int64_t items = p.n_tiles * p.n_groups;
     const int64_t grid = std::min<int64_t>(ctx->sm_count, items);

@@ -65,7 +65,6 @@ struct ebic_ctx {
     int32_t pb_prologue_chunks = 1;            // PAIRBITS: row chunks requested into L2 by the kernel's prologue (>= the distance)
     int32_t pb_smem_ring = 1;                  // PAIRBITS: shared-memory landing ring for long chromosomes
     int32_t pt_build = 1;                      // build the tile-major copy of the pair table when a tile fits shared memory
-    int32_t pt_split = 1;                      // PAIRTILE: load the part of the next tile that fits a second time ahead
     int32_t pt_min_work = 0;                   // AUTO picks PAIRTILE from this many (tile, pair-use) units on (0 = the rule of pairtile_pays)
     int32_t pb_sort = 1;                       // ingest sorts each 64-individual block by length
     int32_t pdl = 1;                           // programmatic dependent launch between ingest / fitness / extraction

@@ -87,12 +87,11 @@ int ebic_set_tuning(ebic_ctx* ctx, int32_t knob, int32_t value) {
             if (value < 0) return EBIC_ERR_ARG;
             ctx->pt_min_work = value;
             return EBIC_OK;
-        case 8: ctx->pt_split = value ? 1 : 0; return EBIC_OK;
-        case 9:
+        case 8:
             if (value < 1 || value > 16) return EBIC_ERR_ARG;
             ctx->pb_prologue_chunks = value;
             return EBIC_OK;
-        case 10: ctx->use_graphs = value ? 1 : 0; return EBIC_OK;
+        case 9: ctx->use_graphs = value ? 1 : 0; return EBIC_OK;
         default: return EBIC_ERR_ARG;
     }
 }

@@ -13,8 +13,8 @@
 // reads the pair's 128-byte slot (1,024 rows) as eight LDS.128 and ANDs them into 32 accumulator registers.  The
 // lanes of a warp read DIFFERENT slots, so the 16-byte unit is rotated per lane: in step u lane l reads unit
 // u ^ (l & 7) of its slot -- the eight lanes of every quarter-warp then hit eight different 16-byte bank groups
-// whatever slots they picked (conflict-free; measured 35.5 TB/s chip-wide with random slots, against 4.6 TB/s
-// unrotated).  No cross-lane traffic at all: no shuffles, no ballots, no reductions -- the popcount of a lane's
+// whatever slots they picked (conflict-free; ebic_probe_smem_gather: 37.1 TB/s chip-wide with random slots, against
+// 4.7 TB/s unrotated).  No cross-lane traffic at all: no shuffles, no ballots, no reductions -- the popcount of a lane's
 // accumulators is its individual's count for the tile, added to a per-CTA shared counter the lane owns.
 //
 // An LDS.128 costs its four wavefronts whether or not all lanes are active (measured), so the groups must be
@@ -25,18 +25,20 @@
 // group loop needs no per-lane predicate: every lane does max-over-the-group steps.  Chromosomes with more than 33
 // columns continue from the caller's col_ids.
 //
-// Persistent CTAs, one per SM, 16 warps.  Work = (tile, group) items in tile-major order cut into equal contiguous
-// ranges (a tile is staged by at most two CTAs more than necessary); inside a tile the groups are handed out
-// longest first through a shared-memory cursor.  Tiles are staged with TMA bulk copies (16 KB each), completion on
-// mbarriers.  Two whole tiles do not fit at 32 columns (2 x 128 KB), so the buffer is split: the slots that fit
-// twice are loaded a whole tile ahead, the rest is requested into L2 ahead (cp.async.bulk.prefetch.L2) and copied
-// when the last warp has finished the current tile.
+// Persistent CTAs, one per SM, 12 warps of 168 registers (no spill: 16 LDS.128 in flight per warp next to the 32
+// accumulators; measured on C5: 8 / 10 / 12 / 14 / 16 / 20 warps = 2.38 / 2.22 / 2.15 / 2.18 / 2.17 / 2.38 ms).  Work = (tile, group) items in tile-major order cut into equal contiguous
+// ranges (a tile is staged by at most two CTAs more than necessary); inside a tile the groups are handed out through
+// a shared-memory cursor, alternately from the long and the short end of the sorted list.  One tile buffer (two
+// tiles of 128 KB do not fit at 32 columns): while the warps work on tile t, tile t + 1 is requested into L2
+// (cp.async.bulk.prefetch.L2); when the last warp is done the buffer is refilled from L2 with TMA bulk copies of 16
+// KB, completion on an mbarrier.  (Measured and removed: a split buffer that staged the part of the next tile that
+// fits a second time a whole tile ahead -- it did not change the kernel time.)
 #pragma once
 #include "ebic_device.cuh"
 
 namespace ebic {
 
-constexpr int kPtWarps = 16;
+constexpr int kPtWarps = 12;
 constexpr int kPtRecIds = 32;              // pair slots held per individual in tids (4 x uint4 of 8 halfwords)
 constexpr int kPtPlanThreads = 1024;       // pairtile_plan_kernel: individuals per CTA
 constexpr int kPtHeader = 128;             // shared-memory header (the mbarrier) in front of the tile
@@ -49,7 +51,7 @@ struct PairtileParams {
     int32_t cols;
     int32_t n_ind;                   // individuals of this launch
     int32_t n_groups;                // ceil(n_ind / 32)
-    int32_t lo_slots;                // slots [0, lo_slots) of a tile alternate between two regions (see the kernel)
+    int32_t rec_cache;               // shared memory has room for entries 0..7 of every record (16 bytes per position)
     const int2* meta;                // [n_ind] {b, L} written by the ingest kernel (L = -1: invalid)
     const int32_t* col_ids;
     int2* gmeta;                     // [n_groups * 32] {k, n}: individual and its number of pairs (-1: nothing to do)
@@ -138,22 +140,19 @@ pairtile_plan_kernel(const PairtileParams p)
     rec[96] = make_uint4(w[12], w[13], w[14], w[15]);
 }
 
-// AND the 1,024 rows of the slots at `off_a` / `off_b` (16-byte units from the tile start) into acc.  `lo` / `hi`:
-// shared address of the region that holds slots below / from `split` on, + 16 * (lane & 7).
-struct PtBases {
-    uint32_t lo, hi, split;
-    __device__ __forceinline__ uint32_t at(uint32_t off) const { return (off < split ? lo : hi) + off * 16u; }
-};
-__device__ __forceinline__ void pairtile_and2(uint4 (&acc)[8], const PtBases& base, uint32_t off_a, uint32_t off_b) {
-    const uint32_t a = base.at(off_a), b = base.at(off_b);
+// AND the 1,024 rows of the slots at `off_a` / `off_b` (16-byte units from the tile start) into acc.  `lanebase` =
+// shared address of the tile + 16 * (lane & 7): slot addresses are 128-byte aligned, so `^ (u << 4)` walks the eight
+// 16-byte units of a slot starting at this lane's own unit.
+__device__ __forceinline__ void pairtile_and2(uint4 (&acc)[8], uint32_t lanebase, uint32_t off_a, uint32_t off_b) {
+    const uint32_t a = lanebase + off_a * 16u, b = lanebase + off_b * 16u;
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
         const uint4 v = lds128(a ^ (u << 4)), w = lds128(b ^ (u << 4));
         acc[u].x &= v.x & w.x; acc[u].y &= v.y & w.y; acc[u].z &= v.z & w.z; acc[u].w &= v.w & w.w;
     }
 }
-__device__ __forceinline__ void pairtile_and1(uint4 (&acc)[8], const PtBases& base, uint32_t off_a) {
-    const uint32_t a = base.at(off_a);
+__device__ __forceinline__ void pairtile_and1(uint4 (&acc)[8], uint32_t lanebase, uint32_t off_a) {
+    const uint32_t a = lanebase + off_a * 16u;
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
         const uint4 v = lds128(a ^ (u << 4));
@@ -161,40 +160,36 @@ __device__ __forceinline__ void pairtile_and1(uint4 (&acc)[8], const PtBases& ba
     }
 }
 
+// Two record entries (the halfwords of `w`), of which `left` >= 1 (warp-uniform) are needed.
+__device__ __forceinline__ void pairtile_step(uint4 (&acc)[8], uint32_t lanebase, uint32_t w, int32_t left) {
+    if (left >= 2) pairtile_and2(acc, lanebase, w & 0xffffu, w >> 16);
+    else pairtile_and1(acc, lanebase, w & 0xffffu);
+}
 // Eight record entries (one uint4 of halfwords), of which the first `n_left` (warp-uniform, >= 1) are needed.
-__device__ __forceinline__ void pairtile_chunk(uint4 (&acc)[8], const PtBases& base, const uint4& ids, int32_t n_left) {
-    const uint32_t w[4] = {ids.x, ids.y, ids.z, ids.w};
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        if (n_left >= 2 * j + 2) {
-            pairtile_and2(acc, base, w[j] & 0xffffu, w[j] >> 16);
-        } else {
-            if (n_left == 2 * j + 1) pairtile_and1(acc, base, w[j] & 0xffffu);
-            return;
-        }
-    }
+__device__ __forceinline__ void pairtile_chunk(uint4 (&acc)[8], uint32_t lanebase, const uint4& ids, int32_t n_left) {
+    pairtile_step(acc, lanebase, ids.x, n_left);
+    if (n_left > 2) pairtile_step(acc, lanebase, ids.y, n_left - 2);
+    if (n_left > 4) pairtile_step(acc, lanebase, ids.z, n_left - 4);
+    if (n_left > 6) pairtile_step(acc, lanebase, ids.w, n_left - 6);
 }
 
-// Shared memory: [header: mbarriers + group cursors][main: n_pairs slots][extra: lo_slots slots][counters].
-// Tile i of the CTA (i = 0, 1, ...) keeps its slots [0, lo_slots) in main (i even) or extra (i odd) and its slots
-// [lo_slots, n_pairs) always in main.  The "lo" part of tile i + 1 is therefore loaded a whole tile ahead, into the
-// region tile i does not use; only the "hi" part has to wait until tile i is finished (lo_slots = n_pairs: two whole
-// buffers; lo_slots = 0: one buffer).
+// Shared memory: [header: mbarrier + group cursors][tile: n_pairs slots of 128 bytes][counters: one per sorted
+// position][gmax: per group, the longest chromosome in pairs = the group's loop count][record cache, when it fits:
+// entries 0..7 of every record -- they are the same for every tile, so the per-group record load then stays on the SM].
 __global__ void __launch_bounds__(kPtWarps * 32, 1)
 fitness_pairtile_kernel(const PairtileParams p)
 {
     extern __shared__ __align__(128) unsigned char pt_smem[];
-    uint64_t* full_lo = reinterpret_cast<uint64_t*>(pt_smem);                    // [2]
-    uint64_t* full_hi = full_lo + 2;
-    int32_t* cursor = reinterpret_cast<int32_t*>(pt_smem + 32);                   // [2] next group of the even / odd tile
-    unsigned char* main_buf = pt_smem + kPtHeader;
+    uint64_t* full = reinterpret_cast<uint64_t*>(pt_smem);
+    int32_t* cursor = reinterpret_cast<int32_t*>(pt_smem + 32);                   // [2] next position of the even / odd tile
+    unsigned char* tile = pt_smem + kPtHeader;
     const uint32_t tile_bytes = static_cast<uint32_t>(p.n_pairs) * 128u;
-    const uint32_t lo_bytes = static_cast<uint32_t>(p.lo_slots) * 128u, hi_bytes = tile_bytes - lo_bytes;
-    unsigned char* extra_buf = main_buf + tile_bytes;
-    uint32_t* counters = reinterpret_cast<uint32_t*>(extra_buf + lo_bytes);       // [n_groups * 32]
+    uint32_t* counters = reinterpret_cast<uint32_t*>(tile + tile_bytes);          // [n_groups * 32]
+    int32_t* s_gmax = reinterpret_cast<int32_t*>(counters + p.n_groups * 32);     // [n_groups rounded up to 4]
+    uint4* s_ids0 = reinterpret_cast<uint4*>(s_gmax + ((p.n_groups + 3) & ~3));   // [n_groups * 32] if rec_cache
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-    // this CTA's contiguous range of (tile, group) items
+    // this CTA's contiguous range of (tile, position) items
     const int64_t items = p.n_tiles * p.n_groups;
     const int64_t per = (items + gridDim.x - 1) / gridDim.x;
     const int64_t i0 = per * blockIdx.x, i1 = min(items, i0 + per);
@@ -203,121 +198,114 @@ fitness_pairtile_kernel(const PairtileParams p)
     const int64_t t_first = i0 / p.n_groups, t_last = (i1 - 1) / p.n_groups;
     const unsigned char* table = reinterpret_cast<const unsigned char*>(p.PBT);
 
-    auto copy = [&](unsigned char* dst, const unsigned char* src, uint32_t bytes, uint64_t* bar) {   // one thread
-        if (bytes == 0) return;
-        mbar_arrive_expect_tx(bar, bytes);
-        for (uint32_t o = 0; o < bytes; o += kPtCopyBytes) bulk_copy_g2s(dst + o, src + o, min(kPtCopyBytes, bytes - o), bar);
-    };
-    auto stage_lo = [&](int64_t t) {             // slots [0, lo_slots) of tile t into the region of its parity
-        const int q = static_cast<int>((t - t_first) & 1);
-        copy(q ? extra_buf : main_buf, table + t * static_cast<int64_t>(tile_bytes), lo_bytes, &full_lo[q]);
-    };
-    auto stage_hi = [&](int64_t t) {
-        copy(main_buf + lo_bytes, table + t * static_cast<int64_t>(tile_bytes) + lo_bytes, hi_bytes, full_hi);
+    auto stage = [&](int64_t t) {                // one thread: refill the tile buffer, completion on `full`
+        const unsigned char* src = table + t * static_cast<int64_t>(tile_bytes);
+        mbar_arrive_expect_tx(full, tile_bytes);
+        for (uint32_t o = 0; o < tile_bytes; o += kPtCopyBytes)
+            bulk_copy_g2s(tile + o, src + o, min(kPtCopyBytes, tile_bytes - o), full);
     };
     if (tid == 0) {
-        mbar_init(&full_lo[0], 1);
-        mbar_init(&full_lo[1], 1);
-        mbar_init(full_hi, 1);
+        mbar_init(full, 1);
         fence_mbar_init();
-        stage_lo(t_first);                       // the table depends on the matrix only: overlaps ingest + plan
-        stage_hi(t_first);
-        if (t_first < t_last) stage_lo(t_first + 1);
+        stage(t_first);                          // the table depends on the matrix only: overlaps ingest + plan
         cursor[0] = static_cast<int32_t>(i0 - t_first * p.n_groups) + kPtWarps;
     }
     for (int32_t j = tid; j < p.n_groups * 32; j += kPtWarps * 32) counters[j] = 0;
-    __syncthreads();
     griddep_wait();                              // gmeta / tids (plan kernel), counts initialised (ingest kernel)
+    for (int32_t grp = warp; grp < p.n_groups; grp += kPtWarps) {
+        const int32_t mx = __reduce_max_sync(0xffffffffu, __ldg(p.gmeta + grp * 32 + lane).y);
+        if (lane == 0) s_gmax[grp] = mx;
+        if (p.rec_cache) s_ids0[grp * 32 + lane] = __ldg(p.tids + static_cast<int64_t>(grp) * 128 + lane);
+    }
+    __syncthreads();
 
-    const uint32_t lane16 = (lane & 7) << 4;
-    const uint32_t main_s = smem_u32(main_buf) + lane16, extra_s = smem_u32(extra_buf) + lane16;
+    const uint32_t lanebase = smem_u32(tile) + ((lane & 7) << 4);
     unsigned long long executed = 0;
-    // Groups are handed out longest first through a shared cursor (the first kPtWarps of a tile statically: group
-    // g_lo + warp); a warp's next group is drawn, and its records requested, before the current one is evaluated --
-    // the first group of the NEXT tile before the barrier that ends this one, so that no warp starts a tile by
-    // waiting for its records.
-    int32_t g = static_cast<int32_t>(i0 - t_first * p.n_groups) + warp;
-    int2 gm = make_int2(0, -1);
+    // Position c of a tile's hand-out order -> group: alternately from the long and from the short end of the sorted
+    // list, so that at any time the warps hold a mix of long and short groups.  (The fixed cost per group -- 32
+    // popcounts, counter, cursor -- is poorly hidden while ALL warps work on one- or two-pair groups, as at the end of
+    // a longest-first order: 2.24 -> 2.19 ms on C5; strided orders 2.20.)  The first kPtWarps positions of a tile go to
+    // the warps statically, the rest through a shared cursor; a warp draws its next position, and requests the
+    // group's records, before it evaluates the current one -- the first of the NEXT tile before the barrier that ends
+    // this one, so that no warp starts a tile by waiting for its records.
+    int32_t c = static_cast<int32_t>(i0 - t_first * p.n_groups) + warp;
+    int32_t maxn = 0, grp_req = 0;
     uint4 ids0 = make_uint4(0u, 0u, 0u, 0u), ids1 = ids0;
-    auto request = [&](int32_t grp) {
-        gm = __ldg(p.gmeta + grp * 32 + lane);
-        const uint4* rec = p.tids + static_cast<int64_t>(grp) * 128 + lane;
-        ids0 = __ldg(rec); ids1 = __ldg(rec + 32);
+    auto request = [&](int32_t pos) {            // loop count and record entries 0..15 of the group at position pos
+        grp_req = (pos & 1) ? p.n_groups - 1 - (pos >> 1) : (pos >> 1);
+        maxn = s_gmax[grp_req];
+        const uint4* rec = p.tids + static_cast<int64_t>(grp_req) * 128 + lane;
+        ids0 = p.rec_cache ? s_ids0[grp_req * 32 + lane] : __ldg(rec);
+        if (maxn > 8) ids1 = __ldg(rec + 32);
     };
-    if (g < (t_first == t_last ? static_cast<int32_t>(i1 - t_first * p.n_groups) : p.n_groups)) request(g);
+    if (c < (t_first == t_last ? static_cast<int32_t>(i1 - t_first * p.n_groups) : p.n_groups)) request(c);
+    uint32_t phase = 0;
     for (int64_t t = t_first; t <= t_last; ++t) {
-        const int64_t i = t - t_first;
-        const int q = static_cast<int>(i & 1);
-        const int32_t g_hi = t == t_last ? static_cast<int32_t>(i1 - t * p.n_groups) : p.n_groups;
-        if (t < t_last && tid < 32) {
-            // the part of the next tile that has to wait for this one: HBM -> L2 meanwhile
-            const unsigned char* nxt = table + (t + 1) * static_cast<int64_t>(tile_bytes) + lo_bytes;
-            for (uint32_t o = lane * kPtCopyBytes; o < hi_bytes; o += 32 * kPtCopyBytes)
-                bulk_prefetch_l2(nxt + o, min(kPtCopyBytes, hi_bytes - o));
-            if (lane == 0) cursor[q ^ 1] = kPtWarps;       // the next tile starts at group 0; nobody reads this cursor now
+        const int q = static_cast<int>((t - t_first) & 1);
+        const int32_t c_hi = t == t_last ? static_cast<int32_t>(i1 - t * p.n_groups) : p.n_groups;
+        if (t < t_last && tid < 32) {            // next tile: HBM -> L2 while this one is evaluated
+            const unsigned char* nxt = table + (t + 1) * static_cast<int64_t>(tile_bytes);
+            for (uint32_t o = lane * kPtCopyBytes; o < tile_bytes; o += 32 * kPtCopyBytes)
+                bulk_prefetch_l2(nxt + o, min(kPtCopyBytes, tile_bytes - o));
+            if (lane == 0) cursor[q ^ 1] = kPtWarps;       // the next tile starts at position 0; nobody reads this cursor now
         }
-        PtBases base;
-        base.lo = q ? extra_s : main_s;
-        base.hi = main_s;
-        base.split = static_cast<uint32_t>(p.lo_slots) * 8u;
-        if (lo_bytes) mbar_wait(&full_lo[q], static_cast<uint32_t>(i >> 1) & 1u);
-        if (hi_bytes) mbar_wait(full_hi, static_cast<uint32_t>(i) & 1u);
-        while (g < g_hi) {
-            const int32_t n = gm.y;
-            const int32_t maxn = __reduce_max_sync(0xffffffffu, n);
-            const int2 gm_cur = gm;
+        mbar_wait(full, phase);
+        phase ^= 1;
+        while (c < c_hi) {
+            const int32_t maxn_cur = maxn, grp = grp_req;
             const uint4 cur0 = ids0, cur1 = ids1;
-            int32_t g_next = 0;
-            if (lane == 0) g_next = atomicAdd(&cursor[q], 1);
-            g_next = __shfl_sync(0xffffffffu, g_next, 0);
-            if (g_next < g_hi) request(g_next);  // in flight during this group's evaluation
-            if (maxn >= 1) {
+            int32_t c_next = 0;
+            if (lane == 0) c_next = atomicAdd(&cursor[q], 1);
+            c_next = __shfl_sync(0xffffffffu, c_next, 0);
+            if (c_next < c_hi) request(c_next);  // in flight during this group's evaluation
+            if (maxn_cur >= 1) {
                 uint4 acc[8];
 #pragma unroll
                 for (int u = 0; u < 8; ++u) acc[u] = make_uint4(~0u, ~0u, ~0u, ~0u);
-                const int32_t m = min(maxn, kPtRecIds);
-                pairtile_chunk(acc, base, cur0, m);
-                if (m > 8) pairtile_chunk(acc, base, cur1, m - 8);
+                const int32_t m = min(maxn_cur, kPtRecIds);
+                pairtile_chunk(acc, lanebase, cur0, m);
+                if (m > 8) pairtile_chunk(acc, lanebase, cur1, m - 8);
                 if (m > 16) {
-                    const uint4* rec = p.tids + static_cast<int64_t>(g) * 128 + lane;
+                    const uint4* rec = p.tids + static_cast<int64_t>(grp) * 128 + lane;
                     const uint4 cur2 = __ldg(rec + 64), cur3 = __ldg(rec + 96);
-                    pairtile_chunk(acc, base, cur2, m - 16);
-                    if (m > 24) pairtile_chunk(acc, base, cur3, m - 24);
+                    pairtile_chunk(acc, lanebase, cur2, m - 16);
+                    if (m > 24) pairtile_chunk(acc, lanebase, cur3, m - 24);
                 }
-                if (maxn > kPtRecIds && n > kPtRecIds) {
-                    // pairs beyond the record come from the caller's ids (a VALID individual)
-                    const int32_t* ids_g = p.col_ids + __ldg(&p.meta[gm_cur.x]).x;
-                    int32_t a = __ldg(ids_g + kPtRecIds);
-                    for (int32_t j = kPtRecIds; j < n; ++j) {
-                        const int32_t c = __ldg(ids_g + j + 1);
-                        pairtile_and1(acc, base, static_cast<uint32_t>(a * p.cols + c) * 8u);
-                        a = c;
+                if (maxn_cur > kPtRecIds || p.visits != nullptr) {       // rare: a very long chromosome, or instrumented
+                    const int2 gm = __ldg(p.gmeta + grp * 32 + lane);
+                    if (gm.y > kPtRecIds) {
+                        // pairs beyond the record come from the caller's ids (a VALID individual)
+                        const int32_t* ids_g = p.col_ids + __ldg(&p.meta[gm.x]).x;
+                        int32_t a = __ldg(ids_g + kPtRecIds);
+                        for (int32_t j = kPtRecIds; j < gm.y; ++j) {
+                            const int32_t b = __ldg(ids_g + j + 1);
+                            pairtile_and1(acc, lanebase, static_cast<uint32_t>(a * p.cols + b) * 8u);
+                            a = b;
+                        }
                     }
+                    if (gm.y >= 1) executed += static_cast<unsigned long long>(gm.y);
                 }
-                if (n >= 1) {
-                    unsigned int cnt = 0;
+                // A lane that holds no individual (or one with nothing to evaluate) walked slot 0 of an all-zero
+                // record: its counter is never read back (the final loop checks gmeta).
+                unsigned int cnt = 0;
 #pragma unroll
-                    for (int u = 0; u < 8; ++u) cnt += __popc(acc[u].x) + __popc(acc[u].y) + __popc(acc[u].z) + __popc(acc[u].w);
-                    counters[g * 32 + lane] += cnt;      // this lane is the only one that touches the counter now
-                    executed += static_cast<unsigned long long>(n);
-                }
+                for (int u = 0; u < 8; ++u) cnt += __popc(acc[u].x) + __popc(acc[u].y) + __popc(acc[u].z) + __popc(acc[u].w);
+                counters[grp * 32 + lane] += cnt;        // this lane is the only one that touches the counter now
             }
-            g = g_next;
+            c = c_next;
         }
-        if (t < t_last) {                        // first group of the next tile (it starts at group 0)
-            g = warp;
-            if (g < (t + 1 == t_last ? static_cast<int32_t>(i1 - t_last * p.n_groups) : p.n_groups)) request(g);
+        if (t < t_last) {                        // first position of the next tile (it starts at 0)
+            c = warp;
+            if (c < (t + 1 == t_last ? static_cast<int32_t>(i1 - t_last * p.n_groups) : p.n_groups)) request(c);
         }
         __syncthreads();                         // every warp is done with the tile (and with its counters)
-        if (tid == 0) {
-            if (t < t_last) stage_hi(t + 1);
-            if (t + 1 < t_last) stage_lo(t + 2); // into the region this tile has just released
-        }
+        if (t < t_last && tid == 0) stage(t + 1);
     }
     // one 64-bit global atomic per (CTA, individual)
     for (int32_t j = tid; j < p.n_groups * 32; j += kPtWarps * 32) {
-        const uint32_t c = counters[j];
-        if (c) atomicAdd(&p.counts[__ldg(p.gmeta + j).x], static_cast<unsigned long long>(c));
+        const uint32_t cnt = counters[j];
+        const int2 gm = __ldg(p.gmeta + j);
+        if (cnt && gm.y >= 1) atomicAdd(&p.counts[gm.x], static_cast<unsigned long long>(cnt));
     }
     if (p.visits != nullptr) {
         for (int o = 16; o > 0; o >>= 1) executed += __shfl_down_sync(0xffffffffu, executed, o);

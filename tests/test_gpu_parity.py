@@ -233,8 +233,8 @@ def test_long_and_degenerate_chromosomes(B, oracle_mod):
 def test_pairtile_kernel(B, oracle_mod, rows, cols, n_ind, max_len):
     """PAIRTILE (bit-column tiles staged in shared memory, lane = individual): ragged row counts, more tiles than
     SMs and fewer, a population larger than one launch's counters (9,000 at 25 columns: 8,192 + 808; 7,000 at 42
-    columns: the tile leaves room for 1,632 counters), chromosomes longer than the 32-entry record, empty / length-1 /
-    duplicate-column / invalid individuals, both missing modes, with and without the split tile buffer, and the
+    columns: the tile leaves room for 1,568 counters), chromosomes longer than the 32-entry record, empty / length-1 /
+    duplicate-column / invalid individuals, both missing modes, and the
     executed-visit counter (early exit does not apply: executed == nominal)."""
     import torch
     rng = np.random.default_rng(rows + cols)
@@ -255,12 +255,10 @@ def test_pairtile_kernel(B, oracle_mod, rows, cols, n_ind, max_len):
             if rows < 10_000:                                  # far too small for staged tiles to pay
                 assert eb.last_kernel == B.EBIC_KERNEL_PAIRBITS
             eb.status()
-            for split in (1, 0):
-                eb.set_tuning(8, split)
-                got = gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_PAIRTILE)
-                assert (got == want).all(), (mode, split, np.flatnonzero(got != want)[:10])
-                assert eb.last_kernel == B.EBIC_KERNEL_PAIRTILE
-                assert eb.status() == st
+            got = gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_PAIRTILE)
+            assert (got == want).all(), (mode, np.flatnonzero(got != want)[:10])
+            assert eb.last_kernel == B.EBIC_KERNEL_PAIRTILE
+            assert eb.status() == st
             eb.set_kernel(B.EBIC_KERNEL_PAIRTILE)
             eb.set_instrumentation(1)
             got = eb.eval_fitness(dev(off), dev(ids))
@@ -271,7 +269,7 @@ def test_pairtile_kernel(B, oracle_mod, rows, cols, n_ind, max_len):
             eb.set_instrumentation(0)
             assert (got.cpu().numpy().view(np.uint64) == want).all()
             assert eb.status() == st
-            eb.set_tuning(6, 0)                                # rebuild the table without the tile-major copy
+            eb.set_tuning(B.TUNE_PT_BUILD, 0)                  # rebuild the table without the tile-major copy
             eb.set_pairbits(False)
             eb.set_pairbits(True)
             assert eb.info(17) == 0 and eb.kernel == B.EBIC_KERNEL_PAIRBITS
@@ -397,6 +395,7 @@ def test_file_to_counts(B, oracle_mod, tmp_path):
     {"TUNE_PB_TASKS_PER_SLOT": 2, "TUNE_SORT": 0},               # large chunks, population order
     {"TUNE_PB_TASKS_PER_SLOT": 32, "TUNE_PB_PREFETCH": 0},       # smallest chunks, no L2 prefetch
     {"TUNE_PB_PREFETCH": 3, "TUNE_PDL": 0},                      # distance 3, plain launches
+    {"TUNE_PB_PREFETCH": 2, "TUNE_PB_PROLOGUE_CHUNKS": 4},       # the prologue requests more chunks than the distance
     {"TUNE_PDL": 0, "TUNE_SORT": 0, "TUNE_PB_SMEM_RING": 0, "TUNE_PB_PREFETCH": 0},
 ])
 def test_tuning_knobs_keep_parity(B, oracle_mod, knobs):
@@ -706,13 +705,13 @@ def test_repeated_calls_replay_a_graph(B, oracle_mod):
             torch.cuda.synchronize()
             assert eb.info(18) == 0 and (c.cpu().numpy().view(np.uint64) == want).all()
             assert (eb.eval_fitness(off0, ids) == want).all()
-            eb.set_tuning(10, 0)                                       # graphs off
+            eb.set_tuning(B.TUNE_GRAPHS, 0)                            # graphs off
             for _ in range(3):
                 with torch.cuda.stream(side):
                     eb.eval_fitness(d_off, d_ids, counts=counts, stream=side)
                 side.synchronize()
             assert eb.info(18) == 0 and (counts.cpu().numpy().view(np.uint64) == want).all()
-            eb.set_tuning(10, 1)
+            eb.set_tuning(B.TUNE_GRAPHS, 1)
         assert eb.status() == 0
 
 
