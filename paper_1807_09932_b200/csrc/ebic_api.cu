@@ -333,7 +333,11 @@ int launch_tiled(ebic_ctx* ctx, const void* M, int32_t T, int32_t k0, int32_t n_
 int64_t pairbits_chunk_words(const ebic_ctx* ctx, int32_t n_ind) {
     const int64_t want_tasks = static_cast<int64_t>(ctx->pb_tasks_per_slot) * ctx->sm_count * 32;
     const int64_t cw = (ctx->ld / 32) * n_ind / want_tasks;
-    return std::max<int64_t>(kPairbitsStepWords, std::min<int64_t>(8 * kPairbitsStepWords, cw / kPairbitsStepWords * kPairbitsStepWords));
+    int64_t words = std::max<int64_t>(kPairbitsStepWords, std::min<int64_t>(8 * kPairbitsStepWords, cw / kPairbitsStepWords * kPairbitsStepWords));
+    // the row chunk is the grid's y axis (<= 65,535): a tiny population on a very long matrix gets longer chunks
+    const int64_t ldw = ctx->ld / 32;
+    const int64_t min_words = ((ldw + 65534) / 65535 + kPairbitsStepWords - 1) / kPairbitsStepWords * kPairbitsStepWords;
+    return std::max(words, min_words);
 }
 // The L2 prefetches request EVERY bit column once; that pays only when the population uses most of the cols^2
 // columns (n_ids - n_ind = number of pair uses).  A sparse population (wide matrix: P3 uses 14 % of 96,100
@@ -384,6 +388,7 @@ PairbitsParams pairbits_params(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_
     p.counts = counts;
     p.visits = ctx->count_visits ? ctx->d_visits : nullptr;
     p.n_pairs = ctx->cols * ctx->cols;
+    p.cols_per_task = (p.n_pairs + n_ind - 1) / std::max(n_ind, 1);
     p.prefetch_dist = pairbits_dense(ctx, n_ind, n_ids) ? ctx->pb_prefetch_dist : 0;
     p.prologue_chunks = std::max(p.prefetch_dist, p.prefetch_dist > 0 ? ctx->pb_prologue_chunks : 0);
     return p;
@@ -393,12 +398,11 @@ int launch_pairbits(ebic_ctx* ctx, const int32_t* col_ids, int32_t n_ind, int64_
                     cudaStream_t stream, bool pdl) {
     const PairbitsParams p = pairbits_params(ctx, col_ids, n_ind, n_ids, counts);
     const int64_t cw = p.chunk_words;
-    const int64_t tasks = static_cast<int64_t>(p.n_chunks) * n_ind;
-    const int64_t grid = (tasks + kPairbitsWarps - 1) / kPairbitsWarps;
-    if (grid > 0x7fffffffll) return EBIC_ERR_ARG;
-    ctx->last_grid = static_cast<int32_t>(grid);
+    const int64_t gx = (n_ind + kPairbitsWarps - 1) / kPairbitsWarps;
+    if (p.n_chunks > 65535) return EBIC_ERR_ARG;                 // cannot happen: chunks grow to 65,536 rows (2^31 rows: 32,768)
+    ctx->last_grid = static_cast<int32_t>(std::min<int64_t>(gx * p.n_chunks, 0x7fffffff));
     ctx->last_T = static_cast<int32_t>(cw * 32);
-    const dim3 g(static_cast<unsigned>(grid)), b(kPairbitsWarps * 32);
+    const dim3 g(static_cast<unsigned>(gx), static_cast<unsigned>(p.n_chunks)), b(kPairbitsWarps * 32);
     cudaError_t e;
     if (ctx->pb_smem_ring) {
         const size_t smem = kPairbitsWarps * 4096;

@@ -36,6 +36,7 @@ struct PairbitsParams {
     unsigned long long* counts;
     unsigned long long* visits;      // executed (row, pair) visits (instrumented) or nullptr
     int32_t n_pairs;                 // cols * cols bit columns in PB
+    int32_t cols_per_task;           // ceil(n_pairs / n_ind): bit columns a task requests for the prefetched chunk
     int32_t prefetch_dist;           // tasks of chunk g prefetch a slice of the bit columns of chunk g + dist into L2 (0 = off);
     int32_t prologue_chunks;         // chunks 0 .. prologue_chunks-1 (>= dist) are requested by the kernel's prologue,
                                      // before it waits for the ingest
@@ -138,20 +139,18 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
     return done;
 }
 
-// One warp task: record j = task % n_ind (individual k = its word 1) on row chunk g = task / n_ind.
+// One warp task: record j (individual k = its word 1) on row chunk g.
 // `rec` = this lane's word of the record.
 template <bool EARLY_EXIT, bool SMEM>
-__device__ __forceinline__ void pairbits_task(const PairbitsParams& p, int64_t task, uint32_t rec, int lane, uint32_t ring,
+__device__ __forceinline__ void pairbits_task(const PairbitsParams& p, int64_t g, int32_t j, uint32_t rec, int lane, uint32_t ring,
                                               unsigned long long& executed)
 {
-    const int64_t g = task / p.n_ind;
-    const int32_t j = static_cast<int32_t>(task - g * p.n_ind);
     const int64_t w_begin = g * p.chunk_words;
     if (w_begin >= p.ldw) return;                                // warp-uniform
     if (p.prefetch_dist > 0) {
         // Every bit column of chunk g + dist is requested from HBM exactly once, by one lane of one task of chunk g:
         // the demand loads that arrive `dist` chunks later then hit L2.  (Chunks 0 .. dist-1: the kernel's prologue.)
-        const int32_t per = (p.n_pairs + p.n_ind - 1) / p.n_ind;     // columns per task
+        const int32_t per = p.cols_per_task;                         // ceil(n_pairs / n_ind)
         const int64_t pw = (g + p.prefetch_dist) * p.chunk_words;
         if (pw < p.ldw && g + p.prefetch_dist >= p.prologue_chunks) {
             const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.chunk_words), p.ldw - pw)) * 4u;
@@ -198,10 +197,12 @@ __device__ __forceinline__ void pairbits_task(const PairbitsParams& p, int64_t t
     if (lane == 0 && cnt) atomicAdd(&p.counts[k], static_cast<unsigned long long>(cnt));
 }
 
-// One task per warp, a CTA of kPairbitsWarps warps per consecutive tasks: the hardware block scheduler balances
-// the load.  Launched with programmatic dependent launch right behind the ingest kernel: the prologue (the HBM ->
-// L2 requests for the first chunks of every bit column, which depend on the matrix only) overlaps the ingest;
-// griddep_wait() then orders the record loads and the count atomics behind it.
+// One task per warp; grid = (ceil(n_ind / kPairbitsWarps), n_chunks): blockIdx.y is the row chunk, the CTA's warps
+// take consecutive records of it (no division anywhere on the way to the first load), and the hardware block
+// scheduler -- x fastest -- walks the chunks in order and balances the load.  Launched with programmatic dependent
+// launch right behind the ingest kernel: the prologue (the HBM -> L2 requests for the first chunks of every bit
+// column, which depend on the matrix only) overlaps the ingest; griddep_wait() then orders the record loads and the
+// count atomics behind it.
 template <bool EARLY_EXIT, bool SMEM>
 __global__ void __launch_bounds__(kPairbitsWarps * 32)
 fitness_pairbits_kernel(const PairbitsParams p)
@@ -209,21 +210,21 @@ fitness_pairbits_kernel(const PairbitsParams p)
     extern __shared__ __align__(16) unsigned char pb_ring[];     // SMEM: one 4 KB landing ring per warp
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     griddep_launch_dependents();                                 // a dependent extraction launch may be scheduled
-    if (p.prefetch_dist > 0) {
+    if (p.prefetch_dist > 0 && blockIdx.y == 0) {
         // chunks 0 .. prologue_chunks-1 of every bit column, each requested exactly once, spread over the first CTAs
-        const int64_t n_pro = min(static_cast<int64_t>(gridDim.x), static_cast<int64_t>(p.n_pairs + 63) / 64);
-        if (blockIdx.x < n_pro) {
+        const int32_t n_pro = min(static_cast<int32_t>(gridDim.x), (p.n_pairs + 63) / 64);
+        if (static_cast<int32_t>(blockIdx.x) < n_pro) {
             const uint32_t bytes = static_cast<uint32_t>(min(static_cast<int64_t>(p.prologue_chunks) * p.chunk_words, p.ldw)) * 4u;
-            for (int64_t pair = static_cast<int64_t>(blockIdx.x) * 64 + threadIdx.x; pair < p.n_pairs; pair += n_pro * 64)
-                bulk_prefetch_l2(p.PB + pair * p.ldw, bytes);
+            for (int32_t pair = blockIdx.x * 64 + threadIdx.x; pair < p.n_pairs; pair += n_pro * 64)
+                bulk_prefetch_l2(p.PB + static_cast<int64_t>(pair) * p.ldw, bytes);
         }
     }
     griddep_wait();
-    const int64_t task = static_cast<int64_t>(blockIdx.x) * kPairbitsWarps + warp;
-    if (task >= static_cast<int64_t>(p.n_chunks) * p.n_ind) return;
-    const uint32_t rec = __ldg(p.prec + 32ll * (task % p.n_ind) + lane);   // one coalesced 128 B load
+    const int32_t j = blockIdx.x * kPairbitsWarps + warp;
+    if (j >= p.n_ind) return;
+    const uint32_t rec = __ldg(p.prec + 32ll * j + lane);        // one coalesced 128 B load
     unsigned long long executed = 0;
-    pairbits_task<EARLY_EXIT, SMEM>(p, task, rec, lane, SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u, executed);
+    pairbits_task<EARLY_EXIT, SMEM>(p, blockIdx.y, j, rec, lane, SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u, executed);
     if (lane == 0 && p.visits != nullptr && executed) atomicAdd(p.visits, executed);
 }
 

@@ -187,7 +187,7 @@ fitness_prefix_kernel(const PrefixParams pp)
     if (cnt == 1) {                                              // not grouped: the plain task on this member's record
         const int32_t j = __ldg(grp + 1);
         const uint32_t rec = __ldg(p.prec + 32ll * j + lane);
-        pairbits_task<EARLY_EXIT, false>(p, g_chunk * p.n_ind + j, rec, lane, 0u, executed);
+        pairbits_task<EARLY_EXIT, false>(p, g_chunk, j, rec, lane, 0u, executed);
     } else {
         uint32_t rec[kPrefixGroup];
 #pragma unroll
