@@ -61,7 +61,7 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
 
 /*
  * Tuning knobs of the launch configuration (DESIGN.md 6.4 says how the defaults were chosen).  `knob`:
- *   0  PAIRBITS warp tasks per resident warp slot (default 8; 1..64): sets the rows per task
+ *   0  PAIRBITS warp tasks per resident warp slot (default 12; 1..64): sets the rows per task
  *   1  PAIRBITS L2 prefetch distance in row chunks (default 1; 0 = off, <= 8)
  *   2  PAIRBITS shared-memory landing ring for chromosomes of >= 9 columns (default 1)
  *   3  ingest sorts every block of 64 individuals by length, so the two warps of a PAIRBITS CTA finish together

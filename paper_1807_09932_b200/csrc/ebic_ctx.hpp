@@ -60,7 +60,7 @@ struct ebic_ctx {
     int32_t kernel_request = 0;                // EBIC_KERNEL_AUTO
     int32_t early_exit = 1;
     int32_t extract_pairbits = 1;              // extraction reads the pair table when it exists
-    int32_t pb_tasks_per_slot = 8;             // PAIRBITS: warp tasks per resident warp slot
+    int32_t pb_tasks_per_slot = 12;            // PAIRBITS: warp tasks per resident warp slot
     int32_t pb_prefetch_dist = 1;              // PAIRBITS: L2 prefetch distance in chunks (0 = off)
     int32_t pb_prologue_chunks = 1;            // PAIRBITS: row chunks requested into L2 by the kernel's prologue (>= the distance)
     int32_t pb_smem_ring = 1;                  // PAIRBITS: shared-memory landing ring for long chromosomes
