@@ -613,7 +613,10 @@ int extract_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids
     const bool pdl = ctx->pdl != 0;
     ctx->launches++;
     if (ctx->PB && ctx->extract_pairbits) {
-        const dim3 grid(static_cast<unsigned>((words32 + 255) / 256), static_cast<unsigned>(std::min<int32_t>(n_chosen, 65535)));
+        // about 16 CTAs per SM in total: a CTA's prologue (chosen -> offsets -> ids) is paid once for several blocks
+        const int64_t n_wblocks = (words32 + 1023) / 1024;
+        const int64_t gx = std::max<int64_t>(1, std::min<int64_t>(n_wblocks, (16ll * ctx->sm_count + n_chosen - 1) / n_chosen));
+        const dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>(std::min<int32_t>(n_chosen, 65535)));
         return ebic_host::cuda_status(launch_pdl(
             extract_rows_pairbits_kernel, grid, dim3(256), 0, stream, pdl, ctx->PB, ctx->ld, ctx->rows, ctx->cols,
             ctx->missing_mode == EBIC_MISSING_ON, ctx->nanmask, offsets, col_ids, n_ind, n_ids, chosen, n_chosen,

@@ -117,9 +117,10 @@ extract_rows_kernel(const float* __restrict__ Mc, int64_t ld, int64_t rows, int3
 
 // Extraction from the pair-relation bit columns (loader_kernels.cuh): for L >= 2 the mask IS the AND of
 // the individual's L-1 bit columns, so a chosen individual costs (L-1) * rows / 8 bytes of HBM reads
-// instead of 4 * L * rows -- 32x less.  One thread per 32-bit mask word; a warp reads 128 contiguous
-// bytes of a bit column per pair.  Padding rows are NaN, so bits >= rows are already zero.  L <= 1 as above.
-// grid.x over blocks of 256 words, grid.y over chosen (strided).
+// instead of 4 * L * rows -- 32x less.  One thread per FOUR 32-bit mask words (16-byte loads, four in flight per
+// thread); a warp reads 512 contiguous bytes of a bit column per pair.  Padding rows are NaN, so bits >= rows are already zero.  L <= 1 as above.
+// grid.x strided over blocks of 1,024 words (a CTA validates its individual once and then streams several blocks),
+// grid.y over chosen (strided).
 __global__ void __launch_bounds__(256)
 extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_t rows, int32_t cols,
                              int32_t missing_on, const uint32_t* __restrict__ nanmask,
@@ -133,9 +134,9 @@ extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_
     __shared__ int32_t s_bad;
     __shared__ unsigned int s_cnt;
     const int tid = threadIdx.x, lane = tid & 31;
-    const int64_t ldw = ld / 32;
-    const int64_t w = static_cast<int64_t>(blockIdx.x) * 256 + tid;      // this thread's mask word
-    const uint32_t* wbase = PB + min(w, ldw - 1);                          // + pair * ldw
+    const int64_t ldw = ld / 32;                                           // a multiple of 32: 16-byte units never straddle
+    const int64_t ldw4 = ldw >> 2;
+    const int64_t n_wblocks = (words32 + 1023) / 1024;                     // blocks of 1,024 mask words, strided over grid.x
 
     for (int32_t j = blockIdx.y; j < n_chosen; j += gridDim.y) {
         if (tid == 0) {
@@ -168,37 +169,56 @@ extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_
         if (!bad) bad = s_bad;
         if (bad && tid == 0 && blockIdx.x == 0) atomicMax(err, bad);
 
-        unsigned int word = 0;
+        unsigned int local = 0;
+        for (int64_t wb = blockIdx.x; wb < n_wblocks; wb += gridDim.x) {
+        const int64_t w = (wb * 256 + tid) * 4;                            // this thread's four mask words w .. w + 3
+        const uint4* wbase = reinterpret_cast<const uint4*>(PB) + (min(w, ldw - 4) >> 2);   // + pair * (ldw / 4)
+        uint4 word = make_uint4(0u, 0u, 0u, 0u);
         if (w < words32 && !bad) {
             if (L >= 2) {
-                word = 0xffffffffu;
+                word = make_uint4(~0u, ~0u, ~0u, ~0u);
                 const int32_t npr = L - 1;
                 const int32_t ns = min(npr, kExtractMaxSmemIds);
                 int32_t i = 0;
-                for (; i + 4 <= ns; i += 4) {
-                    const unsigned int v0 = __ldg(wbase + static_cast<int64_t>(s_pair[i]) * ldw);
-                    const unsigned int v1 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 1]) * ldw);
-                    const unsigned int v2 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 2]) * ldw);
-                    const unsigned int v3 = __ldg(wbase + static_cast<int64_t>(s_pair[i + 3]) * ldw);
-                    word &= v0 & v1 & v2 & v3;
+                for (; i + 4 <= ns; i += 4) {                   // four 16-byte loads in flight per thread
+                    const uint4 v0 = __ldg(wbase + s_pair[i] * ldw4), v1 = __ldg(wbase + s_pair[i + 1] * ldw4);
+                    const uint4 v2 = __ldg(wbase + s_pair[i + 2] * ldw4), v3 = __ldg(wbase + s_pair[i + 3] * ldw4);
+                    word.x &= v0.x & v1.x & v2.x & v3.x; word.y &= v0.y & v1.y & v2.y & v3.y;
+                    word.z &= v0.z & v1.z & v2.z & v3.z; word.w &= v0.w & v1.w & v2.w & v3.w;
                 }
-                for (; i < ns; ++i) word &= __ldg(wbase + static_cast<int64_t>(s_pair[i]) * ldw);
+                for (; i < ns; ++i) {
+                    const uint4 v = __ldg(wbase + s_pair[i] * ldw4);
+                    word.x &= v.x; word.y &= v.y; word.z &= v.z; word.w &= v.w;
+                }
                 for (; i < npr; ++i) {                          // very long chromosomes: ids from global
                     const int64_t pr = static_cast<int64_t>(__ldg(&col_ids[b + i])) * cols + __ldg(&col_ids[b + i + 1]);
-                    word &= __ldg(wbase + pr * ldw);
+                    const uint4 v = __ldg(wbase + pr * ldw4);
+                    word.x &= v.x; word.y &= v.y; word.z &= v.z; word.w &= v.w;
                 }
             } else {
-                const int64_t left = rows - w * 32;
-                const unsigned int valid = left >= 32 ? 0xffffffffu : left <= 0 ? 0u : ((1u << left) - 1u);
-                if (L == 1 && missing_on && w < ldw)
-                    word = ~nanmask[static_cast<int64_t>(__ldg(&col_ids[b])) * ldw + w] & valid;
-                else
-                    word = valid;
+                unsigned int out[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const int64_t left = rows - (w + c) * 32;
+                    const unsigned int valid = left >= 32 ? 0xffffffffu : left <= 0 ? 0u : ((1u << left) - 1u);
+                    out[c] = (L == 1 && missing_on) ? ~nanmask[static_cast<int64_t>(__ldg(&col_ids[b])) * ldw + w + c] & valid : valid;
+                }
+                word = make_uint4(out[0], out[1], out[2], out[3]);
             }
         }
-        if (w < words32) masks32[static_cast<int64_t>(j) * words32 + w] = word;
+        uint32_t* dst = masks32 + static_cast<int64_t>(j) * words32 + w;
+        if (w + 3 < words32 && (words32 & 3) == 0) {
+            *reinterpret_cast<uint4*>(dst) = word;               // a mask row is 16-byte aligned only if words32 % 4 == 0
+        } else if (w < words32) {
+            dst[0] = word.x;
+            if (w + 1 < words32) dst[1] = word.y; else word.y = 0u;
+            if (w + 2 < words32) dst[2] = word.z; else word.z = 0u;
+            if (w + 3 < words32) dst[3] = word.w; else word.w = 0u;
+        }
+        local += __popc(word.x) + __popc(word.y) + __popc(word.z) + __popc(word.w);
+        }
         if (counts != nullptr) {                                 // warp -> block -> one global atomic per block
-            const unsigned int local = __reduce_add_sync(0xffffffffu, __popc(word));
+            local = __reduce_add_sync(0xffffffffu, local);
             if (lane == 0 && local) atomicAdd(&s_cnt, local);
             __syncthreads();
             if (tid == 0 && s_cnt) atomicAdd(&counts[j], static_cast<unsigned long long>(s_cnt));
