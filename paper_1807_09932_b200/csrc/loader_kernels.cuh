@@ -199,6 +199,7 @@ pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanma
     const bool do0 = a0 < cols, do1 = a1 < cols;
     const int32_t n_stage = (cols + kPairCB - 1) / kPairCB;
     stage(0, 0);
+    uint32_t pb_next = ~__ldg(nan_b);                            // "present" word of column b, fetched one column ahead
     for (int32_t s = 0; s < n_stage; ++s) {
         if (s + 1 < n_stage) {
             stage((s + 1) * kPairCB, (s + 1) & 1);
@@ -217,7 +218,8 @@ pairbits_kernel(const float* __restrict__ Mc, const uint32_t* __restrict__ nanma
                 vb[4 * q] = __uint_as_float(x.x); vb[4 * q + 1] = __uint_as_float(x.y);
                 vb[4 * q + 2] = __uint_as_float(x.z); vb[4 * q + 3] = __uint_as_float(x.w);
             }
-            const uint32_t pb = ~__ldg(nan_b);
+            const uint32_t pb = pb_next;
+            if (s * kPairCB + c + 1 < cols) pb_next = ~__ldg(nan_b + ldw);
             uint32_t w0, w1;
             pair_words(va0, va1, vb, w0, w1);
             w0 &= pa0 & pb;
