@@ -64,7 +64,7 @@ enum { EBIC_MISSING_OFF = 0, EBIC_MISSING_ON = 1 };
  *   missing_mode  EBIC_MISSING_OFF / EBIC_MISSING_ON.
  *   out           receives the context.
  * Transposes to column-major, builds the packed NaN bitmask and per-column non-missing counts and, when it
- * takes at most 8 GiB and half of the free device memory, the pair-relation table (cols^2 bits per padded row:
+ * takes at most 32 GiB and half of the free device memory, the pair-relation table (cols^2 bits per padded row:
  * bit r of pair (a,b) = M[r][b] >= M[r][a]); without the table and with cols <= 127, the
  * 8-bit rank tiles instead.
  * Synchronous: `matrix` may be freed on return.

@@ -32,7 +32,7 @@ using namespace ebic;
 
 namespace {
 
-constexpr int64_t kPairbitsAutoMaxBytes = 8ll << 30;   // ebic_create builds the pair table up to this size
+constexpr int64_t kPairbitsAutoMaxBytes = 32ll << 30;  // ebic_create builds the pair table up to this size (and half of the free memory)
 constexpr int kConsF32 = 31;   // consumer warps of the TILED_F32 kernel (+1 producer = 1024 threads)
 constexpr int kConsR8 = 15;    // consumer warps of the RANK8 kernel     (+1 producer =  512 threads)
 

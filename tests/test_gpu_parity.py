@@ -277,6 +277,24 @@ def test_pairtile_kernel(B, oracle_mod, rows, cols, n_ind, max_len):
                 eb.set_kernel(B.EBIC_KERNEL_PAIRTILE)
 
 
+def test_pair_table_beyond_8_gib(B, oracle_mod):
+    """A wide matrix whose pair table takes 9.2 GB (150,000 x 700: 490,000 bit columns of 18.8 KB): built by
+    ebic_create (cap: 32 GiB and half of the free memory), PAIRBITS and the pair-table extraction against the oracle --
+    the 64-bit offsets of a table larger than 2^32 bytes."""
+    m, off, ids = W.random_case(700, 150_000, 700, 60, (0, 24), 0.01, False, True)
+    st, want = oracle_mod.eval_fitness(m, ON, off, ids)
+    chosen = np.array([0, 7, 33, 59], dtype=np.int32)
+    _, wm, wc = oracle_mod.extract_rows(m, ON, off, ids, chosen)
+    with B.Ebic(m, ON) as eb:
+        assert eb.info(14) > 9_000_000_000 and eb.kernel == B.EBIC_KERNEL_PAIRBITS
+        for ee in (False, True):
+            eb.set_early_exit(ee)
+            assert (gpu_counts(eb, B, off, ids, B.EBIC_KERNEL_AUTO) == want).all(), ee
+        gm, gc = gpu_masks(eb, off, ids, chosen)
+        assert (gm == wm).all() and (gc == wc).all()
+        assert eb.status() == st
+
+
 def test_wide_matrix_falls_back(B, oracle_mod):
     """cols > 127: no rank tiles; cols so large that no float tile of all columns double-buffers: the column-union
     kernel.  The pair table still serves (PAIRBITS); without it AUTO falls back to TILED_F32 / UNION_F32."""
