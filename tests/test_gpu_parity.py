@@ -513,6 +513,30 @@ def test_ring_path_stress(B, oracle_mod):
         assert eb.status() == 0
 
 
+def test_pairtile_stress(B, oracle_mod):
+    """The same stand-in for PAIRTILE's shared-memory paths (tile buffer refilled by TMA behind a barrier, per-lane
+    counters, the hand-out cursor of alternating tile parity): 400 evaluations of freshly randomised populations --
+    1..700 individuals of 0..40 columns, duplicates allowed every third time -- on a matrix of 40 tiles with a ragged
+    last one (fewer tiles than SMs, so most CTAs own a fraction of a tile), every count compared with the oracle."""
+    import torch
+    rows, cols = 40_500, 24
+    m, _, _ = W.random_case(321, rows, cols, 1, (1, 1), 0.01, True, True)
+    rng = np.random.default_rng(77)
+    with B.Ebic(m, ON) as eb:
+        eb.set_kernel(B.EBIC_KERNEL_PAIRTILE)
+        for it in range(400):
+            n_ind = int(rng.integers(1, 701))
+            L = rng.integers(0, 41, n_ind)
+            chroms = [rng.permutation(cols)[:min(l, cols)] if it % 3 else rng.integers(0, cols, l) for l in L]
+            off, ids = csr(chroms)
+            got = eb.eval_fitness(dev(off), dev(ids))
+            st, want = oracle_mod.eval_fitness(m, ON, off, ids)
+            torch.cuda.synchronize()
+            got = got.cpu().numpy().view(np.uint64)
+            assert (got == want).all(), (it, n_ind, np.flatnonzero(got != want)[:10])
+        assert eb.status() == 0
+
+
 def test_probe_read_bandwidth(B):
     """Measurement utility: an L2-resident buffer streams faster than HBM; bad arguments are refused."""
     l2 = B.ebic_probe_read_bandwidth(48 << 20, 40)
