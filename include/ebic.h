@@ -31,7 +31,7 @@
  * Which passage defines which call: ebic_create / ebic_create_sentinel / ebic_read_delimited -- PAPER.md lines
  * 59-61 (the input matrix, its limits, its missing-value marker, its file format); ebic_eval_fitness -- PAPER.md
  * line 60 (row counting under >=) with the population limits of line 59; ebic_extract_rows -- PAPER.md line 62
- * (a bicluster is returned as rows + columns); ebic_eval_extract -- both, one GA generation; ebic_mask_words /
+ * (a bicluster is returned as rows + columns); ebic_eval_extract -- both, one GA generation; ebic_eval_fitness_noalloc -- line 60 again; ebic_mask_words /
  * ebic_status / ebic_strerror / ebic_destroy / ebic_free_host -- bookkeeping the paper does not describe
  * (BASELINE.json north_star (1)).
  */
@@ -53,7 +53,8 @@ enum {
     EBIC_ERR_CUDA = 3,        /* any other CUDA runtime error (no device, launch failure, ...)    */
     EBIC_ERR_BAD_COLUMN = 4,  /* a column id outside [0, cols) was found on the device            */
     EBIC_ERR_BAD_OFFSETS = 5, /* offsets[k] < 0, offsets[k+1] < offsets[k] or offsets[k+1] > n_ids */
-    EBIC_ERR_IO = 6           /* ebic_read_delimited: cannot open / not a delimited matrix / ragged line */
+    EBIC_ERR_IO = 6,          /* ebic_read_delimited: cannot open / not a delimited matrix / ragged line */
+    EBIC_ERR_LIMIT = 7        /* ebic_eval_fitness_noalloc: population larger than the fixed scratch holds */
 };
 enum { EBIC_MISSING_OFF = 0, EBIC_MISSING_ON = 1 };
 
@@ -136,6 +137,42 @@ int ebic_extract_rows(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_
 int ebic_eval_extract(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_ids, int32_t n_ind,
                       int64_t n_ids, uint64_t *counts, const int32_t *chosen, int32_t n_chosen,
                       uint64_t *masks, uint64_t *mask_counts, void *cuda_stream);
+
+/*
+ * ebic_eval_fitness for callers that must not allocate device memory once their set-up is over.
+ *
+ * Who that is.  ebic_eval_fitness keeps per-call scratch (one validated record per individual) in buffers it
+ * grows with cudaFree + cudaMalloc whenever a population is larger than any it has seen.  Some hosts cannot live
+ * with that in their generation loop: a service whose own pool has taken the rest of the HBM after start-up (the
+ * cudaMalloc then fails in the middle of a run, hours in), a loop that shares the GPU with latency-bound streams
+ * (cudaFree waits for the whole device, cudaMalloc may too), and embedders whose rules simply forbid driver
+ * allocations after initialisation.  For them this call computes the same count[k] (same
+ * definition, same validation, same sticky errors as ebic_eval_fitness) and makes no cudaMalloc, cudaFree or
+ * other allocating call: its scratch is a fixed array compiled into libebic.so.
+ *
+ * The price of that array.
+ *   - It is EBIC_NOALLOC_MAX_IND * 136 bytes = 2,176 KiB, and every GPU on which the process loads the library
+ *     holds it until the process exits, used or not.
+ *   - n_ind > EBIC_NOALLOC_MAX_IND is refused with EBIC_ERR_LIMIT before anything is launched (`counts`
+ *     untouched); use ebic_eval_fitness for such populations.
+ *   - There is ONE array per GPU, shared by every context and every call on that GPU.  It still holds the
+ *     previous call's records on entry; the call needs none of them zeroed, because its first kernel rewrites
+ *     every record of 0 .. n_ind-1 before its second kernel reads exactly those.  Two calls that may run at the
+ *     same time on one GPU (different streams, different contexts, different host threads) race on it and return
+ *     garbage: issue them on one stream, or order the streams yourself.  Calls on one stream are safe back to
+ *     back.  ebic_eval_fitness and the other calls do not touch the array.
+ *   - The first call on each GPU looks up the array's device address (cudaGetSymbolAddress, once, under a lock)
+ *     before it launches.  Make that first call during set-up, outside any stream capture.
+ *
+ * Arguments as in ebic_eval_fitness, except that offsets, col_ids and counts must ALL be device pointers (a host
+ * buffer would need a staging allocation: EBIC_ERR_ARG).  Always asynchronous and stream-ordered on `cuda_stream`.
+ * The context is the one ebic_create made during set-up (ebic_create does allocate); it runs PAIRBITS when the
+ * context holds the pair table and DIRECT otherwise, whatever ebic_set_kernel says, with the context's early-exit
+ * setting; the context's own scratch and its captured launch graph are neither used nor disturbed.
+ */
+#define EBIC_NOALLOC_MAX_IND 16384
+int ebic_eval_fitness_noalloc(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_ids, int32_t n_ind,
+                              int64_t n_ids, uint64_t *counts, void *cuda_stream);
 
 /* ceil(rows / 64): uint64 words per mask.  -1 if ctx is NULL. */
 int64_t ebic_mask_words(const ebic_ctx *ctx);

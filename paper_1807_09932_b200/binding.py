@@ -24,6 +24,8 @@ EBIC_ERR_CUDA = 3
 EBIC_ERR_BAD_COLUMN = 4
 EBIC_ERR_BAD_OFFSETS = 5
 EBIC_ERR_IO = 6
+EBIC_ERR_LIMIT = 7
+EBIC_NOALLOC_MAX_IND = 16384
 EBIC_MISSING_OFF = 0
 EBIC_MISSING_ON = 1
 EBIC_KERNEL_AUTO = 0
@@ -50,6 +52,7 @@ SYMBOLS = {
     "ebic_create_sentinel": (ctypes.c_int, [_vp, _i64, _i32, _i32, ctypes.c_float, ctypes.POINTER(_vp)]),
     "ebic_destroy": (ctypes.c_int, [_vp]),
     "ebic_eval_fitness": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _vp]),
+    "ebic_eval_fitness_noalloc": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _vp]),
     "ebic_extract_rows": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _i32, _vp, _vp, _vp]),
     "ebic_eval_extract": (ctypes.c_int, [_vp, _vp, _vp, _i32, _i64, _vp, _vp, _i32, _vp, _vp, _vp]),
     "ebic_mask_words": (_i64, [_vp]),
@@ -132,6 +135,12 @@ def ebic_eval_fitness(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, counts_ptr, s
     st = load_library().ebic_eval_fitness(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, counts_ptr, stream)
     if st != EBIC_OK:
         raise EbicError(st, "ebic_eval_fitness")
+
+
+def ebic_eval_fitness_noalloc(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, counts_ptr, stream=0) -> None:
+    st = load_library().ebic_eval_fitness_noalloc(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, counts_ptr, stream)
+    if st != EBIC_OK:
+        raise EbicError(st, "ebic_eval_fitness_noalloc")
 
 
 def ebic_extract_rows(ctx, offsets_ptr, col_ids_ptr, n_ind, n_ids, chosen_ptr, n_chosen, masks_ptr,
@@ -373,6 +382,25 @@ class Ebic:
             counts = np.empty(n_ind, dtype=np.uint64)
         ebic_eval_fitness(self._ctx, _ptr(offsets), _ptr(col_ids), n_ind, n_ids, _ptr(counts),
                           _stream_handle(stream))
+        return counts
+
+    def eval_fitness_noalloc(self, offsets, col_ids, counts, stream=None):
+        """ebic_eval_fitness_noalloc: the same counts as eval_fitness, from a call that allocates no device memory.
+
+        For GA loops inside a host that has handed the rest of the HBM to its own pool, or that must not stall the
+        device with cudaFree / cudaMalloc once it is running (see include/ebic.h).  All three arguments are CUDA
+        tensors the caller made during set-up -- `counts` (int64 [n_ind]) included, the wrapper allocates nothing
+        either.  At most EBIC_NOALLOC_MAX_IND individuals (EbicError with status EBIC_ERR_LIMIT beyond that); every
+        call on a GPU shares one fixed scratch array, so keep such calls on one stream.  Returns `counts`.
+        """
+        if counts is None or not (_is_cuda(offsets) and _is_cuda(col_ids) and _is_cuda(counts)):
+            raise ValueError("eval_fitness_noalloc: offsets, col_ids and counts must be CUDA tensors supplied by the caller")
+        _check_args("eval_fitness_noalloc", self.device_index, {"offsets": offsets, "col_ids": col_ids}, {"counts": counts})
+        n_ind = int(offsets.shape[0]) - 1
+        if int(counts.shape[0]) < n_ind:
+            raise ValueError("eval_fitness_noalloc: `counts` is shorter than the population")
+        ebic_eval_fitness_noalloc(self._ctx, _ptr(offsets), _ptr(col_ids), n_ind, int(col_ids.shape[0]), _ptr(counts),
+                                  _stream_handle(stream))
         return counts
 
     def extract_rows(self, offsets, col_ids, chosen, masks=None, counts=None, want_counts=True, stream=None):

@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "ebic_ctx.hpp"
@@ -640,6 +641,47 @@ int stage_in(ebic_ctx* ctx, int slot, const void* host, int64_t bytes, cudaStrea
 
 }  // namespace
 
+// ------------------------------------------------------------------------------------------------
+// ebic_eval_fitness_noalloc (include/ebic.h): the count of every individual, for hosts that may not allocate device
+// memory after set-up.  The ingest kernel's products -- meta[k] (8 bytes) and, with the pair table, the 128-byte
+// record prec[j] of every individual -- go into a fixed array that is part of the library image instead of the
+// context's grown buffers.  Layout: [0, 8 * MAX) meta, [8 * MAX, 136 * MAX) prec; MAX = EBIC_NOALLOC_MAX_IND.
+//
+// `noalloc_scratch` below is a __device__ variable.  In HOST code that name is only the handle the runtime
+// registered for it; it is not an address the GPU can use.  The device address differs per GPU and is asked for
+// once per GPU with cudaGetSymbolAddress while that GPU is current (noalloc_scratch_for), and only that pointer is
+// ever handed to a kernel.
+// ------------------------------------------------------------------------------------------------
+constexpr int64_t kNoAllocMetaBytes = 8ll * EBIC_NOALLOC_MAX_IND;
+constexpr int64_t kNoAllocPrecBytes = 128ll * EBIC_NOALLOC_MAX_IND;
+constexpr int kNoAllocMaxDevices = 64;
+
+static __device__ __align__(256) unsigned char noalloc_scratch[kNoAllocMetaBytes + kNoAllocPrecBytes];
+
+namespace {
+
+std::mutex noalloc_mutex;
+unsigned char* noalloc_addr[kNoAllocMaxDevices] = {};     // device address of noalloc_scratch on GPU i, nullptr = not asked yet
+
+// Device address of the array on `device`, which must be the current device.  The first call per GPU asks the runtime.
+int noalloc_scratch_for(int device, unsigned char** out) {
+    if (device < 0 || device >= kNoAllocMaxDevices) return EBIC_ERR_ARG;
+    std::lock_guard<std::mutex> lock(noalloc_mutex);
+    if (!noalloc_addr[device]) {
+        void* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, noalloc_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return EBIC_ERR_CUDA;
+        }
+        noalloc_addr[device] = static_cast<unsigned char*>(p);
+    }
+    *out = noalloc_addr[device];
+    return EBIC_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 static int create_impl(const float* matrix, int64_t rows, int32_t cols, int32_t missing_mode, int32_t use_sentinel,
@@ -949,6 +991,75 @@ int ebic_eval_extract(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_
                              n_ind > 0, n_chosen > 0);
 }
 
+int ebic_eval_fitness_noalloc(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, int32_t n_ind, int64_t n_ids,
+                              uint64_t* counts, void* cuda_stream) {
+    if (!ctx || n_ind < 0 || n_ids < 0) return EBIC_ERR_ARG;
+    if (n_ind > EBIC_NOALLOC_MAX_IND) return EBIC_ERR_LIMIT;         // the fixed array holds no more records than that
+    if (n_ind == 0) return EBIC_OK;
+    if (!offsets || !counts || (!col_ids && n_ids > 0)) return EBIC_ERR_ARG;
+    if (!on_ctx_device(ctx)) return EBIC_ERR_ARG;
+    // host buffers would have to be staged through device memory this call is not allowed to allocate
+    if (!is_device_pointer(offsets) || !is_device_pointer(counts) || (n_ids > 0 && !is_device_pointer(col_ids))) return EBIC_ERR_ARG;
+    unsigned char* scratch = nullptr;
+    int st = noalloc_scratch_for(ctx->device, &scratch);
+    if (st) return st;
+    int2* meta = reinterpret_cast<int2*>(scratch);
+    uint32_t* prec = reinterpret_cast<uint32_t*>(scratch + kNoAllocMetaBytes);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    unsigned long long* d_counts = reinterpret_cast<unsigned long long*>(counts);
+    const bool by_pairs = ctx->PB != nullptr;
+
+    // a3: validation + records, into the fixed array.  Every meta[k] and every record of 0 .. n_ind-1 is rewritten here,
+    // so whatever the previous call left behind is never read; nothing has to be cleared.
+    IngestParams ip;
+    ip.offsets = offsets;
+    ip.col_ids = col_ids;
+    ip.n_ind = n_ind;
+    ip.n_ids = n_ids;
+    ip.cols = ctx->cols;
+    ip.rows = ctx->rows;
+    ip.missing_on = ctx->missing_mode == EBIC_MISSING_ON;
+    ip.sort_by_length = ctx->pb_sort;
+    ip.nonmissing = ctx->nonmissing;
+    ip.meta = meta;
+    ip.idrec = nullptr;
+    ip.id_wide = 0;
+    ip.prec = by_pairs ? prec : nullptr;
+    ip.pair_stride16 = static_cast<uint32_t>(ctx->ld / 128);
+    ip.counts = d_counts;
+    ip.err = ctx->d_err;
+    ingest_population_kernel<<<(n_ind + kIngestBlock - 1) / kIngestBlock, kIngestThreads, 0, stream>>>(ip);
+    ctx->launches++;
+    EBIC_TRY(cudaGetLastError());
+
+    const bool pdl = ctx->pdl != 0;
+    ctx->launches++;
+    if (by_pairs) {
+        PairbitsParams p = pairbits_params(ctx, col_ids, n_ind, n_ids, d_counts);
+        p.prec = prec;                                               // the fixed array, not the context's buffers
+        p.meta = meta;
+        if (p.n_chunks > 65535) return EBIC_ERR_ARG;
+        const dim3 g(static_cast<unsigned>((n_ind + kPairbitsWarps - 1) / kPairbitsWarps), static_cast<unsigned>(p.n_chunks));
+        const dim3 b(kPairbitsWarps * 32);
+        cudaError_t e;
+        if (ctx->pb_smem_ring) {
+            const size_t smem = kPairbitsWarps * 4096;
+            e = ctx->early_exit ? launch_pdl(fitness_pairbits_kernel<true, true>, g, b, smem, stream, pdl, p)
+                                : launch_pdl(fitness_pairbits_kernel<false, true>, g, b, smem, stream, pdl, p);
+        } else {
+            e = ctx->early_exit ? launch_pdl(fitness_pairbits_kernel<true, false>, g, b, 0, stream, pdl, p)
+                                : launch_pdl(fitness_pairbits_kernel<false, false>, g, b, 0, stream, pdl, p);
+        }
+        return ebic_host::cuda_status(e);
+    }
+    const int64_t gx = ctx->ld / 256;
+    int64_t gy = std::max<int64_t>(1, (8ll * ctx->sm_count + gx - 1) / gx);
+    gy = std::min<int64_t>(std::min<int64_t>(gy, n_ind), 65535);
+    const dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>(gy));
+    return ebic_host::cuda_status(launch_pdl(fitness_direct_kernel, grid, dim3(256), 0, stream, pdl, ctx->Mc, ctx->ld,
+                                             static_cast<const int2*>(meta), col_ids, n_ind, d_counts));
+}
+
 int64_t ebic_mask_words(const ebic_ctx* ctx) { return ctx ? (ctx->rows + 63) / 64 : -1; }
 
 int ebic_status(ebic_ctx* ctx, void* cuda_stream) {
@@ -970,6 +1081,7 @@ const char* ebic_strerror(int status) {
         case EBIC_ERR_BAD_COLUMN: return "column id outside [0, cols) in the population";
         case EBIC_ERR_BAD_OFFSETS: return "bad population offsets or chosen index";
         case EBIC_ERR_IO: return "cannot read the file as a delimited matrix";
+        case EBIC_ERR_LIMIT: return "population larger than the fixed scratch of ebic_eval_fitness_noalloc (EBIC_NOALLOC_MAX_IND individuals)";
         default: return "unknown status";
     }
 }

@@ -30,7 +30,7 @@ def test_header_declares_the_boundary():
     nothing else: knobs, read-backs and probes live in include/ebic_debug.h."""
     names = _declared_functions()
     assert names == sorted(["ebic_create", "ebic_create_sentinel", "ebic_destroy", "ebic_eval_fitness",
-                            "ebic_extract_rows", "ebic_eval_extract", "ebic_mask_words", "ebic_status",
+                            "ebic_eval_fitness_noalloc", "ebic_extract_rows", "ebic_eval_extract", "ebic_mask_words", "ebic_status",
                             "ebic_strerror", "ebic_read_delimited", "ebic_free_host"])
     debug = _declared_functions("ebic_debug.h")
     assert not set(names) & set(debug)
