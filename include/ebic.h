@@ -126,7 +126,10 @@ int ebic_extract_rows(ebic_ctx *ctx, const int32_t *offsets, const int32_t *col_
  * the population uploaded once (host pointers) and one stream synchronisation; with device outputs the extraction
  * kernel is chained behind the fitness kernel with programmatic dependent launch and runs alongside its last
  * wave; with host outputs the masks -- which do not depend on the counts -- are extracted first and copied back on
- * a stream the context owns while the fitness kernel runs (everything has completed when the call returns).
+ * a stream the context owns while the fitness kernel runs (everything has completed when the call returns, also when
+ * it returns an error: no copy into `masks` is left in flight).  That overlap needs PINNED host outputs
+ * (cudaHostAlloc / cudaHostRegister): into pageable memory the runtime copies through its own staging buffer and keeps
+ * the calling thread until the copy is done, so the fitness kernel is launched after it -- same results, no overlap.
  * Repetition: a GA loop passes the same device buffers every generation.  When a call with device pointers on a
  * non-default stream repeats the previous call's arguments exactly (pointers, sizes, stream), the library captures
  * its launch sequence into a CUDA graph and replays that graph from then on -- the results are those of the plain

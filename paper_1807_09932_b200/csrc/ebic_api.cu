@@ -52,6 +52,14 @@ int dev_alloc(ebic_ctx* ctx, void** p, int64_t bytes) {
 
 int grow(ebic_ctx* ctx, void** p, int64_t* cap, int64_t bytes) {
     if (bytes <= *cap) return EBIC_OK;
+    // A captured launch sequence (eval_extract_impl) has the addresses of the scratch buffers baked in.  Whatever call
+    // makes one of them move -- typically one that is not replayed itself: host pointers, the default stream, a larger
+    // population -- takes the graph with it; the next matching call starts over with a plain launch.
+    if (ctx->graph_exec) {
+        cudaGraphExecDestroy(ctx->graph_exec);
+        ctx->graph_exec = nullptr;
+        ctx->graph_state = 0;
+    }
     if (*p) {
         cudaError_t e = cudaFree(*p);      // synchronises: earlier work using the buffer has finished
         if (e != cudaSuccess) return ebic_host::cuda_status(e);
@@ -942,21 +950,36 @@ static int eval_extract_impl(ebic_ctx* ctx, const int32_t* offsets, const int32_
         EBIC_TRY(cudaEventRecord(ctx->ev_masks_ready, stream));
         EBIC_TRY(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_masks_ready, 0));
         EBIC_TRY(cudaMemcpyAsync(masks, d_masks, static_cast<size_t>(n_chosen) * words * 8, cudaMemcpyDeviceToHost, ctx->copy_stream));
-        if (mask_counts) EBIC_TRY(cudaMemcpyAsync(mask_counts, d_mcnt, static_cast<size_t>(n_chosen) * 8, cudaMemcpyDeviceToHost, ctx->copy_stream));
-        EBIC_TRY(cudaEventRecord(ctx->ev_masks_copied, ctx->copy_stream));
+        cudaError_t e = cudaSuccess;
+        if (mask_counts) e = cudaMemcpyAsync(mask_counts, d_mcnt, static_cast<size_t>(n_chosen) * 8, cudaMemcpyDeviceToHost, ctx->copy_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(ctx->ev_masks_copied, ctx->copy_stream);
+        if (e != cudaSuccess) {                                 // the first copy is already queued: wait it out
+            cudaStreamSynchronize(ctx->copy_stream);
+            return ebic_host::cuda_status(e);
+        }
     }
-    if (do_eval && (st = eval_device(ctx, d_off, d_ids, n_ind, n_ids, d_counts, stream))) return st;
+    // From here on a copy into the caller's `masks` may be in flight on the copy stream: an error return must not
+    // hand the buffer back while it is still being written, so every exit below drains that stream first.
+    auto leave = [&](int status) {
+        if (status != EBIC_OK && masks_first) {
+            cudaStreamSynchronize(ctx->copy_stream);
+            cudaGetLastError();
+        }
+        return status;
+    };
+    if (do_eval && (st = eval_device(ctx, d_off, d_ids, n_ind, n_ids, d_counts, stream))) return leave(st);
     if (do_extract && !masks_first &&
         (st = extract_device(ctx, d_off, d_ids, n_ind, n_ids, d_chosen, n_chosen, d_masks, d_mcnt, stream, fused)))
         return st;
+    auto ok = [&](cudaError_t e) { return (st = ebic_host::cuda_status(e)) == EBIC_OK; };
     if (!out_dev) {
-        if (do_eval) EBIC_TRY(cudaMemcpyAsync(counts, d_counts, static_cast<size_t>(n_ind) * 8, cudaMemcpyDeviceToHost, stream));
+        if (do_eval && !ok(cudaMemcpyAsync(counts, d_counts, static_cast<size_t>(n_ind) * 8, cudaMemcpyDeviceToHost, stream))) return leave(st);
         if (do_extract && !masks_first) {
             EBIC_TRY(cudaMemcpyAsync(masks, d_masks, static_cast<size_t>(n_chosen) * words * 8, cudaMemcpyDeviceToHost, stream));
             if (mask_counts) EBIC_TRY(cudaMemcpyAsync(mask_counts, d_mcnt, static_cast<size_t>(n_chosen) * 8, cudaMemcpyDeviceToHost, stream));
         }
-        if (masks_first) EBIC_TRY(cudaStreamWaitEvent(stream, ctx->ev_masks_copied, 0));
-        EBIC_TRY(cudaStreamSynchronize(stream));
+        if (masks_first && !ok(cudaStreamWaitEvent(stream, ctx->ev_masks_copied, 0))) return leave(st);
+        if (!ok(cudaStreamSynchronize(stream))) return leave(st);
     } else if (!pop_dev) {
         EBIC_TRY(cudaStreamSynchronize(stream));   // host population buffers may be reused on return
     }

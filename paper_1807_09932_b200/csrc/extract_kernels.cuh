@@ -137,6 +137,9 @@ extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_
     const int64_t ldw = ld / 32;                                           // a multiple of 32: 16-byte units never straddle
     const int64_t ldw4 = ldw >> 2;
     const int64_t n_wblocks = (words32 + 1023) / 1024;                     // blocks of 1,024 mask words, strided over grid.x
+    // 16-byte stores need every mask row 16-byte aligned: a row length that is a multiple of four words AND a
+    // 16-byte-aligned base (include/ebic.h only promises uint64 alignment: the caller may pass an offset view)
+    const bool vec_store = (words32 & 3) == 0 && (reinterpret_cast<uintptr_t>(masks32) & 15) == 0;
 
     for (int32_t j = blockIdx.y; j < n_chosen; j += gridDim.y) {
         if (tid == 0) {
@@ -207,8 +210,8 @@ extract_rows_pairbits_kernel(const uint32_t* __restrict__ PB, int64_t ld, int64_
             }
         }
         uint32_t* dst = masks32 + static_cast<int64_t>(j) * words32 + w;
-        if (w + 3 < words32 && (words32 & 3) == 0) {
-            *reinterpret_cast<uint4*>(dst) = word;               // a mask row is 16-byte aligned only if words32 % 4 == 0
+        if (w + 3 < words32 && vec_store) {
+            *reinterpret_cast<uint4*>(dst) = word;
         } else if (w < words32) {
             dst[0] = word.x;
             if (w + 1 < words32) dst[1] = word.y; else word.y = 0u;

@@ -119,14 +119,31 @@ class ShardedEbic:
 
     def step(self, offsets, col_ids, chosen):
         """One generation: (whole-matrix counts on every rank, this rank's mask shard).  On the CUDA path the
-        local half is one `ebic_eval_extract` call."""
+        local half is one `ebic_eval_extract` call into tensors that are reused every generation (copy what must
+        outlive the next `step`)."""
         import torch.distributed as dist
         if self.ebic is None:
             return self.eval_fitness(offsets, col_ids), self.extract_rows(offsets, col_ids, chosen)
-        counts, masks, _ = self.ebic.eval_extract(offsets, col_ids, chosen, want_counts=False)
+        counts, masks = self._step_buffers(int(offsets.shape[0]) - 1, int(chosen.shape[0]), offsets)
+        self.ebic.eval_extract(offsets, col_ids, chosen, counts=counts, masks=masks, want_counts=False)
         if self.world_size > 1:
             dist.all_reduce(counts, op=dist.ReduceOp.SUM, group=self._group)
         return counts, masks
+
+    def _step_buffers(self, n_ind: int, n_chosen: int, like):
+        """The output tensors `step` hands to the library and to the all-reduce, made once per (population size,
+        number chosen) and reused every generation: with the same pointers in every call the library's captured
+        launch graph stays valid (include/ebic.h, ebic_eval_extract) instead of depending on the caching allocator
+        returning the same addresses.  The tensors `step` returns are therefore overwritten by the next `step`."""
+        import torch
+        if not getattr(like, "is_cuda", False):                    # host arrays: the binding makes numpy outputs
+            return None, None
+        key = (n_ind, n_chosen)
+        if getattr(self, "_step_key", None) != key:
+            self._step_out = (torch.empty(n_ind, dtype=torch.int64, device=like.device),
+                              torch.empty((n_chosen, self.ebic.mask_words), dtype=torch.int64, device=like.device))
+            self._step_key = key
+        return self._step_out
 
     def gather_masks(self, local_masks):
         """Concatenate every rank's mask shard along the word axis (all ranks get the whole mask): ONE

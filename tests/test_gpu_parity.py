@@ -757,6 +757,72 @@ def test_repeated_calls_replay_a_graph(B, oracle_mod):
         assert eb.status() == 0
 
 
+def test_graph_survives_scratch_reallocation(B, oracle_mod):
+    """A captured launch graph holds the addresses of the context's scratch.  A call that cannot be replayed (host
+    pointers) with a population four times as large makes the library reallocate that scratch between two replays:
+    the graph must be dropped with it, not replayed on freed memory.  Every kernel, against the oracle."""
+    import torch
+    rows, cols, n_ind = 30_001, 24, 500
+    m, off, ids = W.random_case(322, rows, cols, n_ind, (0, 12), 0.02, False, True)
+    st, want = oracle_mod.eval_fitness(m, ON, off, ids)
+    assert st == 0
+    side = torch.cuda.Stream()
+    with B.Ebic(m, ON) as eb:
+        d_off, d_ids = dev(off), dev(ids)
+        counts = torch.empty(n_ind, dtype=torch.int64, device="cuda")
+        for i, kern in enumerate(kernels_for(eb, B)):
+            eb.set_kernel(kern)                                        # new epoch: the graph logic starts over
+            for _ in range(3):
+                with torch.cuda.stream(side):
+                    eb.eval_fitness(d_off, d_ids, counts=counts, stream=side)
+                side.synchronize()
+            assert eb.info(18) > 0, B.KERNEL_NAMES[kern]               # a graph is held
+            owned = eb.info(9)
+            # host pointers and a population twice as large as any before it (the buffers are grown with 25 % headroom,
+            # so doubling always outgrows them): scratch regrown
+            _, off4, ids4 = W.random_case(323 + i, 1, cols, 2 * n_ind << i, (0, 12))
+            st4, want4 = oracle_mod.eval_fitness(m, ON, off4, ids4)
+            assert st4 == 0 and (eb.eval_fitness(off4, ids4) == want4).all()
+            assert eb.info(9) > owned
+            assert eb.info(18) == 0, B.KERNEL_NAMES[kern]              # ... and the graph went with it
+            # memory the old scratch occupied may be handed to somebody else: make it so
+            junk = [torch.full((1 << 16,), -1, dtype=torch.int64, device="cuda") for _ in range(8)]
+            for rep in range(4):
+                counts.fill_(-1)
+                side.wait_stream(torch.cuda.current_stream())
+                with torch.cuda.stream(side):
+                    eb.eval_fitness(d_off, d_ids, counts=counts, stream=side)
+                side.synchronize()
+                assert (counts.cpu().numpy().view(np.uint64) == want).all(), (B.KERNEL_NAMES[kern], rep)
+            assert eb.info(18) > 0                                     # captured again on the new buffers
+            assert all(bool((j == -1).all()) for j in junk)
+        assert eb.status() == 0
+
+
+def test_extract_into_an_offset_view(B, oracle_mod):
+    """include/ebic.h promises uint64 alignment for `masks`, no more: a view that starts 8 bytes into an allocation
+    (rows chosen so that a mask is a multiple of 16 bytes long, the case the 16-byte stores serve) must work."""
+    import torch
+    rows = 128 * 77                                                    # 154 uint64 words per mask: even
+    m, off, ids = W.random_case(324, rows, 12, 40, (0, 8), 0.03)
+    chosen = np.arange(40, dtype=np.int32)
+    st, wm, wc = oracle_mod.extract_rows(m, ON, off, ids, chosen)
+    with B.Ebic(m, ON) as eb:
+        assert eb.mask_words % 2 == 0
+        for use_pairbits in (True, False):
+            eb.set_extract_source(use_pairbits)
+            for shift in (1, 2, 3):
+                buf = torch.zeros(40 * eb.mask_words + shift, dtype=torch.int64, device="cuda")
+                masks = buf[shift:].view(40, eb.mask_words)
+                assert masks.data_ptr() == buf.data_ptr() + 8 * shift
+                gm, gc = eb.extract_rows(dev(off), dev(ids), dev(chosen), masks=masks)
+                torch.cuda.synchronize()
+                assert (gm.cpu().numpy().view(np.uint64) == wm).all(), (use_pairbits, shift)
+                assert (gc.cpu().numpy().view(np.uint64) == wc).all()
+                assert (buf[:shift] == 0).all()
+        assert eb.status() == st == 0
+
+
 def test_binding_refuses_wrong_dtypes(B):
     """The C ABI takes raw addresses: the binding must refuse what would be read as garbage (advisor finding)."""
     w = W.make_workload(0)
@@ -796,6 +862,38 @@ def test_row_shards_through_the_cuda_evaluator(B, oracle_mod, world):
             shard_counts += mc
     assert (total == want).all()
     assert (np.concatenate(shards, axis=1) == wm).all() and (shard_counts == wc).all()
+
+
+def test_sharded_step_reuses_its_outputs(B, oracle_mod):
+    """ShardedEbic.step hands the library the same output tensors every generation, so the captured launch graph is
+    replayed from the third generation on whatever the caching allocator does in between; results against the oracle."""
+    import torch
+    from paper_1807_09932_b200.sharded import ShardedEbic
+    w = W.make_workload(3, rows=20_011, n_ind=400)
+    chosen = np.array([0, 7, 399], dtype=np.int32)
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    _, wm, _ = oracle_mod.extract_rows(w.matrix, w.missing_mode, w.offsets, w.col_ids, chosen)
+    sh = ShardedEbic.from_matrix(w.matrix, w.missing_mode, 0, 1)
+    try:
+        d_off, d_ids, d_ch = dev(w.offsets), dev(w.col_ids), dev(chosen)
+        side = torch.cuda.Stream()
+        ptrs = set()
+        for gen in range(5):
+            churn = [torch.empty(1 << (10 + gen), dtype=torch.int64, device="cuda") for _ in range(4)]   # allocator noise
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                counts, masks = sh.step(d_off, d_ids, d_ch)
+            side.synchronize()
+            ptrs.add((counts.data_ptr(), masks.data_ptr()))
+            assert (counts.cpu().numpy().view(np.uint64) == want).all(), gen
+            assert (masks.cpu().numpy().view(np.uint64) == wm).all(), gen
+            if gen >= 2:
+                assert sh.ebic.info(18) > 0, gen                   # replayed
+            del churn
+        assert len(ptrs) == 1
+        assert sh.ebic.status(side) == 0
+    finally:
+        sh.close()
 
 
 # ------------------------------------------------------------------------- full sizes against the oracle
