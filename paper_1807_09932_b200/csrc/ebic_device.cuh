@@ -58,6 +58,12 @@ __device__ __forceinline__ void bulk_copy_g2s(void* smem_dst, const void* gmem_s
         : "memory");
 }
 
+// Orders this thread's earlier generic-proxy accesses to shared memory (plain LDS / STS, and those of other threads
+// it has synchronised with) before later async-proxy accesses (cp.async.bulk writes into the same bytes).
+__device__ __forceinline__ void fence_proxy_async_smem() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
 // L2 prefetch of `bytes` (multiple of 16) at a 16-byte aligned global address; no register or shared-memory
 // destination, no completion to wait for (SASS: UBLKPF).
 __device__ __forceinline__ void bulk_prefetch_l2(const void* gmem_src, uint32_t bytes) {
@@ -104,6 +110,14 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
 // CTAs be scheduled once every CTA of this grid has called it (or exited).  Both are no-ops for plain launches.
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// Load of something an EARLIER kernel on the stream wrote (meta, records, plans, batch lists).  With programmatic
+// dependent launch this kernel is already resident while that kernel writes, and the same addresses are rewritten
+// every generation; PTX allows the read-only path (ld.global.nc, __ldg) only for data nobody writes during the
+// reading kernel's lifetime.  So: a plain load served by L2 (ld.global.cg), issued after griddep_wait().  __ldg stays
+// for what really is immutable while a kernel runs: the matrix, the pair table, the caller's population.
+template <class T>
+__device__ __forceinline__ T ld_produced(const T* p) { return __ldcg(p); }
 
 __device__ __forceinline__ bool is_nan_bits(float v) {
     return (__float_as_uint(v) & 0x7fffffffu) > 0x7f800000u;

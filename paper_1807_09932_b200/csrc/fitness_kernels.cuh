@@ -16,7 +16,7 @@ namespace ebic {
 // grid.x = ld / 256 row blocks, grid.y = population slices.
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-fitness_direct_kernel(const float* __restrict__ Mc, int64_t ld, const int2* __restrict__ meta,
+fitness_direct_kernel(const float* __restrict__ Mc, int64_t ld, const int2* meta,
                       const int32_t* __restrict__ col_ids, int32_t n_ind,
                       unsigned long long* __restrict__ counts)
 {
@@ -27,7 +27,7 @@ fitness_direct_kernel(const float* __restrict__ Mc, int64_t ld, const int2* __re
     const int32_t k_begin = blockIdx.y * per;
     const int32_t k_end = min(n_ind, k_begin + per);
     for (int32_t k = k_begin; k < k_end; ++k) {
-        const int2 m = __ldg(&meta[k]);
+        const int2 m = ld_produced(&meta[k]);
         if (m.y < 2) continue;
         const int32_t* ids = col_ids + m.x;                      // validated by the ingest: every id inside [0, cols)
         float prev = Mc[static_cast<int64_t>(__ldg(&ids[0])) * ld + r];
@@ -174,14 +174,14 @@ struct IdWords {
     static constexpr int kPerWord = 4;
     const uint32_t* rec;             // idrec + 8 * k
     const int32_t* ids;              // col_ids + b
-    __device__ __forceinline__ uint32_t word(int32_t j) const { return __ldg(rec + j); }
+    __device__ __forceinline__ uint32_t word(int32_t j) const { return ld_produced(rec + j); }
     __device__ __forceinline__ uint32_t tail_id(int32_t i) const { return static_cast<uint32_t>(__ldg(ids + i)); }
 };
 struct IdWords16 {
     static constexpr int kPerWord = 2;
     const uint32_t* rec;             // idrec + 16 * k
     const int32_t* ids;
-    __device__ __forceinline__ uint32_t word(int32_t j) const { return __ldg(rec + j); }
+    __device__ __forceinline__ uint32_t word(int32_t j) const { return ld_produced(rec + j); }
     __device__ __forceinline__ uint32_t tail_id(int32_t i) const { return static_cast<uint32_t>(__ldg(ids + i)); }
 };
 // An id record that has been staged in shared memory (UNION_F32: admitted individuals have L <= 32, no tail).
@@ -394,16 +394,16 @@ fitness_tiled_kernel(const TiledParams p)
             int2 m_cur = make_int2(0, 0);
             uint32_t w_cur = 0;
             if (k < kb) {
-                m_cur = __ldg(&p.meta[k]);
-                w_cur = __ldg(p.idrec + static_cast<int64_t>(kRecWords) * k);
+                m_cur = ld_produced(&p.meta[k]);
+                w_cur = ld_produced(p.idrec + static_cast<int64_t>(kRecWords) * k);
             }
             mbar_wait(&full[buf], (j / p.nbuf) & 1);
             for (; k < kb; k += NCONS) {
                 const int2 m = m_cur;
                 const uint32_t w0 = w_cur;
                 if (k + NCONS < kb) {
-                    m_cur = __ldg(&p.meta[k + NCONS]);
-                    w_cur = __ldg(p.idrec + static_cast<int64_t>(kRecWords) * (k + NCONS));
+                    m_cur = ld_produced(&p.meta[k + NCONS]);
+                    w_cur = ld_produced(p.idrec + static_cast<int64_t>(kRecWords) * (k + NCONS));
                 }
                 if (m.y < 2) continue;
                 const IW iw{p.idrec + static_cast<int64_t>(kRecWords) * k, p.col_ids + m.x};

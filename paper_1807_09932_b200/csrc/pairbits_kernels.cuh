@@ -84,8 +84,12 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
             }
             done += 8;
             // Ring reuse: the next round's LDGSTS must not be issued before this round's LDS data has arrived.
-            // `ring` is made to depend on all eight accumulator words (each holds the result of four of the LDS),
-            // so the in-order issue + scoreboard of the warp orders them; no instruction is emitted.
+            // Every lane reads and refills only its OWN 16-byte cells, so this is a same-thread, same-address
+            // read-then-write in program order; __syncwarp() states it as a memory-ordering point the compiler
+            // and the hardware must both honour, and `ring` is additionally made to depend on all eight
+            // accumulator words (each holds the result of four of the LDS) so that the address of the next
+            // LDGSTS does not exist before the loads have returned.
+            __syncwarp();
             asm volatile("" : "+r"(ring) : "r"(acc_a.x), "r"(acc_a.y), "r"(acc_a.z), "r"(acc_a.w),
                                            "r"(acc_b.x), "r"(acc_b.y), "r"(acc_b.z), "r"(acc_b.w) : "memory");
             if (EARLY_EXIT && !__any_sync(0xffffffffu, any4(acc_a) || any4(acc_b))) return done;
@@ -126,7 +130,7 @@ __device__ __forceinline__ int32_t pairbits_step(const uint4* __restrict__ base_
         // pair offsets beyond the 30 a record holds are formed from the caller's ids (a VALID individual: every
         // id is inside [0, cols)); pair q = (id_q, id_{q+1}), q + 1 <= L - 1
         const int32_t n = min(32, npr - seg);
-        const int32_t* ids = p.col_ids + __ldg(&p.meta[k]).x + seg + min(lane, n - 1);
+        const int32_t* ids = p.col_ids + ld_produced(&p.meta[k]).x + seg + min(lane, n - 1);
         const uint32_t mine = (static_cast<uint32_t>(__ldg(ids)) * static_cast<uint32_t>(p.cols) +
                                static_cast<uint32_t>(__ldg(ids + 1))) * p.pair_stride16;
         for (int32_t j = 0; j < n; ++j) {
@@ -222,7 +226,7 @@ fitness_pairbits_kernel(const PairbitsParams p)
     griddep_wait();
     const int32_t j = blockIdx.x * kPairbitsWarps + warp;
     if (j >= p.n_ind) return;
-    const uint32_t rec = __ldg(p.prec + 32ll * j + lane);        // one coalesced 128 B load
+    const uint32_t rec = ld_produced(p.prec + 32ll * j + lane);        // one coalesced 128 B load
     unsigned long long executed = 0;
     pairbits_task<EARLY_EXIT, SMEM>(p, blockIdx.y, j, rec, lane, SMEM ? smem_u32(pb_ring) + warp * 4096 : 0u, executed);
     if (lane == 0 && p.visits != nullptr && executed) atomicAdd(p.visits, executed);

@@ -213,9 +213,9 @@ fitness_pairtile_kernel(const PairtileParams p)
     for (int32_t j = tid; j < p.n_groups * 32; j += kPtWarps * 32) counters[j] = 0;
     griddep_wait();                              // gmeta / tids (plan kernel), counts initialised (ingest kernel)
     for (int32_t grp = warp; grp < p.n_groups; grp += kPtWarps) {
-        const int32_t mx = __reduce_max_sync(0xffffffffu, __ldg(p.gmeta + grp * 32 + lane).y);
+        const int32_t mx = __reduce_max_sync(0xffffffffu, ld_produced(p.gmeta + grp * 32 + lane).y);
         if (lane == 0) s_gmax[grp] = mx;
-        if (p.rec_cache) s_ids0[grp * 32 + lane] = __ldg(p.tids + static_cast<int64_t>(grp) * 128 + lane);
+        if (p.rec_cache) s_ids0[grp * 32 + lane] = ld_produced(p.tids + static_cast<int64_t>(grp) * 128 + lane);
     }
     __syncthreads();
 
@@ -235,8 +235,8 @@ fitness_pairtile_kernel(const PairtileParams p)
         grp_req = (pos & 1) ? p.n_groups - 1 - (pos >> 1) : (pos >> 1);
         maxn = s_gmax[grp_req];
         const uint4* rec = p.tids + static_cast<int64_t>(grp_req) * 128 + lane;
-        ids0 = p.rec_cache ? s_ids0[grp_req * 32 + lane] : __ldg(rec);
-        if (maxn > 8) ids1 = __ldg(rec + 32);
+        ids0 = p.rec_cache ? s_ids0[grp_req * 32 + lane] : ld_produced(rec);
+        if (maxn > 8) ids1 = ld_produced(rec + 32);
     };
     if (c < (t_first == t_last ? static_cast<int32_t>(i1 - t_first * p.n_groups) : p.n_groups)) request(c);
     uint32_t phase = 0;
@@ -267,15 +267,15 @@ fitness_pairtile_kernel(const PairtileParams p)
                 if (m > 8) pairtile_chunk(acc, lanebase, cur1, m - 8);
                 if (m > 16) {
                     const uint4* rec = p.tids + static_cast<int64_t>(grp) * 128 + lane;
-                    const uint4 cur2 = __ldg(rec + 64), cur3 = __ldg(rec + 96);
+                    const uint4 cur2 = ld_produced(rec + 64), cur3 = ld_produced(rec + 96);
                     pairtile_chunk(acc, lanebase, cur2, m - 16);
                     if (m > 24) pairtile_chunk(acc, lanebase, cur3, m - 24);
                 }
                 if (maxn_cur > kPtRecIds || p.visits != nullptr) {       // rare: a very long chromosome, or instrumented
-                    const int2 gm = __ldg(p.gmeta + grp * 32 + lane);
+                    const int2 gm = ld_produced(p.gmeta + grp * 32 + lane);
                     if (gm.y > kPtRecIds) {
                         // pairs beyond the record come from the caller's ids (a VALID individual)
-                        const int32_t* ids_g = p.col_ids + __ldg(&p.meta[gm.x]).x;
+                        const int32_t* ids_g = p.col_ids + ld_produced(&p.meta[gm.x]).x;
                         int32_t a = __ldg(ids_g + kPtRecIds);
                         for (int32_t j = kPtRecIds; j < gm.y; ++j) {
                             const int32_t b = __ldg(ids_g + j + 1);
@@ -299,12 +299,15 @@ fitness_pairtile_kernel(const PairtileParams p)
             if (c < (t + 1 == t_last ? static_cast<int32_t>(i1 - t_last * p.n_groups) : p.n_groups)) request(c);
         }
         __syncthreads();                         // every warp is done with the tile (and with its counters)
-        if (t < t_last && tid == 0) stage(t + 1);
+        if (t < t_last && tid == 0) {
+            fence_proxy_async_smem();            // the warps' LDS (generic proxy) before the refill's bulk-copy writes (async proxy)
+            stage(t + 1);
+        }
     }
     // one 64-bit global atomic per (CTA, individual)
     for (int32_t j = tid; j < p.n_groups * 32; j += kPtWarps * 32) {
         const uint32_t cnt = counters[j];
-        const int2 gm = __ldg(p.gmeta + j);
+        const int2 gm = ld_produced(p.gmeta + j);
         if (cnt && gm.y >= 1) atomicAdd(&p.counts[gm.x], static_cast<unsigned long long>(cnt));
     }
     if (p.visits != nullptr) {

@@ -44,9 +44,9 @@ prefix_plan_kernel(const PrefixParams p, int32_t n_pow2)
     for (int32_t j = tid; j < n_pow2; j += 1024) {
         unsigned long long kk = ~0ull;
         if (j < n) {
-            const int32_t L = static_cast<int32_t>(__ldg(prec + 32ll * j));
+            const int32_t L = static_cast<int32_t>(ld_produced(prec + 32ll * j));
             if (L >= 2 && L <= 31)                   // groupable: the whole chromosome lives in the record
-                kk = (static_cast<unsigned long long>(__ldg(prec + 32ll * j + 2)) << 32) | __ldg(prec + 32ll * j + 3);
+                kk = (static_cast<unsigned long long>(ld_produced(prec + 32ll * j + 2)) << 32) | ld_produced(prec + 32ll * j + 3);
             else if (L >= 32)
                 kk = ~0ull - 1;                      // evaluated, never grouped
         }
@@ -124,11 +124,11 @@ prefix_plan_kernel(const PrefixParams p, int32_t n_pow2)
             // longest prefix (in pairs) common to all members: compare each member with member 0
             P = 30;
             const uint32_t* r0 = prec + 32ll * val[i];
-            for (int32_t m = 0; m < cnt; ++m) P = min(P, static_cast<int32_t>(__ldg(prec + 32ll * val[i + m])) - 1);
+            for (int32_t m = 0; m < cnt; ++m) P = min(P, static_cast<int32_t>(ld_produced(prec + 32ll * val[i + m])) - 1);
             for (int32_t m = 1; m < cnt; ++m) {
                 const uint32_t* rm = prec + 32ll * val[i + m];
                 int32_t q = 0;
-                while (q < P && __ldg(r0 + 2 + q) == __ldg(rm + 2 + q)) ++q;
+                while (q < P && ld_produced(r0 + 2 + q) == ld_produced(rm + 2 + q)) ++q;
                 P = q;
             }
         }
@@ -175,23 +175,23 @@ fitness_prefix_kernel(const PrefixParams pp)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     griddep_launch_dependents();
     griddep_wait();
-    const int64_t n_groups = __ldg(pp.n_groups);
+    const int64_t n_groups = ld_produced(pp.n_groups);
     const int64_t task = static_cast<int64_t>(blockIdx.x) * kPairbitsWarps + warp;
     if (task >= n_groups * p.n_chunks) return;
     const int64_t g_chunk = task / n_groups;
     const int32_t g = static_cast<int32_t>(task - g_chunk * n_groups);
     const int32_t* grp = pp.groups + 8ll * g;
-    const int32_t head = __ldg(grp);
+    const int32_t head = ld_produced(grp);
     const int32_t cnt = head & 0xff, P = head >> 8;
     unsigned long long executed = 0;
     if (cnt == 1) {                                              // not grouped: the plain task on this member's record
-        const int32_t j = __ldg(grp + 1);
-        const uint32_t rec = __ldg(p.prec + 32ll * j + lane);
+        const int32_t j = ld_produced(grp + 1);
+        const uint32_t rec = ld_produced(p.prec + 32ll * j + lane);
         pairbits_task<EARLY_EXIT, false>(p, g_chunk, j, rec, lane, 0u, executed);
     } else {
         uint32_t rec[kPrefixGroup];
 #pragma unroll
-        for (int m = 0; m < kPrefixGroup; ++m) rec[m] = __ldg(p.prec + 32ll * __ldg(grp + 1 + m) + lane);
+        for (int m = 0; m < kPrefixGroup; ++m) rec[m] = ld_produced(p.prec + 32ll * ld_produced(grp + 1 + m) + lane);
         const int64_t w_begin = g_chunk * p.chunk_words, w_end = min(p.ldw, w_begin + p.chunk_words);
         const uint4* PB4 = reinterpret_cast<const uint4*>(p.PB);
         unsigned int c[kPrefixGroup] = {0u, 0u, 0u, 0u};

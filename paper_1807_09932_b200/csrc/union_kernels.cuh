@@ -63,7 +63,7 @@ union_plan_kernel(const UnionParams p)
         // in population order: admit while the union fits.  Newly set bits are rolled back when it does not.
         int32_t u = 0;
         for (int32_t k = k0; k < k1; ++k) {
-            const int2 m = __ldg(&p.meta[k]);
+            const int2 m = ld_produced(&p.meta[k]);
             bool admit = m.y >= 2 && m.y <= 32;
             if (admit) {
                 const int32_t id = (lane < m.y) ? __ldg(p.col_ids + m.x + lane) : -1;
@@ -119,7 +119,7 @@ union_plan_kernel(const UnionParams p)
         uint32_t local = 0;
         const bool admit = s_admit[k - k0] != 0;
         if (admit) {
-            const int2 m = __ldg(&p.meta[k]);
+            const int2 m = ld_produced(&p.meta[k]);
             const int32_t id = __ldg(p.col_ids + m.x + min(lane, m.y - 1));          // padded with the last id
             local = prefix[id >> 5] + __popc(bitmap[id >> 5] & ((1u << (id & 31)) - 1u));
         }
@@ -198,7 +198,7 @@ fitness_union_kernel(const UnionParams p)
             const int buf = j & 1;
             const int64_t t = it / p.n_batches;
             const int32_t b = static_cast<int32_t>(it - t * p.n_batches);
-            const int32_t U = __ldg(&p.ucount[b]);
+            const int32_t U = ld_produced(&p.ucount[b]);
             const int32_t k0 = b * p.batch;
             const int32_t nb = min(p.n_ind, k0 + p.batch) - k0;
             mbar_wait(&empty[buf], ((j >> 1) & 1) ^ 1);          // passes immediately for j < 2
@@ -207,7 +207,7 @@ fitness_union_kernel(const UnionParams p)
             const uint32_t dst = smem_u32(buffer) + lane * 16;
             const float* src = p.Mc + t * kUnionTileRows + lane * 4;
             for (int32_t c0 = pw * 32; c0 < U; c0 += kUnionProd * 32) {
-                const int32_t mine = (c0 + lane < U) ? __ldg(ucols + c0 + lane) : 0;
+                const int32_t mine = (c0 + lane < U) ? ld_produced(ucols + c0 + lane) : 0;
                 const int32_t n = min(32, U - c0);
                 for (int32_t i = 0; i < n; ++i)
                     cp_async16(dst + (c0 + i) * (kUnionTileRows * 4), src + static_cast<int64_t>(__shfl_sync(0xffffffffu, mine, i)) * p.ld);
