@@ -50,7 +50,7 @@ UNIT = "comparisons/s"
 N_CHOSEN = 8
 WORKLOADS = {"c1": 0, "c2": 1, "c3": 2, "c4": 3, "c5": 4, "p1": 5, "p2": 6, "p3": 7}
 KERNELS = {"auto": 0, "direct": 1, "tiled_f32": 2, "rank8": 3, "pairbits": 4, "union_f32": 5, "prefix": 6, "pairtile": 7}
-TRAFFIC_CSV = ROOT / "profiles" / "r02_dram_traffic.csv"
+TRAFFIC_INDEX = ROOT / "profiles" / "r03_traffic_index.csv"     # workload,kernel,kernel_sha,raw_csv (see r03_traffic_index.md)
 KERNEL_SOURCES = ["pairbits_kernels.cuh", "pairtile_kernels.cuh", "fitness_kernels.cuh", "union_kernels.cuh", "ebic_device.cuh"]
 
 
@@ -128,7 +128,7 @@ def pick_chosen(w):
 
 
 def kernel_source_sha() -> str:
-    """Identifies the fitness kernels a committed ncu capture was taken on (profiles/r02_dram_traffic.csv)."""
+    """Identifies the fitness kernels a committed ncu capture was taken on (profiles/r03_traffic_index.csv)."""
     h = hashlib.sha256()
     for name in KERNEL_SOURCES:
         p = ROOT / "paper_1807_09932_b200" / "csrc" / name
@@ -137,20 +137,41 @@ def kernel_source_sha() -> str:
     return h.hexdigest()[:12]
 
 
+def ncu_raw_metric_sum(raw_csv: Path, kernel_substr: str, metrics):
+    """Sum of `metrics` for the LAST launch whose kernel name contains `kernel_substr`, from an
+    `ncu -i <rep> --page raw --csv --print-units base` export (row 1 = metric names, row 2 = units, then one row per
+    profiled launch).  None when the kernel or a metric is not in the file."""
+    with raw_csv.open(newline="") as f:
+        rows = list(csv.reader(f))
+    head = next((i for i, r in enumerate(rows) if "Kernel Name" in r), None)
+    if head is None:
+        return None
+    names = rows[head]
+    k_col = names.index("Kernel Name")
+    hits = [r for r in rows[head + 2:] if len(r) == len(names) and kernel_substr in r[k_col]]
+    if not hits or any(m not in names for m in metrics):
+        return None
+    return sum(float(hits[-1][names.index(m)].replace(",", "")) for m in metrics)
+
+
 def ncu_traffic(workload_key: str, kernel_name: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the fitness kernel from the committed
-    `ncu --set full` captures (profiles/r02_dram_traffic.csv, written by hand from the .txt summaries it names).
-    None -- with the reason -- when there is no capture for this workload / kernel or when the kernels have
-    changed since the capture was taken."""
-    if not TRAFFIC_CSV.exists():
-        return None, "no profiles/r02_dram_traffic.csv"
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the fitness kernel, read from the raw csv export of a
+    committed `ncu --set full` capture (profiles/r03_traffic_index.csv names the export per workload and kernel and the
+    hash of the kernel sources it was taken on; the .md beside it gives the commands).  None -- with the reason -- when
+    there is no capture for this workload / kernel or when the kernels have changed since the capture was taken."""
+    if not TRAFFIC_INDEX.exists():
+        return None, f"no profiles/{TRAFFIC_INDEX.name}"
     sha = kernel_source_sha()
-    with TRAFFIC_CSV.open() as f:
+    with TRAFFIC_INDEX.open() as f:
         for row in csv.DictReader(f):
             if row["workload"] == workload_key and row["kernel"] == kernel_name:
                 if row["kernel_sha"] != sha:
-                    return None, f"capture {row['capture']} is older than the kernel sources ({row['kernel_sha']} != {sha})"
-                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]), f"profiles/{row['capture']}"
+                    return None, f"capture {row['raw_csv']} is older than the kernel sources ({row['kernel_sha']} != {sha})"
+                total = ncu_raw_metric_sum(ROOT / "profiles" / row["raw_csv"], "fitness_" + kernel_name,
+                                           ["dram__bytes_read.sum", "dram__bytes_write.sum"])
+                if total is None:
+                    return None, f"profiles/{row['raw_csv']} holds no fitness_{kernel_name} launch with the two dram metrics"
+                return total, f"profiles/{row['raw_csv']}"
     return None, "no capture for this workload and kernel"
 
 
@@ -158,7 +179,7 @@ def ncu_traffic(workload_key: str, kernel_name: str):
 # roofline of the fitness kernel
 # ----------------------------------------------------------------------------------------------------
 # L2 -> crossbar peak of this B200 as ncu states it: derived__lts__lts2xbar_bytes.sum.peak_sustained = 11,776 B/clk
-# (184 L2 slices x 64 B/clk; profiles/r01_fitness_pairbits_c4_ncu_full.txt), at the L2 clock == sm_max_mhz.
+# (184 L2 slices x 64 B/clk; that metric in profiles/r03_fitness_pairbits_c4_ncu_raw.csv), at the L2 clock == sm_max_mhz.
 L2_XBAR_BYTES_PER_CLK = 184 * 64
 
 
@@ -301,7 +322,24 @@ def best_kernel_without_table(B, eb):
     return B.EBIC_KERNEL_DIRECT
 
 
-def measure_workload(B, key, w, peaks, peaks_kind, probes, flush, reps, early_exit=0, with_alt=True):
+def back_to_back_ms(fn, reps):
+    """Mean of `reps` x 10 calls of fn() issued back to back on the current stream between ONE event pair: no L2 flush,
+    no host synchronisation in between -- generations of a GA loop, replayed from the library's captured graph."""
+    import torch
+    n = max(10, reps * 10)
+    for _ in range(3):
+        fn()
+    s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    s.record()
+    for _ in range(n):
+        fn()
+    e.record()
+    torch.cuda.synchronize()
+    return s.elapsed_time(e) / n
+
+
+def measure_workload(B, key, w, peaks, peaks_kind, probes, flush, reps, early_exit=0, with_alt=True, plain_work=False):
     """One `per_workload` entry: everything measured in this process on the workload `w`."""
     import torch
     t0 = time.time()
@@ -327,6 +365,19 @@ def measure_workload(B, key, w, peaks, peaks_kind, probes, flush, reps, early_ex
     torch.cuda.synchronize()
     kernel_name = B.KERNEL_NAMES[eb.last_kernel]
     step_ms, _ = timed_ms(step, reps, flush)                    # production configuration: no instrumentation
+    b2b_ms = back_to_back_ms(step, reps)                        # the regime a GA loop runs in: no flush, graph replay
+    # the configuration a caller gets without touching a knob (csrc/ebic_ctx.hpp: early exit on)
+    product_default = None
+    if not early_exit:
+        eb.set_early_exit(True)
+        for _ in range(3):
+            step()
+        pd_ms, _ = timed_ms(step, reps, flush)
+        product_default = {"early_exit": True, "kernel": B.KERNEL_NAMES[eb.last_kernel], "step_ms": pd_ms,
+                           "step_ms_back_to_back": back_to_back_ms(step, reps)}
+        eb.set_early_exit(False)
+        for _ in range(3):
+            step()
     eb.set_instrumentation(1)
     eval_only()
     visits = eb.info(10)
@@ -340,7 +391,9 @@ def measure_workload(B, key, w, peaks, peaks_kind, probes, flush, reps, early_ex
     roof = roofline(kernel_name, visits, kernel_ms * 1e-3, peaks, peaks_kind, eb.info(7), probes=probes,
                     traffic=traffic, traffic_source=traffic_src, pairs=pair_stats(w), ld=eb.ld, cols=w.cols)
     entry = {"workload": w.cfg.name, "rows": w.rows, "cols": w.cols, "n_ind": w.n_ind, "kernel": kernel_name,
-             "step_ms": step_ms, "kernel_ms": kernel_ms, "comparisons_per_s": w.comparisons / (step_ms * 1e-3),
+             "early_exit": bool(early_exit), "step_ms": step_ms, "step_ms_back_to_back": b2b_ms,
+             "product_default": product_default,
+             "kernel_ms": kernel_ms, "comparisons_per_s": w.comparisons / (step_ms * 1e-3),
              "bound": roof["bound"], "frac": roof["frac"], "achieved_gbs": roof["achieved"], "peak_gbs": roof["peak"],
              "create_ms": create_ms, "create_breakdown_ms": breakdown, "device_bytes": eb.info(9),
              "pair_table_bytes": eb.info(14), "pair_table_tile_major_bytes": eb.info(17)}
@@ -369,8 +422,61 @@ def measure_workload(B, key, w, peaks, peaks_kind, probes, flush, reps, early_ex
                                # faster per evaluation; None = the other kernel is at least as fast (tiny inputs)
                                "evals": max(0.0, (breakdown["pair_table"] - alt_build) / gain) if gain > 0 else None}
         eb.set_kernel(B.EBIC_KERNEL_AUTO)
+    # a1 on its own ("HBM: read + write once"): the same matrix already on the device, so that the
+    # transpose is timed without the host-to-device copy that dominates create_breakdown_ms.h2d_transpose_pad above
+    try:
+        d_m = torch.from_numpy(w.matrix).cuda()
+        torch.cuda.synchronize()
+        with B.Ebic(d_m, w.missing_mode) as eb_dev:
+            a1_ms = eb_dev.create_breakdown_ms()["h2d_transpose_pad"]
+        del d_m
+        a1_bytes = w.rows * w.cols * 4 + eb.ld * w.cols * 4
+        entry["a1_transpose"] = {"ms": a1_ms, "bytes": a1_bytes, "gbs": a1_bytes / (a1_ms * 1e-3) / 1e9,
+                                 "frac_of_hbm": a1_bytes / (a1_ms * 1e-3) / 1e9 / float(peaks["hbm_gbs"]),
+                                 "what": "transpose_pad_kernel (+ padding fill) from a device-resident row-major matrix: read + write once"}
+    except (RuntimeError, B.EbicError) as exc:                     # not enough memory for a second copy: say so
+        entry["a1_transpose"] = {"skipped": str(exc)[:120]}
+    # SURVEY.md 8(d) as written: the PLAIN work -- float32 values gathered from staged tiles and compared in the
+    # timed kernel, nothing memoised, early exit off -- on the configurations the 60 % target is graded on
+    if plain_work and kernel_name != "tiled_f32":
+        try:
+            eb.set_kernel(B.EBIC_KERNEL_TILED_F32)
+        except B.EbicError:
+            plain_work = False
+    if plain_work:
+        eb.set_early_exit(False)
+        for _ in range(2):
+            eval_only()
+        eb.set_instrumentation(1)
+        eval_only()
+        pw_visits = eb.info(10)
+        eb.set_instrumentation(2)
+        timed_ms(eval_only, max(3, reps // 2), flush)
+        pw_ms = eb.info(11) / 1e6
+        eb.set_instrumentation(0)
+        pw = roofline("tiled_f32", pw_visits, pw_ms * 1e-3, peaks, peaks_kind, eb.info(7), probes=probes, ld=eb.ld, cols=w.cols)
+        entry["plain_work"] = {"kernel": "tiled_f32", "early_exit": False, "kernel_ms": pw_ms, "visits_executed": pw_visits,
+                               "bytes_per_visit": 4, "bound": pw["bound"], "achieved_gbs": pw["achieved"],
+                               "peak_gbs": pw["peak"], "frac": pw["frac"],
+                               "comparisons_per_s": w.comparisons / (pw_ms * 1e-3),
+                               "what": "float32 value visits x 4 B / kernel time / shared-memory pipe peak (SURVEY.md 8(d) as written)"}
+        eb.set_kernel(B.EBIC_KERNEL_AUTO)
     eb.close()
     return entry, roof
+
+
+def work_model(kernel_name, breakdown, create_ms, ms_per_step):
+    """In words, what `value` counts (the judge's request: the line must say when the comparisons are memoised)."""
+    if kernel_name in ("pairbits", "pairtile", "prefix"):
+        return (f"nominal comparisons rows x sum(L-1) per step; the float32 compares are MEMOISED: executed once per "
+                f"dataset in ebic_create (pair-table kernel {breakdown['pair_table']:.3f} ms of create_ms {create_ms:.1f} ms, "
+                f"outside the timed step), the timed {kernel_name} kernel ANDs one bit per (row, pair) -- dtype u32, "
+                f"0.125 B per visit.  The plain float32 work of SURVEY.md 8(d) (4 B per value visit, TILED_F32) is "
+                f"per_workload[*].plain_work; value_amortised charges create_ms to 1,000 generations")
+    if kernel_name == "rank8":
+        return ("nominal comparisons per step on 8-bit dense ranks built once per dataset in ebic_create "
+                f"(rank tiles {breakdown['rank_tiles']:.3f} ms): 1 B per value visit")
+    return "nominal comparisons per step, float32 values compared in the timed kernel: 4 B per value visit"
 
 
 # ----------------------------------------------------------------------------------------------------
@@ -388,7 +494,7 @@ def rank_matrix(w, idx, rank, world, scaling):
         return np.ascontiguousarray(w.matrix[b:e]), w.rows
     if rank > 0:
         rng = np.random.default_rng([5, idx, rank])
-        m = W._draw_matrix(rng, w.cfg.dist, w.rows, w.cols)
+        m = W.draw_matrix(rng, w.cfg.dist, w.rows, w.cols)
         if w.cfg.nan_rate > 0:
             for r0 in range(0, w.rows, 1 << 20):
                 blk = m[r0:r0 + (1 << 20)]
@@ -583,6 +689,9 @@ def run_gpu(args):
                                        if world > 1 else "1 GPU"),
                        **({"functional_check_only": "all ranks on one GPU: timings are not measurements"}
                           if args.one_device and world > 1 else {})},
+            "work_model": work_model(kernel_name, breakdown, create_ms, ms_per_step),
+            "value_amortised": {"generations": 1000, "value": comparisons * 1000 / ((1000 * ms_per_step + create_ms) * 1e-3),
+                                "unit": UNIT, "includes": "ebic_create from the host matrix (create_ms, wall clock) + 1,000 steps"},
             "individuals_rows_per_s": w.n_ind * (w.rows if scaling == "strong" else w.rows * world) / (ms_per_step * 1e-3),
             "clocks": clk.summary(),
             "e2e": {"value": comparisons / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -610,7 +719,7 @@ def run_gpu(args):
                 wk = w if key == args.workload and args.rows is None and args.n_ind is None else W.make_workload(WORKLOADS[key])
                 reps = 5 if wk.comparisons > 1e11 else 20
                 entry, _ = measure_workload(B, key, wk, peaks, peaks_kind, probes, flushed, reps,
-                                            early_exit=args.early_exit)
+                                            early_exit=args.early_exit, plain_work=key in ("c3", "c4", "c5"))
                 entry["wall_s"] = time.time() - t0
                 per.append(entry)
                 log(json.dumps(entry))
@@ -622,6 +731,9 @@ def run_gpu(args):
                                   for e in per if e["workload"].startswith("P")]
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(w, budget_s=args.cpu_budget)
+            # "Single-thread time also reported for C1-C3"
+            out["cpu_baseline"]["single_thread"] = [cpu_baseline(W.make_workload(WORKLOADS[k]), budget_s=2.0, n_threads=1)
+                                                    for k in ("c1", "c2", "c3")]
     if world > 1:
         dist.destroy_process_group()
     return out
@@ -643,21 +755,26 @@ def oracle_sample(w, n_sample, seed=0):
     return off, ids, comparisons
 
 
-def cpu_baseline(w, budget_s=15.0):
+def cpu_baseline(w, budget_s=15.0, n_threads=0):
+    """The oracle as it stands on the host cores (n_threads = 0: all of them; 1: a single thread)."""
     import oracle
-    cores = oracle.max_threads()
+    cores = n_threads if n_threads > 0 else oracle.max_threads()
     # calibrate on a few individuals, then size the sample to ~budget_s of CPU work
     off, ids, comps = oracle_sample(w, max(8, cores), seed=1)
     t0 = time.perf_counter()
-    oracle.eval_fitness(w.matrix, w.missing_mode, off, ids)
+    oracle.eval_fitness(w.matrix, w.missing_mode, off, ids, n_threads=n_threads)
     rate = comps / max(time.perf_counter() - t0, 1e-6)
     n = int(min(w.n_ind, max(cores, budget_s * rate / max(w.comparisons / w.n_ind, 1))))
     off, ids, comps = oracle_sample(w, n, seed=2)
     t0 = time.perf_counter()
-    oracle.eval_fitness(w.matrix, w.missing_mode, off, ids)
+    oracle.eval_fitness(w.matrix, w.missing_mode, off, ids, n_threads=n_threads)
     dt = time.perf_counter() - t0
-    return {"value": comps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{n} of {w.n_ind} individuals x all {w.rows} rows, {comps:.3e} comparisons in {dt:.2f} s"}
+    out = {"value": comps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"{n} of {w.n_ind} individuals x all {w.rows} rows, {comps:.3e} comparisons in {dt:.2f} s"}
+    if n_threads > 0:
+        out["workload"] = w.cfg.name
+        out["whole_evaluation_s"] = w.comparisons / (comps / dt)      # extrapolated from the sample's rate
+    return out
 
 
 def run_reference(args):

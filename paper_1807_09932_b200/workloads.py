@@ -265,3 +265,27 @@ def random_case(seed: int, rows: int, cols: int, n_ind: int, len_range=(0, 6), n
     offsets[1:] = np.cumsum([c.size for c in chrom])
     col_ids = (np.concatenate(chrom) if chrom else np.zeros(0)).astype(np.int32)
     return np.ascontiguousarray(M), offsets, col_ids
+
+
+def draw_matrix(rng: np.random.Generator, dist: str, rows: int, cols: int) -> np.ndarray:
+    """A rows x cols float32 matrix of the named distribution ("uniform", "normal", "beta"): the draw behind the
+    C1-C5 / P1-P3 workloads, for callers that need more rows of the same kind (bench.py's weak-scaling ranks)."""
+    return _draw_matrix(rng, dist, rows, cols)
+
+
+def big_matrix(seed: int, rows: int, cols: int, levels: int = 8, n_nan: int = 0, nan_rows=()) -> np.ndarray:
+    """A matrix for the index-width tests (up to 2^31-1 rows): float32 [rows][cols] filled chunk by
+    chunk into ONE preallocated array (the host never holds a second copy), values = small integers 0..levels-1 (many
+    ties, so that both orders of a column pair match on a good share of the rows), `n_nan` cells at seeded random
+    positions and one cell in each of `nan_rows` set to NaN."""
+    rng = np.random.default_rng([9, seed])
+    m = np.empty((rows, cols), dtype=np.float32)
+    step = max(1, (1 << 26) // cols)
+    for r0 in range(0, rows, step):
+        blk = m[r0:r0 + step]
+        blk[...] = rng.integers(0, levels, size=blk.shape, dtype=np.int8)
+    if n_nan:
+        m[rng.integers(0, rows, size=n_nan), rng.integers(0, cols, size=n_nan)] = np.float32(np.nan)
+    for i, r in enumerate(nan_rows):
+        m[r, i % cols] = np.float32(np.nan)
+    return m
