@@ -641,6 +641,11 @@ def run_gpu(args):
     d2h = int(h_counts.numel() * 8 + h_masks.numel() * 8 + h_mcnt.numel() * 8)
     if world == 1:
         assert (h_counts.numpy() == d_counts.cpu().numpy()).all()
+    # fingerprint of the step's result (whole-matrix counts, after the all-reduce when N > 1): lets a test compare a
+    # bench run with the oracle without bench.py touching the oracle itself
+    d_counts, _ = step()
+    torch.cuda.synchronize()
+    counts_sha = hashlib.sha256(d_counts.cpu().numpy().astype(np.uint64).tobytes()).hexdigest()[:16]
 
     # ---- PAPER.md Fig. 1 shapes (12,483 / 54,675 / 436,444 rows) on this many GPUs, strong split (N > 1 only;
     #      at N = 1 the per_workload block holds them)
@@ -699,6 +704,7 @@ def run_gpu(args):
                     "how": "one ebic_eval_extract call with pinned host buffers: population in, counts + masks out (the masks are extracted first and copied back on a second stream while the fitness kernel runs)"},
             "gpu_launches": int(launches_per_step * args.steps),
             "gpu_launches_per_step": int(launches_per_step),
+            "counts_sha256_16": counts_sha,
             "roofline": roof,
             "probes": probes.as_dict(),
             "ms_per_step_without_kernel_events": plain_ms,

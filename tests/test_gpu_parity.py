@@ -896,6 +896,36 @@ def test_sharded_step_reuses_its_outputs(B, oracle_mod):
         sh.close()
 
 
+def test_bench_two_ranks_on_one_device(oracle_mod):
+    """The N > 1 branch of bench.py (row shards, ShardedEbic.step, the all-reduce, the rank-0 line) as two gloo ranks
+    that share this one GPU: exit code 0, one JSON line, and the fingerprint of the all-reduced counts equals the
+    oracle's counts on the unsharded matrix.  Timings of such a run mean nothing and are not looked at."""
+    import hashlib
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parent.parent
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), str(root / "bench.py"), "--gpus", "2", "--dist-backend", "gloo", "--one-device",
+           "--workload", "c3", "--steps", "2", "--warmup", "3", "--no-per-workload", "--no-cpu-baseline"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=root, env=dict(os.environ))
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [ln for ln in res.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, res.stdout[-2000:]
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["scaling"] == "strong" and "functional_check_only" in out["config"]
+    w = W.make_workload(2)
+    st, want = oracle_mod.eval_fitness(w.matrix, w.missing_mode, w.offsets, w.col_ids)
+    assert st == 0
+    assert out["counts_sha256_16"] == hashlib.sha256(want.astype(np.uint64).tobytes()).hexdigest()[:16]
+
+
 # ------------------------------------------------------------------------- full sizes against the oracle
 @pytest.mark.parametrize("index", [6, 7])
 def test_paper_shapes_full_size(B, oracle_mod, index):
