@@ -981,8 +981,54 @@ def render_table(path):
     return "\n".join(out)
 
 
+def run_knob_sweep(args):
+    """--sweep-knob K:v1,v2,...  One JSON row per (workload of --per-workload, value of ebic_set_tuning knob K): production
+    step with the L2 flushed, the same steps back to back, and the event-bracketed fitness kernel; counts of every
+    setting must equal the first setting's.  This is how the tuning defaults are (re-)derived from a tracked command."""
+    import torch
+    from paper_1807_09932_b200 import binding as B
+    knob, values = args.sweep_knob.split(":")
+    knob, values = int(knob), [int(v) for v in values.split(",")]
+    torch.cuda.set_stream(torch.cuda.Stream())
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for key in [k for k in args.per_workload.split(",") if k]:
+        w = W.make_workload(WORKLOADS[key])
+        eb = B.Ebic(w.matrix, w.missing_mode)
+        eb.set_kernel(KERNELS[args.kernel])
+        eb.set_early_exit(bool(args.early_exit))
+        chosen = pick_chosen(w)
+        d_off, d_ids, d_ch = (torch.from_numpy(a).cuda() for a in (w.offsets, w.col_ids, chosen))
+        counts = torch.empty(w.n_ind, dtype=torch.int64, device="cuda")
+        masks = torch.empty((len(chosen), eb.mask_words), dtype=torch.int64, device="cuda")
+        mcnt = torch.empty(len(chosen), dtype=torch.int64, device="cuda")
+        step = lambda: eb.eval_extract(d_off, d_ids, d_ch, counts=counts, masks=masks, mask_counts=mcnt)   # noqa: E731
+        eval_only = lambda: eb.eval_fitness(d_off, d_ids, counts=counts)                                   # noqa: E731
+        first = None
+        for v in values:
+            eb.set_tuning(knob, v)
+            for _ in range(3):
+                step()
+            torch.cuda.synchronize()
+            got = counts.cpu().numpy().copy()
+            first = got if first is None else first
+            assert (got == first).all(), (key, knob, v)
+            step_ms = [timed_ms(step, args.steps, flush)[0] for _ in range(3)]
+            b2b = back_to_back_ms(step, args.steps)
+            eb.set_instrumentation(2)
+            timed_ms(eval_only, args.steps, flush)
+            kernel_ms = eb.info(11) / 1e6
+            eb.set_instrumentation(0)
+            print(json.dumps({"workload": w.cfg.name, "kernel": B.KERNEL_NAMES[eb.last_kernel], "knob": knob, "value": v,
+                              "step_us_3_medians": [round(x * 1e3, 2) for x in step_ms],
+                              "step_us_back_to_back": round(b2b * 1e3, 2), "kernel_us": round(kernel_ms * 1e3, 2)}), flush=True)
+        eb.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
+    ap.add_argument("--sweep-knob", default=None, dest="sweep_knob", metavar="K:v1,v2,...",
+                    help="sweep ebic_set_tuning knob K (include/ebic_debug.h) over the values on the --per-workload list; "
+                         "one JSON row per setting on stdout")
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
@@ -1017,6 +1063,9 @@ def main():
     args = ap.parse_args()
     if args.render_table:
         print(render_table(args.render_table))
+        return
+    if args.sweep_knob:
+        run_knob_sweep(args)
         return
     if args.warmup < 3 and args.impl == "ebic" and not args.table:
         log("note: fewer than 3 warm-up steps requested; using 3 (timing rules)")

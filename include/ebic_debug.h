@@ -73,6 +73,9 @@ int ebic_set_early_exit(ebic_ctx *ctx, int32_t on);
  *      stated at EBIC_KERNEL_AUTO)
  *   8  PAIRBITS row chunks requested into L2 by the kernel's prologue (default 1; 1..16, at least the distance)
  *   9  replay a repeated all-device call from a captured CUDA graph (default 1; include/ebic.h, ebic_eval_extract)
+ *  10  PAIRBITS on a sparse population (fewer pair uses than 2 * cols^2): bytes of every bit column a record names
+ *      that the ingest kernel requests into L2 ahead of the fitness kernel (multiple of 16, <= 1 MiB, capped at one
+ *      column; 0 = off; DESIGN.md 6.4 gives the measurement behind the default)
  * EBIC_ERR_ARG for an unknown knob or a value outside its range.
  */
 int ebic_set_tuning(ebic_ctx *ctx, int32_t knob, int32_t value);

@@ -40,7 +40,7 @@ KERNEL_NAMES = {0: "auto", 1: "direct", 2: "tiled_f32", 3: "rank8", 4: "pairbits
                 7: "pairtile"}
 # ebic_set_tuning knobs (include/ebic_debug.h)
 (TUNE_PB_TASKS_PER_SLOT, TUNE_PB_PREFETCH, TUNE_PB_SMEM_RING, TUNE_SORT, TUNE_PDL, TUNE_UNION_BATCH, TUNE_PT_BUILD,
- TUNE_PT_MIN_WORK, TUNE_PB_PROLOGUE_CHUNKS, TUNE_GRAPHS) = range(10)
+ TUNE_PT_MIN_WORK, TUNE_PB_PROLOGUE_CHUNKS, TUNE_GRAPHS, TUNE_PB_INGEST_PREFETCH) = range(11)
 
 LIB_PATH = Path(__file__).resolve().parent / "libebic.so"
 

@@ -516,6 +516,10 @@ int eval_device(ebic_ctx* ctx, const int32_t* offsets, const int32_t* col_ids, i
     ip.pair_stride16 = static_cast<uint32_t>(ctx->ld / 128);
     ip.counts = counts;
     ip.err = ctx->d_err;
+    if (by_pairs && !by_prefix && ctx->pb_ingest_prefetch > 0 && !pairbits_dense(ctx, n_ind, n_ids)) {
+        ip.PB = ctx->PB;
+        ip.prefetch_bytes = static_cast<uint32_t>(std::min<int64_t>(ctx->ld / 8, ctx->pb_ingest_prefetch)) & ~15u;
+    }
     ingest_population_kernel<<<(n_ind + kIngestBlock - 1) / kIngestBlock, kIngestThreads, 0, stream>>>(ip);
     ctx->launches++;
     EBIC_TRY(cudaGetLastError());

@@ -67,6 +67,7 @@ struct ebic_ctx {
     int32_t pt_build = 1;                      // build the tile-major copy of the pair table when a tile fits shared memory
     int32_t pt_min_work = 0;                   // AUTO picks PAIRTILE from this many (tile, pair-use) units on (0 = the rule of pairtile_pays)
     int32_t pb_sort = 1;                       // ingest sorts each 64-individual block by length
+    int32_t pb_ingest_prefetch = 0;            // PAIRBITS, sparse populations: bytes of every used bit column the ingest requests into L2 (0 = off)
     int32_t pdl = 1;                           // programmatic dependent launch between ingest / fitness / extraction
     int32_t union_batch = 0;                   // UNION_F32: individuals per batch (0 = chosen from the shape)
     int32_t count_visits = 0;

@@ -92,6 +92,10 @@ int ebic_set_tuning(ebic_ctx* ctx, int32_t knob, int32_t value) {
             ctx->pb_prologue_chunks = value;
             return EBIC_OK;
         case 9: ctx->use_graphs = value ? 1 : 0; return EBIC_OK;
+        case 10:
+            if (value < 0 || value > (1 << 20) || (value & 15)) return EBIC_ERR_ARG;
+            ctx->pb_ingest_prefetch = value;
+            return EBIC_OK;
         default: return EBIC_ERR_ARG;
     }
 }

@@ -46,6 +46,12 @@ struct IngestParams {
     uint32_t pair_stride16;          // 16-byte units per bit column = ld / 128
     unsigned long long* counts;
     int32_t* err;
+    // Sparse populations on the pair table (a wide matrix: the population uses a small part of the cols^2 bit columns,
+    // so the fitness kernel's prologue cannot afford to request all of them): the ingest, which forms every pair
+    // offset anyway, asks L2 for the first `prefetch_bytes` of each bit column a record names (0 = off).  The fitness
+    // kernel then finds its first loads in L2, or on their way, instead of starting a chain of HBM misses.
+    const uint32_t* PB = nullptr;
+    uint32_t prefetch_bytes = 0;     // multiple of 16, at most one bit column (ld / 8)
 };
 
 __global__ void __launch_bounds__(kIngestThreads)
@@ -127,6 +133,8 @@ ingest_population_kernel(const IngestParams p)
             if (lane == 0) v = bad ? 0xffffffffu : static_cast<uint32_t>(L);
             if (lane == 1) v = static_cast<uint32_t>(k);
             p.prec[32 * j + lane] = v;                      // one coalesced 128-byte store
+            if (p.prefetch_bytes != 0 && !bad && lane >= 2 && lane - 2 < L - 1)      // one request per pair of the record
+                bulk_prefetch_l2(reinterpret_cast<const unsigned char*>(p.PB) + static_cast<int64_t>(v) * 16, p.prefetch_bytes);
         }
         if (lane != 0) continue;
         if (bad) {
